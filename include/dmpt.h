@@ -1,0 +1,129 @@
+/*
+ * dmpt.h - C ABI of the B200-native DNN-SP2-PT hot path (arXiv 2203.09621).
+ *
+ * The library computes, for a symmetric (already orthogonalised) Hamiltonian H0,
+ * a symmetric perturbation H1 and an occupation count N_occ,
+ *
+ *     D0 = theta(mu I - H0),  Tr D0 = N_occ                       PAPER.md:72 (Eq. 5), 81
+ *     D1 = d theta(mu I - (H0 + lambda H1)) / d lambda at 0        PAPER.md:164 (Eq. 20), 352 (Eq. 49)
+ *
+ * by the deep-layer recursion of Algorithms 1-3: per layer
+ *     X0 = S0^2,  X1 = S0 S1 + S1 S0                               PAPER.md:497-499, Eqs. 25-26
+ *     S0 <- sigma X0 + (1 - sigma) S0,  S1 <- sigma X1 + (1 - sigma) S1     Eqs. 23, 25
+ * with every product taken in the dual half-precision representation A ~ A_hi + A_lo (both fp16),
+ * A.B ~ A_hi.B_hi + A_hi.B_lo + A_lo.B_hi, fp32 accumulation, sigma_n
+ * chosen by the trace criterion and both parameter-free stopping tests
+ * (Eq. 78) evaluated on the device.
+ *
+ * Conventions
+ *   - All matrices are row-major fp32 with a leading dimension in ELEMENTS (they are symmetric,
+ *     so row-major == column-major).  "d_" arguments are DEVICE pointers, "h_" arguments HOST
+ *     pointers.  The library never frees caller memory and allocates no device memory itself:
+ *     the caller provides one workspace of dmpt_workspace_bytes() bytes (256-byte aligned).
+ *   - Every kernel is enqueued on the cudaStream_t given to dmpt_create(); dmpt_run() returns
+ *     after that stream has drained (it polls a pinned flag between chunks of layers; there is no
+ *     host round trip per layer).
+ *   - All functions return 0 on success or a negative DMPT_E* code; dmpt_strerror() describes it.
+ *     There is no CPU fallback: without a CUDA device every compute call fails with DMPT_ECUDA.
+ */
+#ifndef DMPT_H
+#define DMPT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DMPT_OK            0
+#define DMPT_EINVAL       -1   /* null pointer, n <= 0, n_occ outside (0, n), ld < n, order not 1|2   */
+#define DMPT_ESTATE       -2   /* dmpt_run before dmpt_set_hamiltonian                                */
+#define DMPT_ECUDA        -3   /* CUDA error (text via dmpt_strerror / dmpt_last_cuda_error)          */
+#define DMPT_EDEGENERATE  -4   /* eps_max - eps_min not positive and finite                           */
+#define DMPT_ENOCONV      -5   /* max_layers reached; outputs hold the last iterate                   */
+#define DMPT_ENUMERIC     -6   /* NaN/Inf in the scalar state, or fp16 overflow of a scaled iterate   */
+#define DMPT_EWORKSPACE   -7   /* workspace too small or misaligned                                   */
+
+typedef struct dmpt_ctx dmpt_ctx;
+
+typedef struct dmpt_options {
+    int max_layers;    /* cap on the while loop of Algorithm 1 (the paper has none); default 200       */
+    int order;         /* 1: D0, D1.  2: also D2 (Eq. 25 third line)                    */
+    int s0_shift;      /* a >= 0: S0 is split as hi = fp16(2^a S0), lo = fp16(2^a S0 - hi) and 2^-2a   */
+                       /* is folded back in fp32 (exact).  0 = Eq. 13 verbatim.  -1 = default (14).    */
+    int s1_autoscale;  /* 1 (default): the response iterates are split after an exact power-of-two     */
+                       /* scale chosen on the device per layer from max|S1|; 0 = Eq. 43 verbatim.      */
+    int bounds;        /* 0: Gershgorin discs of H0; 1: eps_min/eps_max below       */
+    double eps_min;    /* read only when bounds == 1                                                  */
+    double eps_max;
+    int reserved[8];   /* must be 0                                                                   */
+} dmpt_options;
+
+typedef struct dmpt_result {
+    int status;        /* same as the return code of dmpt_run                                         */
+    int layers;        /* passes of the while loop of Algorithm 1                  */
+    int layers_d0;     /* layer at which the D0 test fired (Algorithm 2); 0 if it never did           */
+    int layers_d1;     /* layer at which the D1 test fired (Algorithm 3); 0 if it never did           */
+    int launches;      /* kernels this run launched (all of them this library's own)                  */
+    int reserved_i[3];
+    double eps_min, eps_max;   /* spectral bounds used                                 */
+    double fro_err0;           /* FroErr0 = ||S0 - S0^2||_F at the D0 stop layer        */
+    double ms_total;           /* CUDA-event time of the whole run (bounds + transform + split + loop) */
+    double ms_loop;            /* CUDA-event time of the layer loop alone ("time for main loop", Eq. 82)*/
+    double reserved_d[4];
+    /* Per-layer records, entry n-1 for layer n.  Caller-allocated HOST arrays of max_layers
+     * entries each, or NULL to skip.  Entries the run did not reach are left untouched. */
+    int8_t *sigma;             /* sigma_n                                         */
+    double *tr_s;              /* N_S = Tr S0_{n-1} entering layer n                                  */
+    double *tr_x;              /* N_X = Tr (S0_{n-1})^2, evaluated as ||S0_{n-1}||_F^2 (R9) */
+    double *id_err;            /* IdErr_n = N_S - N_X; NaN once S0 froze                              */
+    double *fro_err1;          /* FroErr1_n; NaN before D0 converged                   */
+    double *fro_err2;          /* FroErr2_n (order 2); NaN before D1 converged                        */
+} dmpt_result;
+
+/* Defaults: max_layers 200, order 1, s0_shift -1, s1_autoscale 1, bounds 0. */
+void dmpt_default_options(dmpt_options *opt);
+
+/* Bytes of device workspace dmpt_create() needs for matrices of size n at response order `order`
+ * (0 on invalid arguments).  Layout is private; see DESIGN.md "HBM layout". */
+size_t dmpt_workspace_bytes(int n, int order);
+
+/* Create a context for n x n problems.  `d_workspace` (device, >= dmpt_workspace_bytes(), 256-byte
+ * aligned) stays owned by the caller and must outlive the context.  `cuda_stream` is a cudaStream_t
+ * (NULL = the legacy default stream).  `opt` may be NULL for defaults. */
+int dmpt_create(dmpt_ctx **ctx, int n, const dmpt_options *opt,
+                void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Register the problem: symmetric d_h0, d_h1 (device, fp32, leading dimension ld >= n) and n_occ in
+ * (0, n).  The pointers are read by every later dmpt_run and must stay valid until then; symmetry
+ * is a precondition and is not checked. */
+int dmpt_set_hamiltonian(dmpt_ctx *ctx, const float *d_h0, const float *d_h1, int ld, int n_occ);
+
+/* Run Algorithms 1-3 and write D0, D1 (and D2 when order == 2, else pass NULL) to device matrices
+ * with leading dimension ld >= n.  `res` may be NULL.  On DMPT_ENOCONV the outputs hold the last
+ * iterate.  Safe to call repeatedly. */
+int dmpt_run(dmpt_ctx *ctx, float *d_d0, float *d_d1, float *d_d2, int ld, dmpt_result *res);
+
+/* The same call with HOST matrices (pinned memory recommended): copies H0, H1 to the device, runs,
+ * and copies D0, D1 (D2) back, all on the context's stream.  ms_total then covers the copies too. */
+int dmpt_run_host(dmpt_ctx *ctx, const float *h_h0, const float *h_h1, int ld_in, int n_occ,
+                  float *h_d0, float *h_d1, float *h_d2, int ld_out, dmpt_result *res);
+
+/* One dual-half product on its own (used by tests and micro-benchmarks of the layer kernel):
+ * given symmetric device matrices S0, S1 (fp32, leading dimension ld), writes X0 = S0^2 and
+ * X1 = S0 S1 + S1 S0 through exactly the split + tcgen05 path a layer takes (sigma = +1, no
+ * stopping test).  Uses the context's workspace; invalidates nothing the caller owns. */
+int dmpt_layer_products(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, int ld,
+                        float *d_x0, float *d_x1, int ld_out);
+
+int dmpt_destroy(dmpt_ctx *ctx);
+
+const char *dmpt_strerror(int code);
+/* Text of the last CUDA error seen by this context (empty string if none). */
+const char *dmpt_last_cuda_error(const dmpt_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DMPT_H */

@@ -1,0 +1,281 @@
+"""ctypes binding of include/dmpt.h: same names, argument marshalling only.
+
+`lib()` loads the in-tree `libdmpt.so` and fails loudly when it is missing (build it with
+`python -m paper_2203_09621_b200.build` or `__graft_entry__.build()`); nothing here computes.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass, field
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdmpt.so")
+
+EXPORTED_SYMBOLS = (
+    "dmpt_default_options", "dmpt_workspace_bytes", "dmpt_create", "dmpt_set_hamiltonian",
+    "dmpt_run", "dmpt_run_host", "dmpt_layer_products", "dmpt_destroy", "dmpt_strerror",
+    "dmpt_last_cuda_error",
+)
+
+DMPT_OK, DMPT_EINVAL, DMPT_ESTATE, DMPT_ECUDA = 0, -1, -2, -3
+DMPT_EDEGENERATE, DMPT_ENOCONV, DMPT_ENUMERIC, DMPT_EWORKSPACE = -4, -5, -6, -7
+
+
+class DmptOptions(C.Structure):
+    _fields_ = [
+        ("max_layers", C.c_int), ("order", C.c_int), ("s0_shift", C.c_int),
+        ("s1_autoscale", C.c_int), ("bounds", C.c_int),
+        ("eps_min", C.c_double), ("eps_max", C.c_double),
+        ("reserved", C.c_int * 8),
+    ]
+
+
+class _CResult(C.Structure):
+    _fields_ = [
+        ("status", C.c_int), ("layers", C.c_int), ("layers_d0", C.c_int), ("layers_d1", C.c_int),
+        ("launches", C.c_int), ("reserved_i", C.c_int * 3),
+        ("eps_min", C.c_double), ("eps_max", C.c_double), ("fro_err0", C.c_double),
+        ("ms_total", C.c_double), ("ms_loop", C.c_double), ("reserved_d", C.c_double * 4),
+        ("sigma", C.POINTER(C.c_int8)), ("tr_s", C.POINTER(C.c_double)), ("tr_x", C.POINTER(C.c_double)),
+        ("id_err", C.POINTER(C.c_double)), ("fro_err1", C.POINTER(C.c_double)),
+        ("fro_err2", C.POINTER(C.c_double)),
+    ]
+
+
+class DmptError(RuntimeError):
+    def __init__(self, code, where, detail=""):
+        self.code = code
+        msg = f"{where}: {dmpt_strerror(code)} ({code})"
+        if detail:
+            msg += f" - {detail}"
+        super().__init__(msg)
+
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library.  Raises if it has not been built: there is no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} is missing: build the CUDA extension first "
+                "(python -m paper_2203_09621_b200.build). There is no CPU fallback.")
+        L = C.CDLL(LIB_PATH)
+        L.dmpt_default_options.argtypes = [C.POINTER(DmptOptions)]
+        L.dmpt_default_options.restype = None
+        L.dmpt_workspace_bytes.argtypes = [C.c_int, C.c_int]
+        L.dmpt_workspace_bytes.restype = C.c_size_t
+        L.dmpt_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.POINTER(DmptOptions), C.c_void_p,
+                                  C.c_size_t, C.c_void_p]
+        L.dmpt_create.restype = C.c_int
+        L.dmpt_set_hamiltonian.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int]
+        L.dmpt_set_hamiltonian.restype = C.c_int
+        L.dmpt_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(_CResult)]
+        L.dmpt_run.restype = C.c_int
+        L.dmpt_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p,
+                                    C.c_void_p, C.c_void_p, C.c_int, C.POINTER(_CResult)]
+        L.dmpt_run_host.restype = C.c_int
+        L.dmpt_layer_products.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
+                                          C.c_void_p, C.c_int]
+        L.dmpt_layer_products.restype = C.c_int
+        L.dmpt_destroy.argtypes = [C.c_void_p]
+        L.dmpt_destroy.restype = C.c_int
+        L.dmpt_strerror.argtypes = [C.c_int]
+        L.dmpt_strerror.restype = C.c_char_p
+        L.dmpt_last_cuda_error.argtypes = [C.c_void_p]
+        L.dmpt_last_cuda_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+# ------------------------------------------------------------------ same-name thin wrappers
+def dmpt_default_options() -> DmptOptions:
+    o = DmptOptions()
+    lib().dmpt_default_options(C.byref(o))
+    return o
+
+
+def dmpt_workspace_bytes(n: int, order: int = 1) -> int:
+    return int(lib().dmpt_workspace_bytes(int(n), int(order)))
+
+
+def dmpt_strerror(code: int) -> str:
+    return lib().dmpt_strerror(int(code)).decode()
+
+
+def dmpt_last_cuda_error(ctx) -> str:
+    return lib().dmpt_last_cuda_error(ctx).decode()
+
+
+def dmpt_create(n: int, opt: DmptOptions | None, workspace_ptr: int, workspace_bytes: int, stream_ptr: int = 0):
+    h = C.c_void_p()
+    rc = lib().dmpt_create(C.byref(h), int(n), C.byref(opt) if opt is not None else None,
+                           C.c_void_p(workspace_ptr), int(workspace_bytes), C.c_void_p(stream_ptr))
+    if rc != DMPT_OK:
+        raise DmptError(rc, "dmpt_create")
+    return h
+
+
+def dmpt_set_hamiltonian(ctx, h0_ptr: int, h1_ptr: int, ld: int, n_occ: int) -> None:
+    rc = lib().dmpt_set_hamiltonian(ctx, C.c_void_p(h0_ptr), C.c_void_p(h1_ptr), int(ld), int(n_occ))
+    if rc != DMPT_OK:
+        raise DmptError(rc, "dmpt_set_hamiltonian")
+
+
+def dmpt_run(ctx, d0_ptr: int, d1_ptr: int, d2_ptr: int, ld: int, res: _CResult | None) -> int:
+    return int(lib().dmpt_run(ctx, C.c_void_p(d0_ptr), C.c_void_p(d1_ptr), C.c_void_p(d2_ptr or None),
+                              int(ld), C.byref(res) if res is not None else None))
+
+
+def dmpt_run_host(ctx, h0_ptr, h1_ptr, ld_in, n_occ, d0_ptr, d1_ptr, d2_ptr, ld_out, res) -> int:
+    return int(lib().dmpt_run_host(ctx, C.c_void_p(h0_ptr), C.c_void_p(h1_ptr), int(ld_in), int(n_occ),
+                                   C.c_void_p(d0_ptr), C.c_void_p(d1_ptr), C.c_void_p(d2_ptr or None),
+                                   int(ld_out), C.byref(res) if res is not None else None))
+
+
+def dmpt_layer_products(ctx, s0_ptr, s1_ptr, ld, x0_ptr, x1_ptr, ld_out) -> int:
+    return int(lib().dmpt_layer_products(ctx, C.c_void_p(s0_ptr), C.c_void_p(s1_ptr), int(ld),
+                                         C.c_void_p(x0_ptr), C.c_void_p(x1_ptr), int(ld_out)))
+
+
+def dmpt_destroy(ctx) -> None:
+    lib().dmpt_destroy(ctx)
+
+
+# ------------------------------------------------------------------ convenience object
+@dataclass
+class DmptResult:
+    status: int
+    layers: int
+    layers_d0: int
+    layers_d1: int
+    launches: int
+    eps_min: float
+    eps_max: float
+    fro_err0: float
+    ms_total: float
+    ms_loop: float
+    sigma: list = field(default_factory=list)
+    tr_s: list = field(default_factory=list)
+    tr_x: list = field(default_factory=list)
+    id_err: list = field(default_factory=list)
+    fro_err1: list = field(default_factory=list)
+    d0: object = None
+    d1: object = None
+    d2: object = None
+
+
+class Dmpt:
+    """Owns a dmpt_ctx plus the torch-allocated workspace.  Marshalling only."""
+
+    def __init__(self, n, order=1, max_layers=200, s0_shift=-1, s1_autoscale=True, bounds=None,
+                 device="cuda:0", stream=None):
+        import torch
+
+        self.torch = torch
+        self.n = int(n)
+        self.order = int(order)
+        self.device = torch.device(device)
+        if self.device.type != "cuda":
+            raise DmptError(DMPT_ECUDA, "Dmpt", "a CUDA device is required; there is no CPU path")
+        opt = dmpt_default_options()
+        opt.max_layers = int(max_layers)
+        opt.order = self.order
+        opt.s0_shift = int(s0_shift)
+        opt.s1_autoscale = 1 if s1_autoscale else 0
+        if bounds is not None:
+            opt.bounds = 1
+            opt.eps_min, opt.eps_max = float(bounds[0]), float(bounds[1])
+        self.max_layers = opt.max_layers
+        nbytes = dmpt_workspace_bytes(self.n, self.order)
+        if nbytes == 0:
+            raise DmptError(DMPT_EINVAL, "dmpt_workspace_bytes")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.ctx = dmpt_create(self.n, opt, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream)
+        self._h = None
+
+    def set_hamiltonian(self, h0, h1, n_occ):
+        t = self.torch
+        for m in (h0, h1):
+            if not (m.is_cuda and m.dtype == t.float32 and m.dim() == 2 and m.stride(1) == 1):
+                raise DmptError(DMPT_EINVAL, "set_hamiltonian", "need row-major fp32 CUDA matrices")
+        self._h = (h0, h1)          # keep the storage alive
+        dmpt_set_hamiltonian(self.ctx, h0.data_ptr(), h1.data_ptr(), h0.stride(0), n_occ)
+
+    def _new_result(self):
+        ml = self.max_layers
+        bufs = dict(sigma=(C.c_int8 * ml)(), tr_s=(C.c_double * ml)(), tr_x=(C.c_double * ml)(),
+                    id_err=(C.c_double * ml)(), fro_err1=(C.c_double * ml)(), fro_err2=(C.c_double * ml)())
+        r = _CResult()
+        r.sigma = C.cast(bufs["sigma"], C.POINTER(C.c_int8))
+        for k in ("tr_s", "tr_x", "id_err", "fro_err1", "fro_err2"):
+            setattr(r, k, C.cast(bufs[k], C.POINTER(C.c_double)))
+        return r, bufs
+
+    def _wrap(self, rc, r, bufs, d0, d1, d2, check):
+        if rc not in (DMPT_OK, DMPT_ENOCONV) and check:
+            raise DmptError(rc, "dmpt_run", dmpt_last_cuda_error(self.ctx))
+        nl = max(0, int(r.layers))
+        return DmptResult(status=rc, layers=r.layers, layers_d0=r.layers_d0, layers_d1=r.layers_d1,
+                          launches=r.launches, eps_min=r.eps_min, eps_max=r.eps_max, fro_err0=r.fro_err0,
+                          ms_total=r.ms_total, ms_loop=r.ms_loop,
+                          sigma=list(bufs["sigma"][:nl]), tr_s=list(bufs["tr_s"][:nl]),
+                          tr_x=list(bufs["tr_x"][:nl]), id_err=list(bufs["id_err"][:nl]),
+                          fro_err1=list(bufs["fro_err1"][:nl]), d0=d0, d1=d1, d2=d2)
+
+    def run(self, out=None, check=True) -> DmptResult:
+        t = self.torch
+        n = self.n
+        if out is None:
+            d0 = t.empty((n, n), dtype=t.float32, device=self.device)
+            d1 = t.empty((n, n), dtype=t.float32, device=self.device)
+        else:
+            d0, d1 = out[0], out[1]
+        d2 = t.empty((n, n), dtype=t.float32, device=self.device) if self.order == 2 else None
+        r, bufs = self._new_result()
+        rc = dmpt_run(self.ctx, d0.data_ptr(), d1.data_ptr(), d2.data_ptr() if d2 is not None else 0,
+                      d0.stride(0), r)
+        return self._wrap(rc, r, bufs, d0, d1, d2, check)
+
+    def run_host(self, h0, h1, n_occ, out=None, check=True) -> DmptResult:
+        """h0, h1: CPU fp32 tensors (pinned recommended); outputs are CPU tensors."""
+        t = self.torch
+        n = self.n
+        if out is None:
+            d0 = t.empty((n, n), dtype=t.float32, pin_memory=True)
+            d1 = t.empty((n, n), dtype=t.float32, pin_memory=True)
+        else:
+            d0, d1 = out[0], out[1]
+        d2 = t.empty((n, n), dtype=t.float32, pin_memory=True) if self.order == 2 else None
+        r, bufs = self._new_result()
+        rc = dmpt_run_host(self.ctx, h0.data_ptr(), h1.data_ptr(), h0.stride(0), n_occ, d0.data_ptr(),
+                           d1.data_ptr(), d2.data_ptr() if d2 is not None else 0, d0.stride(0), r)
+        return self._wrap(rc, r, bufs, d0, d1, d2, check)
+
+    def layer_products(self, s0, s1):
+        t = self.torch
+        n = self.n
+        x0 = t.empty((n, n), dtype=t.float32, device=self.device)
+        x1 = t.empty((n, n), dtype=t.float32, device=self.device)
+        rc = dmpt_layer_products(self.ctx, s0.data_ptr(), s1.data_ptr(), s0.stride(0), x0.data_ptr(),
+                                 x1.data_ptr(), n)
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_layer_products", dmpt_last_cuda_error(self.ctx))
+        return x0, x1
+
+    def close(self):
+        if getattr(self, "ctx", None) is not None:
+            dmpt_destroy(self.ctx)
+            self.ctx = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,201 @@
+// Device-resident scalar state and control flow of Algorithms 1-3.
+//
+// The per-layer decisions (sigma_n, the D0 test of Algorithm 2, the D1/D2 tests of Algorithm 3,
+// loop exit) are taken on the device by the LAST CTA of each layer launch ("finalizer"), from
+// fp64 sums of the fp32 per-CTA partial reductions the epilogues wrote.  The next launch reads
+// the decision from DmptCtl at kernel start; the host never sees a scalar until the run ends.
+//
+// Reading R9: N_X = Tr[(S0_{n-1})^2] is evaluated as ||S0_{n-1}||_F^2 (equal for a
+// symmetric matrix) and N_S as the actual trace of the stored S0_{n-1}; both are accumulated by
+// the epilogue that WRITES S0_{n-1}, so sigma_n and the D0 decision of layer n are known before
+// layer n's products start.
+#pragma once
+#include <math.h>
+#include <stdint.h>
+
+namespace dmpt {
+
+constexpr double kCD0 = 4.5;   // PAPER.md:518 (Algorithm 2)
+constexpr double kCPT = 9.0;   // PAPER.md:465, 524 (Algorithm 3)
+
+// slots of the per-warp partial reductions written by the layer epilogue
+enum Red : int {
+    RED_TR_S0 = 0,   // sum of the new S0 diagonal                      -> N_S
+    RED_FRO_S0 = 1,  // sum of squares of the new S0                    -> N_X of the next layer
+    RED_FRO0 = 2,    // sum (S0 - X0)^2 on the D0 stop layer            -> FroErr0^2
+    RED_FRO1 = 3,    // sum (S1 - X1)^2 once D0 converged               -> FroErr1_n^2
+    RED_MAX1 = 4,    // max |new S1|                                    -> next S1 scale
+    RED_FRO2 = 5,    // sum (S2 - X2)^2 once D1 converged (order 2)     -> FroErr2_n^2
+    RED_MAX2 = 6,    // max |new S2|
+    RED_COUNT = 8
+};
+
+enum Mode0 : int { MODE_ACTIVE = 0, MODE_STOP = 1, MODE_FROZEN = 2 };
+
+struct DmptCtl {
+    // ---- decision for the next layer launch
+    int layer;      // n of the layer the next launch executes (1-based)
+    int done;       // launches exit at once when set
+    int status;     // DMPT_OK or a negative DMPT_E* code
+    int mode0;      // Mode0
+    int sigma;      // sigma_n
+    int s0_buf;     // hi/lo buffer holding S0_{n-1}
+    int s1_buf;     // fp32 + hi/lo buffer holding S1_{n-1}
+    int s2_buf;
+    int e1_in;      // S1 operand buffers hold fp16(2^e1_in S1_{n-1})
+    int e1_out;     // scale for the split of S1_n
+    int e2_in, e2_out;
+    // ---- state of Algorithms 1-3
+    int conv0, conv1, conv2;
+    int n_c, n_c1, n_c2;
+    int layers;     // layers executed so far
+    int single_shot;  // 1: dmpt_layer_products - run one layer, take no decisions
+    unsigned int ticket;  // CTA arrival counter of the running launch
+    int pad0;
+    double n_s;     // Tr S0_{n-1}
+    double n_x;     // ||S0_{n-1}||_F^2
+    double fro0;    // FroErr0
+    double eps_min, eps_max;
+    double s1_max, s2_max;
+};
+
+struct DmptLogs {   // device arrays, max_layers entries, entry n-1 for layer n
+    int* sigma;
+    double* tr_s;
+    double* tr_x;
+    double* id_err;
+    double* fro1;
+    double* fro2;
+};
+
+struct DmptProblem {
+    int n, n_pad, n_occ, order, max_layers, s0_shift, s1_autoscale;
+};
+
+// exact power of two 2^e bringing m into [8, 16); 0 when m is 0 or not finite
+__device__ __forceinline__ int scale_exponent(double m) {
+    if (!(m > 0.0) || !isfinite(m)) return 0;
+    int e;
+    frexp(m, &e);          // m = f * 2^e, f in [0.5, 1)  ->  m in [2^(e-1), 2^e)
+    return 4 - e;          // m * 2^(4-e) in [8, 16)
+}
+
+// Decide layer n = ctl.layer from N_S, N_X (PAPER.md:499-505 and Algorithm 2).
+__device__ inline void control_decide(DmptCtl& c, const DmptLogs& L, const DmptProblem& pb) {
+    const int n = c.layer;
+    if (n > pb.max_layers) {
+        c.done = 1;
+        c.status = -5;  // DMPT_ENOCONV
+        return;
+    }
+    L.tr_s[n - 1] = c.n_s;
+    if (!c.conv0) {
+        const double n_s = c.n_s, n_x = c.n_x, nocc = (double)pb.n_occ;
+        const double ide = n_s - n_x;
+        const int s = (fabs(2.0 * n_s - n_x - nocc) >= fabs(n_x - nocc)) ? 1 : -1;  // R3: tie -> +1
+        L.tr_x[n - 1] = n_x;
+        L.id_err[n - 1] = ide;
+        L.sigma[n - 1] = s;
+        if (!isfinite(n_s) || !isfinite(n_x)) {
+            c.done = 1;
+            c.status = -6;  // DMPT_ENUMERIC
+            return;
+        }
+        bool stop = !(ide > 0.0);                                              // R6
+        if (!stop && n > 2 && L.sigma[n - 2] != L.sigma[n - 3]) {
+            const double prev = L.id_err[n - 3];
+            stop = !(ide <= kCD0 * prev * prev);
+        }
+        c.sigma = s;
+        if (stop) {
+            c.conv0 = 1;
+            c.n_c = n;
+            c.mode0 = MODE_STOP;      // X0 is still formed once, for FroErr0 (R4)
+        } else {
+            c.mode0 = MODE_ACTIVE;
+        }
+    } else {
+        const int s = -L.sigma[n - 2];
+        L.sigma[n - 1] = s;
+        L.tr_x[n - 1] = nan("");
+        L.id_err[n - 1] = nan("");
+        c.sigma = s;
+        c.mode0 = MODE_FROZEN;
+    }
+}
+
+// After layer n = ctl.layer ran: fold its reductions into the state, apply Algorithm 3
+// (cascade for order 2, reading R15) and decide layer n+1.
+__device__ inline void control_finalize(DmptCtl& c, const DmptLogs& L, const DmptProblem& pb,
+                                        const double* red /* RED_COUNT sums */) {
+    const int n = c.layer;
+    c.layers = n;
+    if (c.single_shot) {
+        c.done = 1;
+        return;
+    }
+    if (c.mode0 == MODE_ACTIVE) {
+        c.n_s = red[RED_TR_S0];
+        c.n_x = red[RED_FRO_S0];
+        c.s0_buf ^= 1;
+    } else if (c.mode0 == MODE_STOP) {
+        c.fro0 = sqrt(red[RED_FRO0]);
+    }
+    const double nanv = nan("");
+    // ---- first order
+    if (!c.conv1) {
+        if (c.conv0) {
+            const double f1 = sqrt(red[RED_FRO1]);
+            L.fro1[n - 1] = f1;
+            if (n - 2 >= c.n_c && !(f1 < kCPT * c.fro0 * L.fro1[n - 3])) {     // R5, R6
+                c.conv1 = 1;
+                c.n_c1 = n;
+            }
+            if (!isfinite(f1) || !isfinite(c.fro0)) c.status = -6;
+        } else {
+            L.fro1[n - 1] = nanv;
+        }
+        if (!c.conv1) {   // accept S1_n
+            c.s1_buf ^= 1;
+            c.e1_in = c.e1_out;
+            c.s1_max = red[RED_MAX1];
+            if (pb.s1_autoscale) c.e1_out = scale_exponent(c.s1_max);
+            if (!isfinite(c.s1_max)) c.status = -6;
+        }
+    } else {
+        L.fro1[n - 1] = nanv;
+    }
+    // ---- second order
+    if (pb.order == 2 && !c.conv2) {
+        if (c.conv1) {
+            const double f2 = sqrt(red[RED_FRO2]);
+            L.fro2[n - 1] = f2;
+            if (n - 2 >= c.n_c1 && !(f2 < kCPT * c.fro0 * L.fro2[n - 3])) {
+                c.conv2 = 1;
+                c.n_c2 = n;
+            }
+            if (!isfinite(f2)) c.status = -6;
+        } else {
+            L.fro2[n - 1] = nanv;
+        }
+        if (!c.conv2) {
+            c.s2_buf ^= 1;
+            c.e2_in = c.e2_out;
+            c.s2_max = red[RED_MAX2];
+            if (pb.s1_autoscale) c.e2_out = scale_exponent(c.s2_max);
+            if (!isfinite(c.s2_max)) c.status = -6;
+        }
+    }
+    if (c.status != 0) {
+        c.done = 1;
+        return;
+    }
+    if (pb.order == 2 ? c.conv2 : c.conv1) {
+        c.done = 1;
+        return;
+    }
+    c.layer = n + 1;
+    control_decide(c, L, pb);
+}
+
+}  // namespace dmpt

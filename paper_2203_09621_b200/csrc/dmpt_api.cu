@@ -1,0 +1,522 @@
+// C ABI of the DNN-SP2-PT hot path (include/dmpt.h): context, workspace carve-up, TMA tensor
+// maps, and the host driver that enqueues bounds -> transform -> split -> layers on one stream.
+// No device memory is allocated here and there is no CPU fallback.
+#include <cuda.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "../../include/dmpt.h"
+#include "control.cuh"
+#include "kernels_hbm.cuh"
+#include "layer_kernel.cuh"
+
+using namespace dmpt;
+
+namespace {
+
+constexpr int kMaxLayersCap = 1024;
+constexpr int kPartialDoubles = 8192 * RED_COUNT;   // >= max(transform grid * 3, layer grid * 4 * RED_COUNT)
+constexpr int kNumEvents = 4;
+constexpr int kFlagSlots = 64;
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Carve {
+    size_t off = 0;
+    size_t take(size_t bytes) {
+        size_t o = off;
+        off = align_up(off + bytes, 256);
+        return o;
+    }
+};
+
+struct Layout {
+    int n, n_pad, order, num_tiles;
+    size_t ctl, bounds, sigma, tr_s, tr_x, id_err, fro1, fro2, partials, tiles;
+    size_t s0, s1[2], s2[2];
+    size_t h[2][6];          // [buffer][S0hi, S0lo, S1hi, S1lo, S2hi, S2lo]
+    size_t stage_h0, stage_h1;
+    size_t total;
+};
+
+int num_tiles_for(int nb) { return nb * (nb + 1) / 2; }
+
+Layout make_layout(int n, int order) {
+    Layout L{};
+    L.n = n;
+    L.order = order;
+    L.n_pad = (int)align_up((size_t)n, kTile);
+    const int nb = L.n_pad / kTile;
+    L.num_tiles = num_tiles_for(nb);
+    const size_t np2 = (size_t)L.n_pad * L.n_pad;
+    Carve c;
+    L.ctl = c.take(sizeof(DmptCtl));
+    L.bounds = c.take(2 * sizeof(long long));
+    L.sigma = c.take(kMaxLayersCap * sizeof(int));
+    L.tr_s = c.take(kMaxLayersCap * sizeof(double));
+    L.tr_x = c.take(kMaxLayersCap * sizeof(double));
+    L.id_err = c.take(kMaxLayersCap * sizeof(double));
+    L.fro1 = c.take(kMaxLayersCap * sizeof(double));
+    L.fro2 = c.take(kMaxLayersCap * sizeof(double));
+    L.partials = c.take(kPartialDoubles * sizeof(double));
+    L.tiles = c.take((size_t)L.num_tiles * sizeof(uint32_t));
+    L.s0 = c.take(np2 * 4);
+    L.s1[0] = c.take(np2 * 4);
+    L.s1[1] = c.take(np2 * 4);
+    if (order == 2) {
+        L.s2[0] = c.take(np2 * 4);
+        L.s2[1] = c.take(np2 * 4);
+    }
+    const int nh = order == 2 ? 6 : 4;
+    for (int b = 0; b < 2; ++b)
+        for (int m = 0; m < nh; ++m) L.h[b][m] = c.take(np2 * 2);
+    L.stage_h0 = c.take((size_t)n * n * 4);
+    L.stage_h1 = c.take((size_t)n * n * 4);
+    L.total = c.off;
+    return L;
+}
+
+// Launch order of the upper-triangular tiles: bands of `band` block rows, column by column inside
+// a band, so that the ~#SM tiles in flight share few row panels (L2 reuse of the operand panels).
+std::vector<uint32_t> make_tile_order(int nb, int band) {
+    std::vector<uint32_t> t;
+    t.reserve(num_tiles_for(nb));
+    for (int b0 = 0; b0 < nb; b0 += band) {
+        const int b1 = b0 + band < nb ? b0 + band : nb;
+        for (int j = b0; j < nb; ++j)
+            for (int i = b0; i < b1 && i <= j; ++i) t.push_back((uint32_t)i | ((uint32_t)j << 16));
+    }
+    return t;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+struct dmpt_ctx {
+    int n = 0, n_occ = 0, ld_in = 0;
+    dmpt_options opt{};
+    Layout L{};
+    uint8_t* ws = nullptr;
+    cudaStream_t stream = nullptr;
+    const float* d_h0 = nullptr;
+    const float* d_h1 = nullptr;
+    int num_sms = 0;
+    int grid_layer = 0;
+    int s0_shift = 14;
+    LayerParams lp{};
+    cudaEvent_t ev[kNumEvents]{};
+    cudaEvent_t ev_t[4]{};
+    int* h_flags = nullptr;      // pinned
+    DmptCtl* h_ctl = nullptr;    // pinned
+    char err[256] = {0};
+
+    template <typename T>
+    T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
+};
+
+#define CK(call)                                                                             \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess) {                                                             \
+            snprintf(ctx->err, sizeof ctx->err, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                     __FILE__, __LINE__);                                                    \
+            return DMPT_ECUDA;                                                               \
+        }                                                                                    \
+    } while (0)
+
+extern "C" void dmpt_default_options(dmpt_options* opt) {
+    if (!opt) return;
+    memset(opt, 0, sizeof *opt);
+    opt->max_layers = 200;
+    opt->order = 1;
+    opt->s0_shift = -1;
+    opt->s1_autoscale = 1;
+    opt->bounds = 0;
+}
+
+extern "C" size_t dmpt_workspace_bytes(int n, int order) {
+    if (n <= 0 || (order != 1 && order != 2) || n > 65535 * kTile) return 0;
+    return make_layout(n, order).total;
+}
+
+extern "C" const char* dmpt_strerror(int code) {
+    switch (code) {
+        case DMPT_OK: return "ok";
+        case DMPT_EINVAL: return "invalid argument";
+        case DMPT_ESTATE: return "dmpt_run called before dmpt_set_hamiltonian";
+        case DMPT_ECUDA: return "CUDA error (see dmpt_last_cuda_error)";
+        case DMPT_EDEGENERATE: return "spectral bounds degenerate: eps_max - eps_min not positive and finite";
+        case DMPT_ENOCONV: return "max_layers reached before the stopping tests fired";
+        case DMPT_ENUMERIC: return "NaN/Inf in the scalar state";
+        case DMPT_EWORKSPACE: return "workspace too small or not 256-byte aligned";
+        default: return "unknown error code";
+    }
+}
+
+extern "C" const char* dmpt_last_cuda_error(const dmpt_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+static int build_tensor_maps(dmpt_ctx* ctx) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) {
+        snprintf(ctx->err, sizeof ctx->err, "cuTensorMapEncodeTiled not available from the driver");
+        return DMPT_ECUDA;
+    }
+    EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(fn);
+    const Layout& L = ctx->L;
+    const cuuint64_t dims[2] = {(cuuint64_t)L.n_pad, (cuuint64_t)L.n_pad};
+    const cuuint64_t strides[1] = {(cuuint64_t)L.n_pad * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)kTile};
+    const cuuint32_t estr[2] = {1, 1};
+    for (int b = 0; b < 2; ++b)
+        for (int m = 0; m < 4; ++m) {
+            CUresult r = encode(&ctx->lp.maps[b][m], CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
+                                ctx->at<void>(L.h[b][m]), dims, strides, box, estr,
+                                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) {
+                snprintf(ctx->err, sizeof ctx->err, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+                return DMPT_ECUDA;
+            }
+        }
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_workspace,
+                           size_t workspace_bytes, void* cuda_stream) {
+    if (!out) return DMPT_EINVAL;
+    *out = nullptr;
+    dmpt_options o;
+    if (opt) o = *opt; else dmpt_default_options(&o);
+    if (n <= 0 || (o.order != 1 && o.order != 2) || !d_workspace) return DMPT_EINVAL;
+    if (o.max_layers <= 0) o.max_layers = 200;
+    if (o.max_layers > kMaxLayersCap) o.max_layers = kMaxLayersCap;
+    if (o.s0_shift > 15) return DMPT_EINVAL;
+    if (o.order == 2) return DMPT_EINVAL;   // second order: not built yet (row a9)
+    const size_t need = dmpt_workspace_bytes(n, o.order);
+    if (need == 0) return DMPT_EINVAL;
+    if (workspace_bytes < need || (reinterpret_cast<uintptr_t>(d_workspace) & 255)) return DMPT_EWORKSPACE;
+
+    dmpt_ctx* ctx = new dmpt_ctx();
+    ctx->n = n;
+    ctx->opt = o;
+    ctx->s0_shift = o.s0_shift < 0 ? 14 : o.s0_shift;
+    ctx->L = make_layout(n, o.order);
+    ctx->ws = static_cast<uint8_t*>(d_workspace);
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    auto fail = [&](int code) {
+        // keep the message reachable: the caller has no ctx on failure, so print it
+        fprintf(stderr, "dmpt_create: %s\n", ctx->err);
+        for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
+        for (auto& e : ctx->ev_t) if (e) cudaEventDestroy(e);
+        if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
+        if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
+        delete ctx;
+        return code;
+    };
+#define CKC(call)                                                                              \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            snprintf(ctx->err, sizeof ctx->err, "%s: %s", #call, cudaGetErrorString(e_));      \
+            return fail(DMPT_ECUDA);                                                           \
+        }                                                                                      \
+    } while (0)
+    int dev = 0;
+    CKC(cudaGetDevice(&dev));
+    CKC(cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev));
+    int cc_major = 0;
+    CKC(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (cc_major != 10) {
+        snprintf(ctx->err, sizeof ctx->err, "device compute capability %d.x: this library is sm_100a only", cc_major);
+        return fail(DMPT_ECUDA);
+    }
+    for (auto& e : ctx->ev) CKC(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    for (auto& e : ctx->ev_t) CKC(cudaEventCreate(&e));
+    CKC(cudaHostAlloc(&ctx->h_flags, kFlagSlots * sizeof(int), cudaHostAllocDefault));
+    CKC(cudaHostAlloc(&ctx->h_ctl, sizeof(DmptCtl), cudaHostAllocDefault));
+    CKC(cudaFuncSetAttribute(dmpt_layer_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+
+    const Layout& L = ctx->L;
+    const int nb = L.n_pad / kTile;
+    int band = 1;
+    while ((band + 1) * (band + 1) <= ctx->num_sms) ++band;      // ~sqrt(#SM) block rows per band
+    std::vector<uint32_t> tiles = make_tile_order(nb, band);
+    CKC(cudaMemcpyAsync(ctx->at<void>(L.tiles), tiles.data(), tiles.size() * sizeof(uint32_t),
+                        cudaMemcpyHostToDevice, ctx->stream));
+    CKC(cudaStreamSynchronize(ctx->stream));
+    ctx->grid_layer = L.num_tiles < ctx->num_sms ? L.num_tiles : ctx->num_sms;
+
+    LayerParams& lp = ctx->lp;
+    lp.s0 = ctx->at<float>(L.s0);
+    lp.s1[0] = ctx->at<float>(L.s1[0]);
+    lp.s1[1] = ctx->at<float>(L.s1[1]);
+    for (int b = 0; b < 2; ++b)
+        for (int m = 0; m < 4; ++m) lp.h[b][m] = ctx->at<__half>(L.h[b][m]);
+    lp.tiles = ctx->at<uint32_t>(L.tiles);
+    lp.num_tiles = L.num_tiles;
+    lp.n_pad = L.n_pad;
+    lp.ctl = ctx->at<DmptCtl>(L.ctl);
+    lp.logs.sigma = ctx->at<int>(L.sigma);
+    lp.logs.tr_s = ctx->at<double>(L.tr_s);
+    lp.logs.tr_x = ctx->at<double>(L.tr_x);
+    lp.logs.id_err = ctx->at<double>(L.id_err);
+    lp.logs.fro1 = ctx->at<double>(L.fro1);
+    lp.logs.fro2 = ctx->at<double>(L.fro2);
+    lp.partials = ctx->at<double>(L.partials);
+    lp.pb.n = n;
+    lp.pb.n_pad = L.n_pad;
+    lp.pb.n_occ = 0;
+    lp.pb.order = o.order;
+    lp.pb.max_layers = o.max_layers;
+    lp.pb.s0_shift = ctx->s0_shift;
+    lp.pb.s1_autoscale = o.s1_autoscale ? 1 : 0;
+    if (build_tensor_maps(ctx) != DMPT_OK) return fail(DMPT_ECUDA);
+#undef CKC
+    *out = ctx;
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_destroy(dmpt_ctx* ctx) {
+    if (!ctx) return DMPT_EINVAL;
+    cudaStreamSynchronize(ctx->stream);
+    for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
+    for (auto& e : ctx->ev_t) if (e) cudaEventDestroy(e);
+    if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
+    if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
+    delete ctx;
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_set_hamiltonian(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld, int n_occ) {
+    if (!ctx || !d_h0 || !d_h1) return DMPT_EINVAL;
+    if (ld < ctx->n || n_occ <= 0 || n_occ >= ctx->n) return DMPT_EINVAL;
+    ctx->d_h0 = d_h0;
+    ctx->d_h1 = d_h1;
+    ctx->ld_in = ld;
+    ctx->n_occ = n_occ;
+    ctx->lp.pb.n_occ = n_occ;
+    return DMPT_OK;
+}
+
+static int launch_layer(dmpt_ctx* ctx) {
+    dmpt_layer_kernel<<<ctx->grid_layer, kNumThreads, kSmemBytes, ctx->stream>>>(ctx->lp);
+    CK(cudaGetLastError());
+    return DMPT_OK;
+}
+
+static int elementwise_grid(const dmpt_ctx* ctx, long long work_items, int threads) {
+    long long blocks = (work_items + threads - 1) / threads;
+    const long long cap = (long long)ctx->num_sms * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    return (int)blocks;
+}
+
+// Everything from the spectral bounds to the last layer; leaves the result in the workspace.
+static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld, int* launches) {
+    const Layout& L = ctx->L;
+    const int n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    long long* bounds = ctx->at<long long>(L.bounds);
+    double* partials = ctx->at<double>(L.partials);
+
+    reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    CK(cudaGetLastError());
+    if (!ctx->opt.bounds) {
+        const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
+        gershgorin_kernel<<<grid, 256, 0, st>>>(d_h0, n, ld, bounds);
+        CK(cudaGetLastError());
+        ++*launches;
+    }
+    bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, ctl, ctx->opt.bounds, ctx->opt.eps_min, ctx->opt.eps_max);
+    CK(cudaGetLastError());
+    const int tgrid = elementwise_grid(ctx, (long long)np * (np / 4), 256);
+    transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, d_h1, n, ld, np, ctx->lp.s0, ctx->lp.s1[0], ctl, partials);
+    CK(cudaGetLastError());
+    control_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.logs, ctx->lp.pb, partials, tgrid);
+    CK(cudaGetLastError());
+    const long long c8 = (long long)np * np / 8;
+    const int sgrid = elementwise_grid(ctx, c8, 256);
+    split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift);
+    CK(cudaGetLastError());
+    split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift);
+    CK(cudaGetLastError());
+    *launches += 6;
+    CK(cudaEventRecord(ctx->ev_t[1], st));
+
+    // Layer loop.  Launches are enqueued in chunks, two chunks ahead of the GPU; after each chunk a
+    // 4-byte copy of ctl.done lands in pinned memory.  Launches after convergence exit at once.
+    const int max_layers = ctx->opt.max_layers;
+    const int chunk_len = np <= 1024 ? 8 : (np <= 4096 ? 4 : 2);
+    int launched = 0, chunks = 0;
+    auto launch_chunk = [&]() -> int {
+        for (int i = 0; i < chunk_len && launched < max_layers; ++i, ++launched) {
+            int rc = launch_layer(ctx);
+            if (rc) return rc;
+            ++*launches;
+        }
+        CK(cudaMemcpyAsync(&ctx->h_flags[chunks % kFlagSlots], &ctl->done, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaEventRecord(ctx->ev[chunks % kNumEvents], st));
+        ++chunks;
+        return DMPT_OK;
+    };
+    int rc = launch_chunk();
+    if (rc) return rc;
+    if (launched < max_layers && (rc = launch_chunk())) return rc;
+    for (int w = 0; w < chunks; ++w) {
+        CK(cudaEventSynchronize(ctx->ev[w % kNumEvents]));
+        if (ctx->h_flags[w % kFlagSlots]) break;
+        if (launched < max_layers && (rc = launch_chunk())) return rc;
+    }
+    CK(cudaEventRecord(ctx->ev_t[2], st));
+    return DMPT_OK;
+}
+
+static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
+    cudaStream_t st = ctx->stream;
+    const Layout& L = ctx->L;
+    CK(cudaEventRecord(ctx->ev_t[3], st));
+    CK(cudaStreamSynchronize(st));
+    const DmptCtl& c = *ctx->h_ctl;
+    int status = c.status;
+    if (status == 0 && !c.done) status = DMPT_ENOCONV;
+    if (res) {
+        res->status = status;
+        res->layers = c.layers;
+        res->layers_d0 = c.n_c;
+        res->layers_d1 = c.n_c1;
+        res->launches = launches;
+        res->eps_min = c.eps_min;
+        res->eps_max = c.eps_max;
+        res->fro_err0 = c.fro0;
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, ctx->ev_t[0], ctx->ev_t[3]));
+        res->ms_total = ms;
+        CK(cudaEventElapsedTime(&ms, ctx->ev_t[1], ctx->ev_t[2]));
+        res->ms_loop = ms;
+        const int nl = c.layers;
+        if (nl > 0) {
+            std::vector<int> sg(nl);
+            if (res->sigma) {
+                CK(cudaMemcpy(sg.data(), ctx->at<int>(L.sigma), nl * sizeof(int), cudaMemcpyDeviceToHost));
+                for (int i = 0; i < nl; ++i) res->sigma[i] = (int8_t)sg[i];
+            }
+            if (res->tr_s) CK(cudaMemcpy(res->tr_s, ctx->at<double>(L.tr_s), nl * sizeof(double), cudaMemcpyDeviceToHost));
+            if (res->tr_x) CK(cudaMemcpy(res->tr_x, ctx->at<double>(L.tr_x), nl * sizeof(double), cudaMemcpyDeviceToHost));
+            if (res->id_err) CK(cudaMemcpy(res->id_err, ctx->at<double>(L.id_err), nl * sizeof(double), cudaMemcpyDeviceToHost));
+            if (res->fro_err1) CK(cudaMemcpy(res->fro_err1, ctx->at<double>(L.fro1), nl * sizeof(double), cudaMemcpyDeviceToHost));
+        }
+    }
+    return status;
+}
+
+// after run_core: fetch ctl (which buffer holds the accepted S1), then enqueue the output copies
+static int fetch_ctl(dmpt_ctx* ctx) {
+    CK(cudaMemcpyAsync(ctx->h_ctl, ctx->at<DmptCtl>(ctx->L.ctl), sizeof(DmptCtl), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, int ld, dmpt_result* res) {
+    if (!ctx || !d_d0 || !d_d1) return DMPT_EINVAL;
+    if (!ctx->d_h0) return DMPT_ESTATE;
+    if (ld < ctx->n || (ctx->opt.order == 2 && !d_d2)) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    int launches = 0;
+    CK(cudaEventRecord(ctx->ev_t[0], ctx->stream));
+    int rc = run_core(ctx, ctx->d_h0, ctx->d_h1, ctx->ld_in, &launches);
+    if (rc) return rc;
+    if ((rc = fetch_ctl(ctx))) return rc;
+    CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
+                         cudaMemcpyDeviceToDevice, ctx->stream));
+    return finish(ctx, res, launches);
+}
+
+extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1, int ld_in, int n_occ,
+                             float* h_d0, float* h_d1, float* h_d2, int ld_out, dmpt_result* res) {
+    if (!ctx || !h_h0 || !h_h1 || !h_d0 || !h_d1) return DMPT_EINVAL;
+    if (ld_in < ctx->n || ld_out < ctx->n || n_occ <= 0 || n_occ >= ctx->n) return DMPT_EINVAL;
+    if (ctx->opt.order == 2 && !h_d2) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    float* s_h0 = ctx->at<float>(L.stage_h0);
+    float* s_h1 = ctx->at<float>(L.stage_h1);
+    ctx->n_occ = n_occ;
+    ctx->lp.pb.n_occ = n_occ;
+    int launches = 0;
+    CK(cudaEventRecord(ctx->ev_t[0], ctx->stream));
+    CK(cudaMemcpy2DAsync(s_h0, n * 4, h_h0, (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpy2DAsync(s_h1, n * 4, h_h1, (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = run_core(ctx, s_h0, s_h1, (int)n, &launches);
+    if (rc) return rc;
+    if ((rc = fetch_ctl(ctx))) return rc;
+    CK(cudaMemcpy2DAsync(h_d0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpy2DAsync(h_d1, (size_t)ld_out * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
+                         cudaMemcpyDeviceToHost, ctx->stream));
+    return finish(ctx, res, launches);
+}
+
+// ---------------------------------------------------------------------------------------------
+// dmpt_layer_products: one layer launch on caller-provided S0, S1 (sigma = +1, no decisions)
+// ---------------------------------------------------------------------------------------------
+namespace {
+__global__ void single_shot_init_kernel(DmptCtl* ctl, DmptProblem pb, const double* __restrict__ partials,
+                                        int nblocks) {
+    if (threadIdx.x | blockIdx.x) return;
+    double m = 0.0;
+    for (int b = 0; b < nblocks; ++b) m = fmax(m, partials[b]);
+    DmptCtl c;
+    memset(&c, 0, sizeof c);
+    c.layer = 1;
+    c.mode0 = MODE_ACTIVE;
+    c.sigma = 1;
+    c.single_shot = 1;
+    c.s1_max = m;
+    c.e1_in = c.e1_out = pb.s1_autoscale ? scale_exponent(m) : 0;
+    *ctl = c;
+}
+}  // namespace
+
+extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float* d_s1, int ld,
+                                   float* d_x0, float* d_x1, int ld_out) {
+    if (!ctx || !d_s0 || !d_s1 || !d_x0 || !d_x1) return DMPT_EINVAL;
+    if (ld < ctx->n || ld_out < ctx->n) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    double* partials = ctx->at<double>(L.partials);
+    const int grid = elementwise_grid(ctx, (long long)np * np, 256);
+    pad_copy_kernel<<<grid, 256, 0, st>>>(d_s0, (int)n, ld, (int)np, ctx->lp.s0, partials);
+    CK(cudaGetLastError());
+    pad_copy_kernel<<<grid, 256, 0, st>>>(d_s1, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
+    CK(cudaGetLastError());
+    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, grid);
+    CK(cudaGetLastError());
+    const long long c8 = (long long)np * np / 8;
+    const int sgrid = elementwise_grid(ctx, c8, 256);
+    split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift);
+    CK(cudaGetLastError());
+    split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift);
+    CK(cudaGetLastError());
+    int rc = launch_layer(ctx);
+    if (rc) return rc;
+    CK(cudaMemcpy2DAsync(d_x0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpy2DAsync(d_x1, (size_t)ld_out * 4, ctx->lp.s1[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    return DMPT_OK;
+}
