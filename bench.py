@@ -1,0 +1,326 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the DNN-SP2-PT hot path (arXiv 2203.09621) on B200.
+
+A "step" is one pass of the whole hot path: dmpt_run = Gershgorin bounds -> initial transform ->
+split -> every deep layer until both parameter-free stopping tests fire -> D0, D1.  The workload
+is BASELINE.json configs[3] (N = 16384, the size the metric is quoted on; synthetic, seeded, see
+DESIGN.md "Input recipe").  Matrices are 1 GiB each: every timed pass streams inputs far larger
+than the 126 MB L2, so no explicit L2 flush is needed (stated in `config`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--n 16384]
+    python bench.py --impl reference      # the fp64 CPU oracle, bounded sample, same JSON line
+
+value      paper-convention Tflops (one FMA = one flop, Eq. 82):
+           (5 N^3 L_active + 3 N^3 L_frozen) / time of the whole dmpt_run, inputs resident in HBM.
+e2e        the same through dmpt_run_host: H0, H1 in pinned host memory, D0, D1 read back.
+roofline   the layer kernel (tcgen05 GEMM + fused epilogue): EXECUTED tensor flops (2 per FMA, as
+           the measured peak counts them) per launch / its average launch duration (CUDA events on
+           the launching stream around the layer loop), against MEASURED_PEAKS.json.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "dmpt_layer_tflops_fma1"
+UNIT = "Tflops (FMA=1)"
+NOMINAL_FP16_TFMA = 1125.0     # 2250 Tflops dense fp16 at 2 flops/FMA (B200_PROFILING.md)
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._pump, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], None, [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+                pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def flops_paper(n, layers, layers_d0):
+    """Eq. 82 with the layers after S0 froze counted as 3 N^3 (SURVEY.md 8(d) accounting rules)."""
+    la = layers_d0 if layers_d0 > 0 else layers
+    lf = layers - la
+    return (5.0 * la + 3.0 * lf) * float(n) ** 3
+
+
+def fma_executed(n_pad, layers, layers_d0):
+    """Tensor FMAs the layer kernel issues: upper-triangular 128x128 tiles only, 9 (6 once S0 froze)
+    128x128xK products per tile."""
+    nb = n_pad // 128
+    tiles = nb * (nb + 1) // 2
+    la = layers_d0 if layers_d0 > 0 else layers
+    lf = layers - la
+    per_mma = 128.0 * 128.0 * n_pad
+    return tiles * per_mma * (9.0 * la + 6.0 * lf)
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline and --impl reference): the only places that touch oracle/
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(config, n_sample, layers):
+    """Time oracle.dnn_sp2_pt (fp64, numpy/host BLAS, as it stands) for `layers` layers of the
+    bench workload's generator at size n_sample.  Returns (Tflops FMA=1, seconds, threads)."""
+    from oracle.dnn_sp2_pt import dnn_sp2_pt
+    from workloads import make_config
+
+    wl = make_config(config, n=n_sample)
+    t0 = time.perf_counter()
+    res = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, max_layers=layers)
+    dt = time.perf_counter() - t0
+    fl = flops_paper(n_sample, res.layers, res.layers_d0)
+    return fl / dt / 1e12, dt, len(os.sched_getaffinity(0))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    n_s, layers = args.ref_n, args.ref_layers
+    for _ in range(args.warmup and 1):          # one untimed pass pages numpy/BLAS in
+        oracle_sample(args.config, min(n_s, 512), 1)
+    vals, secs = [], []
+    cores = len(os.sched_getaffinity(0))
+    for _ in range(args.steps):
+        v, dt, cores = oracle_sample(args.config, n_s, layers)
+        vals.append(v)
+        secs.append(dt)
+    value = sum(vals) / len(vals)
+    sample = f"oracle.dnn_sp2_pt (fp64) on the config-{args.config} generator at n={n_s}, first {layers} layers, per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(secs) / len(secs),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": {"workload": workload_name(args), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_name(args):
+    return (f"BASELINE.json configs[{args.config - 1}] (config {args.config}): N={args.n}, first-order response, "
+            "seeded synthetic gapped Hamiltonian")
+
+
+# ---------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2203_09621_b200 import Dmpt
+    from workloads import make_config
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU path")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # Replicas only: every rank solves its own seeded problem of the same
+    # configuration; there is no data-path collective.
+    wl = make_config(args.config, n=args.n, device=str(dev), seed=None if rank == 0 else 20220309 + args.config + 1000 * rank)
+    n = wl.n
+    h0_host = torch.from_numpy(wl.h0).pin_memory()
+    h1_host = torch.from_numpy(wl.h1).pin_memory()
+    h0 = h0_host.to(dev)
+    h1 = h1_host.to(dev)
+    solver = Dmpt(n, device=dev)
+    solver.set_hamiltonian(h0, h1, wl.n_occ)
+    d0 = torch.empty((n, n), dtype=torch.float32, device=dev)
+    d1 = torch.empty((n, n), dtype=torch.float32, device=dev)
+    d0_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
+    d1_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    for _ in range(args.warmup):
+        res = solver.run(out=(d0, d1))
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    # ---- device-resident arm: K steps between two barriers, CUDA events on the launching stream
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    flops = fma = ms_loop = 0.0
+    launches = layers_total = 0
+    for _ in range(args.steps):
+        res = solver.run(out=(d0, d1))
+        flops += flops_paper(n, res.layers, res.layers_d0)
+        fma += fma_executed(solver_n_pad(n), res.layers, res.layers_d0)
+        ms_loop += res.ms_loop
+        launches += res.launches
+        layers_total += res.layers
+    ev1.record()
+    barrier()
+    ms = max_over_ranks(ev0.elapsed_time(ev1))
+    clocks = sampler.stop() if rank == 0 else None
+    total_flops = sum_over_ranks(flops)
+    value = total_flops / (ms * 1e-3) / 1e12
+
+    # ---- end-to-end arm: host buffers through dmpt_run_host, copies inside the timed region
+    for _ in range(1):
+        solver.run_host(h0_host, h1_host, wl.n_occ, out=(d0_host, d1_host))
+    barrier()
+    ev0.record()
+    e2e_flops = 0.0
+    for _ in range(args.steps):
+        r2 = solver.run_host(h0_host, h1_host, wl.n_occ, out=(d0_host, d1_host))
+        e2e_flops += flops_paper(n, r2.layers, r2.layers_d0)
+    ev1.record()
+    barrier()
+    ms_e2e = max_over_ranks(ev0.elapsed_time(ev1))
+    e2e_value = sum_over_ranks(e2e_flops) / (ms_e2e * 1e-3) / 1e12
+
+    if rank == 0:
+        peaks, peaks_kind = load_peaks()
+        peak_tf = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
+        layer_ms = ms_loop / max(1, layers_total)
+        achieved_tf = 2.0 * fma / (ms_loop * 1e-3) / 1e12
+        cpu_v, cpu_dt, cores = oracle_sample(args.config, args.ref_n, args.ref_layers)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f16 x f16 -> f32 (dual-half), f64 scalars",
+            "data": "synthetic", "gpu_launches": launches,
+            "config": {"workload": workload_name(args), "n": n, "n_occ": wl.n_occ, "order": 1,
+                       "layers": res.layers, "layers_d0": res.layers_d0, "gap": wl.meta.get("gap"),
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "inputs larger than L2 (1 GiB per matrix at N=16384); no flush needed",
+                       "time_to_d1_ms": ms / args.steps, "loop_ms": ms_loop / args.steps,
+                       "tflops_fma1_loop_only": flops / (ms_loop * 1e-3) / 1e12,
+                       "frac_nominal_fp16_peak_fma1": value / NOMINAL_FP16_TFMA,
+                       "paper_context": "~120 Tflops (FMA=1) on one A100, N=19008 (PAPER.md:546); another machine"},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
+                    "h2d_bytes_per_step": 2 * n * n * 4, "d2h_bytes_per_step": 2 * n * n * 4},
+            "roofline": {"bound": "tensor", "kernel": "dmpt_layer_kernel", "achieved": achieved_tf, "peak": peak_tf,
+                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": args.traffic,
+                         "peak_kind": f"bf16_tflops_sustained, {peaks_kind} (fp16 = bf16 rate), 2 flops per FMA",
+                         "avg_launch_ms": layer_ms, "executed_tfma_per_s": achieved_tf / 2.0,
+                         "frac_nominal_1125_tfma": achieved_tf / 2.0 / NOMINAL_FP16_TFMA},
+            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": cpu_dt,
+                             "sample": f"oracle.dnn_sp2_pt (fp64) on the config-{args.config} generator at "
+                                       f"n={args.ref_n}, first {args.ref_layers} layers"},
+        }
+        print(json.dumps(line), flush=True)
+    solver.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def solver_n_pad(n):
+    return (n + 127) // 128 * 128
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--n", type=int, default=None, help="override the matrix size (default: the config's)")
+    ap.add_argument("--ref-n", type=int, default=4096, help="size of the oracle's bounded sample")
+    ap.add_argument("--ref-layers", type=int, default=6)
+    ap.add_argument("--traffic", type=float, default=None, help="dram bytes per layer launch from ncu (profiles/)")
+    args = ap.parse_args()
+    if args.n is None:
+        from workloads import CONFIGS
+        args.n = CONFIGS[args.config]["n"]
+    if args.warmup < 3 and args.impl == "ours":
+        print("bench.py: warmup raised to 3 (timing rules)", file=sys.stderr)
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -57,7 +57,9 @@ typedef struct dmpt_options {
     int bounds;        /* 0: Gershgorin discs of H0; 1: eps_min/eps_max below       */
     double eps_min;    /* read only when bounds == 1                                                  */
     double eps_max;
-    int reserved[8];   /* must be 0                                                                   */
+    int wave_sync;     /* 1 (default): the CTAs of a layer launch re-align at every tile boundary so that   */
+                       /* tiles in flight share operand panels through L2 (cooperative launch); 0: free run */
+    int reserved[7];   /* must be 0                                                                   */
 } dmpt_options;
 
 typedef struct dmpt_result {
@@ -82,7 +84,7 @@ typedef struct dmpt_result {
     double *fro_err2;          /* FroErr2_n (order 2); NaN before D1 converged                        */
 } dmpt_result;
 
-/* Defaults: max_layers 200, order 1, s0_shift -1, s1_autoscale 1, bounds 0. */
+/* Defaults: max_layers 200, order 1, s0_shift -1, s1_autoscale 1, bounds 0, wave_sync 1. */
 void dmpt_default_options(dmpt_options *opt);
 
 /* Bytes of device workspace dmpt_create() needs for matrices of size n at response order `order`

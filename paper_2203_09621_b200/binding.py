@@ -27,7 +27,7 @@ class DmptOptions(C.Structure):
         ("max_layers", C.c_int), ("order", C.c_int), ("s0_shift", C.c_int),
         ("s1_autoscale", C.c_int), ("bounds", C.c_int),
         ("eps_min", C.c_double), ("eps_max", C.c_double),
-        ("reserved", C.c_int * 8),
+        ("wave_sync", C.c_int), ("reserved", C.c_int * 7),
     ]
 
 
@@ -172,7 +172,7 @@ class Dmpt:
     """Owns a dmpt_ctx plus the torch-allocated workspace.  Marshalling only."""
 
     def __init__(self, n, order=1, max_layers=200, s0_shift=-1, s1_autoscale=True, bounds=None,
-                 device="cuda:0", stream=None):
+                 device="cuda:0", stream=None, wave_sync=True):
         import torch
 
         self.torch = torch
@@ -186,6 +186,7 @@ class Dmpt:
         opt.order = self.order
         opt.s0_shift = int(s0_shift)
         opt.s1_autoscale = 1 if s1_autoscale else 0
+        opt.wave_sync = 1 if wave_sync else 0
         if bounds is not None:
             opt.bounds = 1
             opt.eps_min, opt.eps_max = float(bounds[0]), float(bounds[1])

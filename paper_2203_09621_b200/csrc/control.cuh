@@ -51,7 +51,7 @@ struct DmptCtl {
     int layers;     // layers executed so far
     int single_shot;  // 1: dmpt_layer_products - run one layer, take no decisions
     unsigned int ticket;  // CTA arrival counter of the running launch
-    int pad0;
+    unsigned int wave;    // wave-boundary arrivals of the running launch (LayerParams::wave_sync)
     double n_s;     // Tr S0_{n-1}
     double n_x;     // ||S0_{n-1}||_F^2
     double fro0;    // FroErr0

@@ -141,6 +141,7 @@ extern "C" void dmpt_default_options(dmpt_options* opt) {
     opt->s0_shift = -1;
     opt->s1_autoscale = 1;
     opt->bounds = 0;
+    opt->wave_sync = 1;
 }
 
 extern "C" size_t dmpt_workspace_bytes(int n, int order) {
@@ -266,6 +267,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.tiles = ctx->at<uint32_t>(L.tiles);
     lp.num_tiles = L.num_tiles;
     lp.n_pad = L.n_pad;
+    lp.wave_sync = (o.wave_sync && L.num_tiles > ctx->grid_layer) ? 1 : 0;
     lp.ctl = ctx->at<DmptCtl>(L.ctl);
     lp.logs.sigma = ctx->at<int>(L.sigma);
     lp.logs.tr_s = ctx->at<double>(L.tr_s);
@@ -310,8 +312,15 @@ extern "C" int dmpt_set_hamiltonian(dmpt_ctx* ctx, const float* d_h0, const floa
 }
 
 static int launch_layer(dmpt_ctx* ctx) {
-    dmpt_layer_kernel<<<ctx->grid_layer, kNumThreads, kSmemBytes, ctx->stream>>>(ctx->lp);
-    CK(cudaGetLastError());
+    if (ctx->lp.wave_sync) {
+        // the wave barrier needs every CTA resident: a cooperative launch guarantees it or fails
+        void* args[] = {&ctx->lp};
+        CK(cudaLaunchCooperativeKernel((const void*)dmpt_layer_kernel, dim3(ctx->grid_layer), dim3(kNumThreads),
+                                       args, kSmemBytes, ctx->stream));
+    } else {
+        dmpt_layer_kernel<<<ctx->grid_layer, kNumThreads, kSmemBytes, ctx->stream>>>(ctx->lp);
+        CK(cudaGetLastError());
+    }
     return DMPT_OK;
 }
 
@@ -332,26 +341,26 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     long long* bounds = ctx->at<long long>(L.bounds);
     double* partials = ctx->at<double>(L.partials);
 
-    reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
     CK(cudaGetLastError());
     if (!ctx->opt.bounds) {
         const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
-        gershgorin_kernel<<<grid, 256, 0, st>>>(d_h0, n, ld, bounds);
+        dmpt_gershgorin_kernel<<<grid, 256, 0, st>>>(d_h0, n, ld, bounds);
         CK(cudaGetLastError());
         ++*launches;
     }
-    bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, ctl, ctx->opt.bounds, ctx->opt.eps_min, ctx->opt.eps_max);
+    dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, ctl, ctx->opt.bounds, ctx->opt.eps_min, ctx->opt.eps_max);
     CK(cudaGetLastError());
     const int tgrid = elementwise_grid(ctx, (long long)np * (np / 4), 256);
-    transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, d_h1, n, ld, np, ctx->lp.s0, ctx->lp.s1[0], ctl, partials);
+    dmpt_transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, d_h1, n, ld, np, ctx->lp.s0, ctx->lp.s1[0], ctl, partials);
     CK(cudaGetLastError());
-    control_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.logs, ctx->lp.pb, partials, tgrid);
+    dmpt_control_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.logs, ctx->lp.pb, partials, tgrid);
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
-    split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift);
     CK(cudaGetLastError());
-    split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift);
     CK(cudaGetLastError());
     *launches += 6;
     CK(cudaEventRecord(ctx->ev_t[1], st));
@@ -501,17 +510,17 @@ extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float
     DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
     double* partials = ctx->at<double>(L.partials);
     const int grid = elementwise_grid(ctx, (long long)np * np, 256);
-    pad_copy_kernel<<<grid, 256, 0, st>>>(d_s0, (int)n, ld, (int)np, ctx->lp.s0, partials);
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s0, (int)n, ld, (int)np, ctx->lp.s0, partials);
     CK(cudaGetLastError());
-    pad_copy_kernel<<<grid, 256, 0, st>>>(d_s1, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s1, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
     CK(cudaGetLastError());
     single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, grid);
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
-    split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift);
     CK(cudaGetLastError());
-    split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift);
     CK(cudaGetLastError());
     int rc = launch_layer(ctx);
     if (rc) return rc;

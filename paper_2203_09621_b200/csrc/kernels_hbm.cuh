@@ -51,7 +51,7 @@ __device__ __forceinline__ T warp_max(T v) {
 //     eps_min = min_i (H0_ii - r_i), eps_max = max_i (H0_ii + r_i), r_i = sum_{j != i} |H0_ij|.
 //     bounds[0], bounds[1]: ordered-int encodings, initialised to +inf / -inf by the host.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) gershgorin_kernel(const float* __restrict__ h0, int n, int ld,
+__global__ void __launch_bounds__(256) dmpt_gershgorin_kernel(const float* __restrict__ h0, int n, int ld,
                                                          long long* __restrict__ bounds) {
     const int warps_per_block = blockDim.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -88,9 +88,9 @@ __global__ void __launch_bounds__(256) gershgorin_kernel(const float* __restrict
 //        S0 = (eps_max I - H0)/W,  S1 = -H1/W,  W = eps_max - eps_min,
 //     written to n_pad x n_pad fp32 workspace matrices (zero outside n x n), together with the
 //     first reductions: Tr S0, ||S0||_F^2, max|S1| as per-block partials (summed in a fixed order
-//     by control_init_kernel).  Each element is formed in fp64 and rounded once to fp32.
+//     by dmpt_control_init_kernel).  Each element is formed in fp64 and rounded once to fp32.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) transform_kernel(const float* __restrict__ h0,
+__global__ void __launch_bounds__(256) dmpt_transform_kernel(const float* __restrict__ h0,
                                                         const float* __restrict__ h1, int n, int ld,
                                                         int n_pad, float* __restrict__ s0,
                                                         float* __restrict__ s1,
@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(256) transform_kernel(const float* __restrict_
 }
 
 // zero-padded copy of a caller matrix into an n_pad x n_pad workspace matrix (dmpt_layer_products)
-__global__ void __launch_bounds__(256) pad_copy_kernel(const float* __restrict__ src, int n, int ld,
+__global__ void __launch_bounds__(256) dmpt_pad_copy_kernel(const float* __restrict__ src, int n, int ld,
                                                        int n_pad, float* __restrict__ dst,
                                                        double* __restrict__ partials /* [grid] max */) {
     const long long total = (long long)n_pad * n_pad;
@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(256) pad_copy_kernel(const float* __restrict__
 // Scalar set-up between the transform and the first layer: spectral bounds -> ctl (before the
 // transform), then first reductions -> ctl and the decision for layer 1 (after it).
 // ---------------------------------------------------------------------------------------------
-__global__ void reset_state_kernel(DmptCtl* ctl, long long* bounds) {
+__global__ void dmpt_reset_state_kernel(DmptCtl* ctl, long long* bounds) {
     if (threadIdx.x | blockIdx.x) return;
     DmptCtl c;
     memset(&c, 0, sizeof c);
@@ -193,7 +193,7 @@ __global__ void reset_state_kernel(DmptCtl* ctl, long long* bounds) {
     bounds[1] = dbl_to_ordered(-INFINITY);
 }
 
-__global__ void bounds_to_ctl_kernel(const long long* __restrict__ bounds, DmptCtl* ctl, int use_given,
+__global__ void dmpt_bounds_to_ctl_kernel(const long long* __restrict__ bounds, DmptCtl* ctl, int use_given,
                                      double eps_min, double eps_max) {
     if (threadIdx.x | blockIdx.x) return;
     const double lo = use_given ? eps_min : ordered_to_dbl(bounds[0]);
@@ -210,7 +210,7 @@ __global__ void bounds_to_ctl_kernel(const long long* __restrict__ bounds, DmptC
     }
 }
 
-__global__ void control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProblem pb,
+__global__ void dmpt_control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProblem pb,
                                     const double* __restrict__ partials, int nblocks) {
     if (threadIdx.x | blockIdx.x) return;
     DmptCtl c = *ctl;
@@ -235,6 +235,7 @@ __global__ void control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProblem pb,
 //     (readings R12/R17): hi = fp16(2^e x), lo = fp16(2^e x - hi), round-to-nearest-even.
 //     8 elements per thread: two 128-bit loads, one 128-bit store per output.
 //     `which` selects the exponent on the device: 0 -> s0_shift, 1 -> ctl->e1_in, 2 -> ctl->e2_in.
+//     For which == 0 the matrix split is M = S0 - I/2 (residual form, layer_kernel.cuh).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void split_scaled(float x, float scale, __half& hi, __half& lo) {
     const float t = x * scale;              // exact: scale is a power of two (barring overflow)
@@ -242,20 +243,23 @@ __device__ __forceinline__ void split_scaled(float x, float scale, __half& hi, _
     lo = __float2half_rn(t - __half2float(hi));
 }
 
-__global__ void __launch_bounds__(256) split_kernel(const float* __restrict__ x, long long count8,
-                                                    __half* __restrict__ hi, __half* __restrict__ lo,
-                                                    const DmptCtl* __restrict__ ctl, int which, int s0_shift) {
+__global__ void __launch_bounds__(256) dmpt_split_kernel(const float* __restrict__ x, long long count8, int n_pad,
+                                                         __half* __restrict__ hi, __half* __restrict__ lo,
+                                                         const DmptCtl* __restrict__ ctl, int which, int s0_shift) {
     const int e = which == 0 ? s0_shift : (which == 1 ? ctl->e1_in : ctl->e2_in);
     const float scale = exp2f((float)e);
+    const float diag_shift = which == 0 ? 0.5f : 0.f;      // order 0: the operands hold M = S0 - I/2
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < count8;
          i += (long long)gridDim.x * blockDim.x) {
         const float4 v0 = ldg_stream4(x + i * 8);
         const float4 v1 = ldg_stream4(x + i * 8 + 4);
-        const float v[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+        float v[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+        const long long e0 = i * 8;
+        const int row = (int)(e0 / n_pad), col = (int)(e0 - (long long)row * n_pad);
         __align__(16) __half h[8];
         __align__(16) __half l[8];
 #pragma unroll
-        for (int t = 0; t < 8; ++t) split_scaled(v[t], scale, h[t], l[t]);
+        for (int t = 0; t < 8; ++t) split_scaled(col + t == row ? v[t] - diag_shift : v[t], scale, h[t], l[t]);
         *reinterpret_cast<uint4*>(hi + i * 8) = *reinterpret_cast<const uint4*>(h);
         *reinterpret_cast<uint4*>(lo + i * 8) = *reinterpret_cast<const uint4*>(l);
     }

@@ -1,24 +1,39 @@
 // One deep layer of DNN-SP2-PT in ONE launch (steps a4-a8 of DESIGN.md):
 //
-//   X0 = S0^2               = hi0.hi0 + hi0.lo0 + lo0.hi0                  PAPER.md:124-136 (Eqs. 14-16)
-//   X1 = S0 S1 + S1 S0      = sum of the 3 dual-half terms of each product PAPER.md:309-329 (Eqs. 44-46)
+//   X0 = S0^2,  X1 = S0 S1 + S1 S0 in the dual half-precision representation,
+//       each product = hi.hi + hi.lo + lo.hi, fp16 operands, fp32 accumulation
+//                                                  PAPER.md:124-136 (Eqs. 14-16), 309-329 (Eqs. 44-46)
 //   S0 <- sigma X0 + (1 - sigma) S0,  S1 <- sigma X1 + (1 - sigma) S1      PAPER.md:182, 193 (Eqs. 23, 25)
 //   re-split of the new iterates to (hi, lo) fp16                          PAPER.md:120 (Eq. 13)
 //   Tr S0, ||S0||_F^2, ||S0 - X0||_F^2, ||S1 - X1||_F^2, max|S1|
 //   Algorithms 2 and 3 + the decision for the next layer (last CTA)
 //
+// Residual form.  With M = S0 - I/2 the two products are
+// taken as  P0 = M.M  and  P1 = M.S1 + S1.M,  and
+//       R = S0 - X0 = I/4 - P0,        V = X1 - S1 = P1,
+//       S0 <- S0 - sigma R,            S1 <- S1 + sigma V,
+// which is Eqs. 23/25 rewritten (S0^2 = S0 - R, 2 S0 - S0^2 = S0 + R; likewise for S1).  The same
+// operand count and the same nine tensor-core products per tile; FroErr0 = ||R||_F and
+// FroErr1 = ||V||_F fall out directly.  The operand matrices hold the split of M and of S1.
+//
+// Promoted accumulation.  tcgen05 accumulates in fp32 with TRUNCATION (measured: -0.9 ulp of the
+// final sum per K=16 step, i.e. a relative bias of 4e-5 at K = 16384).  Every kChunkK columns of K
+// the TMEM accumulators are therefore drained into fp32 registers of the epilogue warps with
+// round-to-nearest adds and restarted from zero, which bounds the bias by that of kChunkK/16 steps.
+//
 // Design (sm_100a).  All iterates are exactly symmetric, so C[i,j] = sum_k A[i,k] B[j,k]: both
 // operands of every product are K-major row panels of the same fp16 matrices ("TN" GEMM, the
 // natural TMA/UMMA layout), and only output tiles on or above the diagonal are computed; each
-// is stored twice (direct and mirrored), which keeps the iterates bit-symmetric.  A tile of X0
-// and the matching tile of X1 are accumulated side by side in TMEM from the SAME eight operand
-// tiles per k-block (S0hi, S0lo, S1hi, S1lo for row panel I and for row panel J): 9 MMAs per 8
+// is stored twice (direct and mirrored), which keeps the iterates bit-symmetric.  A tile of P0
+// and the matching tile of P1 are accumulated side by side in TMEM from the SAME eight operand
+// tiles per k-block (Mhi, Mlo, S1hi, S1lo for row panel I and for row panel J): 9 MMAs per 8
 // tiles loaded, against 1 per 2 for a plain GEMM.  Executed tensor work per layer is
 // 4.5 N^3 FMA (3 N^3 once S0 froze) against the paper's 5 N^3 (3 N^3).
 //
 // Warp roles: warp 0 TMA producer, warp 1 MMA issuer (one elected lane) and TMEM owner,
-// warps 2-5 epilogue (one TMEM lane quadrant each).  TMEM holds two accumulator stages
-// (2 x [X0 | X1] x 128 columns) so the epilogue of tile t overlaps the MMAs of tile t+1.
+// warps 2-9 epilogue: warp w owns TMEM lane quadrant w % 4 and column half (w - 2) / 4 of both
+// accumulators (64 + 64 fp32 registers per thread).  TMEM holds two accumulator stages
+// (2 x [P0 | P1] x 128 columns): the drain of chunk c overlaps the MMAs of chunk c + 1.
 #pragma once
 #include <cuda_fp16.h>
 
@@ -35,41 +50,135 @@ constexpr int kStages = 3;
 constexpr int kOpBytes = kTile * kRowBytes;          // 8 KiB per operand tile
 constexpr int kOpsPerStage = 8;
 constexpr int kStageBytes = kOpBytes * kOpsPerStage; // 64 KiB
+constexpr int kChunkK = 128;               // promotion interval along K
+constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;
-constexpr int kNumThreads = 192;
 constexpr int kEpiWarp0 = 2;
-constexpr int kNumEpiWarps = 4;
+constexpr int kNumEpiWarps = 8;
+constexpr int kNumThreads = 32 * (kEpiWarp0 + kNumEpiWarps);   // 320
+constexpr int kHalfCols = kTile / 2;       // accumulator columns per epilogue thread and product
+constexpr int kSub = 16;                   // columns per step of the final epilogue
 constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
 
-// operand slots inside a stage
-enum Op : int { A0H = 0, A0L = 1, A1H = 2, A1L = 3, B0H = 4, B0L = 5, B1H = 6, B1L = 7 };
+// operand slots inside a stage (A = row panel I, B = row panel J)
+enum Op : int { AMH = 0, AML = 1, A1H = 2, A1L = 3, BMH = 4, BML = 5, B1H = 6, B1L = 7 };
 
 struct LayerParams {
-    CUtensorMap maps[2][4];     // [buffer][S0hi, S0lo, S1hi, S1lo], box = kBK x kTile, SWIZZLE_64B
+    CUtensorMap maps[2][4];     // [buffer][Mhi, Mlo, S1hi, S1lo], box = kBK x kTile, SWIZZLE_64B
     float* s0;                  // fp32 S0, updated in place, ld = n_pad
     float* s1[2];               // fp32 S1, ping-pong
     __half* h[2][4];            // fp16 operand matrices the epilogue writes, same order as maps
     const uint32_t* tiles;      // (I | J << 16), I <= J, in launch order
     int num_tiles;
     int n_pad;
+    int wave_sync;              // 1: producers of all CTAs re-align at every tile boundary (L2 reuse)
     DmptCtl* ctl;
     DmptLogs logs;
     DmptProblem pb;
     double* partials;           // [gridDim.x][kNumEpiWarps][RED_COUNT]
 };
 
-__device__ __forceinline__ void st_f4(float* p, float a, float b, float c, float d) {
-    *reinterpret_cast<float4*>(p) = make_float4(a, b, c, d);
-}
 __device__ __forceinline__ uint32_t pack2(__half a, __half b) {
     return (uint32_t)__half_as_ushort(a) | ((uint32_t)__half_as_ushort(b) << 16);
 }
-// 32 fp16 of one row (packed two per register) -> four 128-bit stores
-__device__ __forceinline__ void st_h32(__half* p, const uint32_t (&w)[16]) {
+
+// Final epilogue of one product for one thread: row `gr`, columns gc_base .. gc_base + 63 held in
+// acc[].  ORDER 0: acc = (2^a M)(2^a M) sums;  ORDER 1: acc = P1 sums.
+//   mode: 0 = update and store, 1 = measure only (D0 stop layer: FroErr0, S0 untouched).
+struct EpiOut {
+    float* dst;            // fp32 matrix to write (S0 in place, or the S1 ping-pong target)
+    const float* old;      // fp32 matrix holding the previous iterate
+    __half* hi;
+    __half* lo;
+};
+
+template <int ORDER>
+__device__ __forceinline__ void final_epilogue(float (&acc)[kHalfCols], const EpiOut& o, int ld, int gr,
+                                               int gc_base, bool diag_tile, bool store, float sig,
+                                               float unscale, float scale, bool want_fro, double& r_tr,
+                                               double& r_fs, double& r_fro, float& r_max) {
 #pragma unroll
-    for (int j = 0; j < 16; j += 4)
-        *reinterpret_cast<uint4*>(p + 2 * j) = make_uint4(w[j], w[j + 1], w[j + 2], w[j + 3]);
+    for (int sc = 0; sc < kHalfCols / kSub; ++sc) {
+        const int gc0 = gc_base + sc * kSub;
+        if (diag_tile && gc0 + kSub - 1 < gr) continue;          // strictly below the diagonal: mirrored by others
+        float old[kSub];
+#pragma unroll
+        for (int j = 0; j < kSub; j += 4) {
+            const float4 v = *reinterpret_cast<const float4*>(o.old + (size_t)gr * ld + gc0 + j);
+            old[j] = v.x; old[j + 1] = v.y; old[j + 2] = v.z; old[j + 3] = v.w;
+        }
+        float f_tr = 0.f, f_fs = 0.f, f_fro = 0.f;
+        uint32_t ph[kSub / 2], pl[kSub / 2];
+        __half hprev = __float2half_rn(0.f), lprev = hprev;
+#pragma unroll
+        for (int j = 0; j < kSub; ++j) {
+            const int gc = gc0 + j;
+            const float w = gr < gc ? 2.f : (gr == gc ? 1.f : 0.f);
+            const float dg = gr == gc ? 1.f : 0.f;
+            float nw, delta;
+            if (ORDER == 0) {
+                delta = fmaf(-unscale, acc[sc * kSub + j], 0.25f * dg);      // R = I/4 - M.M
+                nw = fmaf(-sig, delta, old[j]);                              // S0 - sigma R
+            } else {
+                delta = unscale * acc[sc * kSub + j];                        // V = M.S1 + S1.M
+                nw = fmaf(sig, delta, old[j]);                               // S1 + sigma V
+            }
+            if (want_fro) f_fro = fmaf(w * delta, delta, f_fro);
+            acc[sc * kSub + j] = nw;
+            if (ORDER == 0) {
+                f_fs = fmaf(w * nw, nw, f_fs);
+                f_tr += dg * nw;
+            } else if (w != 0.f) {
+                r_max = fmaxf(r_max, fabsf(nw));
+            }
+            __half hh, ll;
+            split_scaled(ORDER == 0 ? nw - 0.5f * dg : nw, scale, hh, ll);   // operands hold M = S0 - I/2
+            if (j & 1) { ph[j >> 1] = pack2(hprev, hh); pl[j >> 1] = pack2(lprev, ll); }
+            hprev = hh; lprev = ll;
+        }
+        r_tr += (double)f_tr;
+        r_fs += (double)f_fs;
+        r_fro += (double)f_fro;
+        if (!store) continue;
+        if (!diag_tile) {
+            float* d = o.dst + (size_t)gr * ld + gc0;
+#pragma unroll
+            for (int j = 0; j < kSub; j += 4)
+                *reinterpret_cast<float4*>(d + j) = make_float4(acc[sc * kSub + j], acc[sc * kSub + j + 1],
+                                                                acc[sc * kSub + j + 2], acc[sc * kSub + j + 3]);
+#pragma unroll
+            for (int j = 0; j < kSub / 2; j += 4) {
+                *reinterpret_cast<uint4*>(o.hi + (size_t)gr * ld + gc0 + 2 * j) = make_uint4(ph[j], ph[j + 1], ph[j + 2], ph[j + 3]);
+                *reinterpret_cast<uint4*>(o.lo + (size_t)gr * ld + gc0 + 2 * j) = make_uint4(pl[j], pl[j + 1], pl[j + 2], pl[j + 3]);
+            }
+            // mirrored copy: for a fixed j the 32 lanes write 32 consecutive elements of row gc0 + j
+#pragma unroll
+            for (int j = 0; j < kSub; ++j) {
+                const size_t m = (size_t)(gc0 + j) * ld + gr;
+                const uint32_t hw = ph[j >> 1], lw = pl[j >> 1];
+                o.dst[m] = acc[sc * kSub + j];
+                o.hi[m] = __ushort_as_half((unsigned short)((j & 1) ? (hw >> 16) : (hw & 0xFFFF)));
+                o.lo[m] = __ushort_as_half((unsigned short)((j & 1) ? (lw >> 16) : (lw & 0xFFFF)));
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < kSub; ++j) {
+                const int gc = gc0 + j;
+                const uint32_t hw = ph[j >> 1], lw = pl[j >> 1];
+                const __half hh = __ushort_as_half((unsigned short)((j & 1) ? (hw >> 16) : (hw & 0xFFFF)));
+                const __half ll = __ushort_as_half((unsigned short)((j & 1) ? (lw >> 16) : (lw & 0xFFFF)));
+                if (gr <= gc) {
+                    const size_t dct = (size_t)gr * ld + gc;
+                    o.dst[dct] = acc[sc * kSub + j]; o.hi[dct] = hh; o.lo[dct] = ll;
+                }
+                if (gr < gc) {
+                    const size_t m = (size_t)gc * ld + gr;
+                    o.dst[m] = acc[sc * kSub + j]; o.hi[m] = hh; o.lo[m] = ll;
+                }
+            }
+        }
+    }
 }
 
 __global__ void __launch_bounds__(kNumThreads, 1)
@@ -92,13 +201,13 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const int num_kb = p.n_pad / kBK;
-    const bool with_x0 = c.mode0 != MODE_FROZEN;
+    const int num_chunks = p.n_pad / kChunkK;
+    const bool with_p0 = c.mode0 != MODE_FROZEN;
 
     if (warp == 0 && lane == 0) {
-        for (int m = 0; m < 4; ++m) {
+        for (int m = 0; m < 2; ++m) {
             prefetch_tensormap(&p.maps[c.s0_buf][m]);
-            prefetch_tensormap(&p.maps[c.s1_buf][m]);
+            prefetch_tensormap(&p.maps[c.s1_buf][2 + m]);
         }
         for (int s = 0; s < kStages; ++s) {
             mbar_init(full_bar(s), 1);
@@ -122,13 +231,28 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     if (warp == 0) {
         // =========================== TMA producer ===========================
         if (lane == 0) {
-            const CUtensorMap* m0h = &p.maps[c.s0_buf][0];
-            const CUtensorMap* m0l = &p.maps[c.s0_buf][1];
+            const CUtensorMap* mmh = &p.maps[c.s0_buf][0];
+            const CUtensorMap* mml = &p.maps[c.s0_buf][1];
             const CUtensorMap* m1h = &p.maps[c.s1_buf][2];
             const CUtensorMap* m1l = &p.maps[c.s1_buf][3];
+            const int num_kb = p.n_pad / kBK;
             int stage = 0;
             uint32_t phase = 0;
-            for (int t = blockIdx.x; t < p.num_tiles; t += gridDim.x) {
+            unsigned int wave = 0;
+            const unsigned int num_waves = (p.num_tiles + gridDim.x - 1) / gridDim.x;
+            for (int t = blockIdx.x; t < p.num_tiles; t += gridDim.x, ++wave) {
+                if (p.wave_sync && wave > 0) {
+                    // re-align the K phase of all CTAs: tiles in flight then stream the same k-blocks of
+                    // few row panels at the same time and share them through L2
+                    __threadfence();
+                    atomicAdd(&p.ctl->wave, 1u);
+                    const unsigned int target = gridDim.x * wave;
+                    unsigned int spins = 0;
+                    while (ld_acquire_u32(&p.ctl->wave) < target) {
+                        __nanosleep(64);
+                        if (++spins > (1u << 26)) __trap();
+                    }
+                }
                 const uint32_t tl = p.tiles[t];
                 const int row_i = (int)(tl & 0xFFFF) * kTile, row_j = (int)(tl >> 16) * kTile;
                 for (int kb = 0; kb < num_kb; ++kb) {
@@ -137,10 +261,10 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                     const uint32_t base = smem_base + stage * kStageBytes;
                     mbar_arrive_expect_tx(fb, kStageBytes);
                     const int k0 = kb * kBK;
-                    tma_load_2d(base + A0H * kOpBytes, m0h, fb, k0, row_i);
-                    tma_load_2d(base + B0H * kOpBytes, m0h, fb, k0, row_j);
-                    tma_load_2d(base + A0L * kOpBytes, m0l, fb, k0, row_i);
-                    tma_load_2d(base + B0L * kOpBytes, m0l, fb, k0, row_j);
+                    tma_load_2d(base + AMH * kOpBytes, mmh, fb, k0, row_i);
+                    tma_load_2d(base + BMH * kOpBytes, mmh, fb, k0, row_j);
+                    tma_load_2d(base + AML * kOpBytes, mml, fb, k0, row_i);
+                    tma_load_2d(base + BML * kOpBytes, mml, fb, k0, row_j);
                     tma_load_2d(base + A1H * kOpBytes, m1h, fb, k0, row_i);
                     tma_load_2d(base + B1H * kOpBytes, m1h, fb, k0, row_j);
                     tma_load_2d(base + A1L * kOpBytes, m1l, fb, k0, row_i);
@@ -148,6 +272,8 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
+            // CTAs with fewer tiles still owe their arrivals to the later waves
+            if (p.wave_sync && wave < num_waves && wave > 0) atomicAdd(&p.ctl->wave, num_waves - wave);
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
@@ -158,215 +284,106 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             int acc = 0;
             uint32_t acc_phase = 0;
             for (int t = blockIdx.x; t < p.num_tiles; t += gridDim.x) {
-                mbar_wait(tempty_bar(acc), acc_phase ^ 1);
-                tc_fence_after();
-                const uint32_t d0 = tmem_base + acc * 256;        // X0 accumulator columns
-                const uint32_t d1 = d0 + 128;                     // X1 accumulator columns
-                for (int kb = 0; kb < num_kb; ++kb) {
-                    mbar_wait(full_bar(stage), phase);
+                for (int ch = 0; ch < num_chunks; ++ch) {
+                    mbar_wait(tempty_bar(acc), acc_phase ^ 1);
                     tc_fence_after();
-                    const uint32_t base = smem_base + stage * kStageBytes;
-                    uint64_t d[kOpsPerStage];
+                    const uint32_t d0 = tmem_base + acc * 256;        // P0 accumulator columns
+                    const uint32_t d1 = d0 + 128;                     // P1 accumulator columns
+                    for (int kb = 0; kb < kKbPerChunk; ++kb) {
+                        mbar_wait(full_bar(stage), phase);
+                        tc_fence_after();
+                        const uint32_t base = smem_base + stage * kStageBytes;
+                        uint64_t d[kOpsPerStage];
 #pragma unroll
-                    for (int o = 0; o < kOpsPerStage; ++o) d[o] = make_smem_desc<kRowBytes>(base + o * kOpBytes);
+                        for (int o = 0; o < kOpsPerStage; ++o) d[o] = make_smem_desc<kRowBytes>(base + o * kOpBytes);
 #pragma unroll
-                    for (int ks = 0; ks < kBK / 16; ++ks) {
-                        const uint64_t adv = (uint64_t)(ks * 32 >> 4);     // 16 fp16 = 32 bytes along K
-                        const uint32_t first = (kb | ks) != 0;
-                        if (with_x0) {
-                            umma_f16<1>(d0, d[A0H] + adv, d[B0H] + adv, idesc, first);   // hi.hi
-                            umma_f16<1>(d0, d[A0H] + adv, d[B0L] + adv, idesc, 1);       // hi.lo
-                            umma_f16<1>(d0, d[A0L] + adv, d[B0H] + adv, idesc, 1);       // lo.hi
+                        for (int ks = 0; ks < kBK / 16; ++ks) {
+                            const uint64_t adv = (uint64_t)(ks * 32 >> 4);     // 16 fp16 = 32 bytes along K
+                            const uint32_t first = (kb | ks) != 0;
+                            if (with_p0) {
+                                umma_f16<1>(d0, d[AMH] + adv, d[BMH] + adv, idesc, first);   // hi.hi
+                                umma_f16<1>(d0, d[AMH] + adv, d[BML] + adv, idesc, 1);       // hi.lo
+                                umma_f16<1>(d0, d[AML] + adv, d[BMH] + adv, idesc, 1);       // lo.hi
+                            }
+                            umma_f16<1>(d1, d[AMH] + adv, d[B1H] + adv, idesc, first);       // M.S1
+                            umma_f16<1>(d1, d[A1H] + adv, d[BMH] + adv, idesc, 1);           // S1.M
+                            umma_f16<1>(d1, d[AMH] + adv, d[B1L] + adv, idesc, 1);
+                            umma_f16<1>(d1, d[AML] + adv, d[B1H] + adv, idesc, 1);
+                            umma_f16<1>(d1, d[A1H] + adv, d[BML] + adv, idesc, 1);
+                            umma_f16<1>(d1, d[A1L] + adv, d[BMH] + adv, idesc, 1);
                         }
-                        umma_f16<1>(d1, d[A0H] + adv, d[B1H] + adv, idesc, first);       // S0.S1
-                        umma_f16<1>(d1, d[A1H] + adv, d[B0H] + adv, idesc, 1);           // S1.S0
-                        umma_f16<1>(d1, d[A0H] + adv, d[B1L] + adv, idesc, 1);
-                        umma_f16<1>(d1, d[A0L] + adv, d[B1H] + adv, idesc, 1);
-                        umma_f16<1>(d1, d[A1H] + adv, d[B0L] + adv, idesc, 1);
-                        umma_f16<1>(d1, d[A1L] + adv, d[B0H] + adv, idesc, 1);
+                        umma_commit(empty_bar(stage));                 // frees the smem stage
+                        if (++stage == kStages) { stage = 0; phase ^= 1; }
                     }
-                    umma_commit(empty_bar(stage));                 // frees the smem stage
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                    umma_commit(tfull_bar(acc));                       // chunk accumulators complete
+                    if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
                 }
-                umma_commit(tfull_bar(acc));                       // accumulators complete
-                if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
             }
         }
     } else {
         // =========================== epilogue ===========================
         const int q = warp & 3;                         // TMEM lane quadrant this warp may read
+        const int half = (warp - kEpiWarp0) >> 2;       // which 64 accumulator columns
         const int ld = p.n_pad;
         const float sig = (float)c.sigma;
-        const float keep = 1.f - sig;                   // (1 - sigma): 0 or 2
         const float unscale0 = exp2f(-2.f * (float)p.pb.s0_shift);
         const float unscale1 = exp2f(-(float)(p.pb.s0_shift + c.e1_in));
         const float scale0 = exp2f((float)p.pb.s0_shift);
         const float scale1 = exp2f((float)c.e1_out);
         const bool upd0 = c.mode0 == MODE_ACTIVE;
-        const bool need_old0 = (upd0 && c.sigma < 0) || c.mode0 == MODE_STOP;
         const bool conv0 = c.conv0 != 0;                // FroErr1 wanted (stop layer or frozen)
-        float* s0 = p.s0;
-        const float* s1_old = p.s1[c.s1_buf];
-        float* s1_new = p.s1[c.s1_buf ^ 1];
-        __half* o0h = p.h[c.s0_buf ^ 1][0];
-        __half* o0l = p.h[c.s0_buf ^ 1][1];
-        __half* o1h = p.h[c.s1_buf ^ 1][2];
-        __half* o1l = p.h[c.s1_buf ^ 1][3];
+        EpiOut o0, o1;
+        o0.dst = p.s0; o0.old = p.s0;
+        o0.hi = p.h[c.s0_buf ^ 1][0]; o0.lo = p.h[c.s0_buf ^ 1][1];
+        o1.dst = p.s1[c.s1_buf ^ 1]; o1.old = p.s1[c.s1_buf];
+        o1.hi = p.h[c.s1_buf ^ 1][2]; o1.lo = p.h[c.s1_buf ^ 1][3];
 
-        double r_tr = 0.0, r_fs0 = 0.0, r_f0 = 0.0, r_f1 = 0.0;
-        float r_mx1 = 0.f;
+        double r_tr = 0.0, r_fs0 = 0.0, r_f0 = 0.0, r_f1 = 0.0, r_dummy = 0.0;
+        float r_mx1 = 0.f, r_mx_dummy = 0.f;
         int acc = 0;
         uint32_t acc_phase = 0;
         for (int t = blockIdx.x; t < p.num_tiles; t += gridDim.x) {
             const uint32_t tl = p.tiles[t];
             const int ti = (int)(tl & 0xFFFF), tj = (int)(tl >> 16);
-            const bool diag = ti == tj;
             const int gr = ti * kTile + q * 32 + lane;  // global row of this thread's TMEM lane
-            mbar_wait(tfull_bar(acc), acc_phase);
-            tc_fence_after();
-            const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + acc * 256;
-            for (int ch = 0; ch < kTile / 32; ++ch) {
-                if (diag && ch < q) continue;           // chunk strictly below the diagonal
-                const int gc0 = tj * kTile + ch * 32;
-                uint32_t v[32];
-                float f_tr = 0.f, f_fs0 = 0.f, f_f0 = 0.f, f_f1 = 0.f;
-                // ------------------------------------------------ order 0
-                if (with_x0) {
-                    tmem_ld_32x32(trow + ch * 32, v);
-                    float old[32];
-                    if (need_old0) {
+            const int gc_base = tj * kTile + half * kHalfCols;
+            float a0[kHalfCols], a1[kHalfCols];
 #pragma unroll
-                        for (int j = 0; j < 32; j += 4) {
-                            const float4 o = *reinterpret_cast<const float4*>(s0 + (size_t)gr * ld + gc0 + j);
-                            old[j] = o.x; old[j + 1] = o.y; old[j + 2] = o.z; old[j + 3] = o.w;
-                        }
-                    }
-                    tmem_ld_wait();
-                    if (upd0) {
-                        __half hh[32], ll[32];
-                        uint32_t ph[16], pl[16];
-                        float nw[32];
+            for (int j = 0; j < kHalfCols; ++j) { a0[j] = 0.f; a1[j] = 0.f; }
+            // ---- promoted accumulation: drain every chunk with round-to-nearest adds
+            for (int ch = 0; ch < num_chunks; ++ch) {
+                mbar_wait(tfull_bar(acc), acc_phase);
+                tc_fence_after();
+                const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + acc * 256 + half * kHalfCols;
+                uint32_t v[16];
+                if (with_p0) {
 #pragma unroll
-                        for (int j = 0; j < 32; ++j) {
-                            const float x = __uint_as_float(v[j]) * unscale0;
-                            const float s = need_old0 ? fmaf(keep, old[j], sig * x) : x;
-                            nw[j] = s;
-                            split_scaled(s, scale0, hh[j], ll[j]);
-                            if (j & 1) { ph[j >> 1] = pack2(hh[j - 1], hh[j]); pl[j >> 1] = pack2(ll[j - 1], ll[j]); }
-                            const int gc = gc0 + j;
-                            const float w = gr < gc ? 2.f : (gr == gc ? 1.f : 0.f);
-                            f_fs0 = fmaf(w * s, s, f_fs0);
-                            if (gr == gc) f_tr += s;
-                        }
-                        if (!diag) {
+                    for (int g = 0; g < kHalfCols / 16; ++g) {
+                        tmem_ld_32x16(trow + g * 16, v);
+                        tmem_ld_wait();
 #pragma unroll
-                            for (int j = 0; j < 32; j += 4)
-                                st_f4(s0 + (size_t)gr * ld + gc0 + j, nw[j], nw[j + 1], nw[j + 2], nw[j + 3]);
-                            st_h32(o0h + (size_t)gr * ld + gc0, ph);
-                            st_h32(o0l + (size_t)gr * ld + gc0, pl);
-#pragma unroll
-                            for (int j = 0; j < 32; ++j) {
-                                const size_t m = (size_t)(gc0 + j) * ld + gr;
-                                s0[m] = nw[j];
-                                o0h[m] = hh[j];
-                                o0l[m] = ll[j];
-                            }
-                        } else {
-#pragma unroll
-                            for (int j = 0; j < 32; ++j) {
-                                const int gc = gc0 + j;
-                                if (gr <= gc) {
-                                    const size_t dct = (size_t)gr * ld + gc;
-                                    s0[dct] = nw[j]; o0h[dct] = hh[j]; o0l[dct] = ll[j];
-                                }
-                                if (gr < gc) {
-                                    const size_t m = (size_t)gc * ld + gr;
-                                    s0[m] = nw[j]; o0h[m] = hh[j]; o0l[m] = ll[j];
-                                }
-                            }
-                        }
-                    } else {
-                        // D0 stop layer: FroErr0^2 = sum (S0 - X0)^2, S0 untouched (R4)
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) {
-                            const float x = __uint_as_float(v[j]) * unscale0;
-                            const int gc = gc0 + j;
-                            const float w = gr < gc ? 2.f : (gr == gc ? 1.f : 0.f);
-                            const float dlt = old[j] - x;
-                            f_f0 = fmaf(w * dlt, dlt, f_f0);
-                        }
+                        for (int j = 0; j < 16; ++j) a0[g * 16 + j] += __uint_as_float(v[j]);
                     }
                 }
-                // ------------------------------------------------ order 1
-                {
-                    tmem_ld_32x32(trow + 128 + ch * 32, v);
-                    float old[32];
-                    const bool need_old1 = c.sigma < 0 || conv0;
-                    if (need_old1) {
 #pragma unroll
-                        for (int j = 0; j < 32; j += 4) {
-                            const float4 o = *reinterpret_cast<const float4*>(s1_old + (size_t)gr * ld + gc0 + j);
-                            old[j] = o.x; old[j + 1] = o.y; old[j + 2] = o.z; old[j + 3] = o.w;
-                        }
-                    }
+                for (int g = 0; g < kHalfCols / 16; ++g) {
+                    tmem_ld_32x16(trow + 128 + g * 16, v);
                     tmem_ld_wait();
-                    __half hh[32], ll[32];
-                    uint32_t ph[16], pl[16];
-                    float nw[32];
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const float x = __uint_as_float(v[j]) * unscale1;
-                        const float s = need_old1 ? fmaf(keep, old[j], sig * x) : x;
-                        nw[j] = s;
-                        split_scaled(s, scale1, hh[j], ll[j]);
-                        if (j & 1) { ph[j >> 1] = pack2(hh[j - 1], hh[j]); pl[j >> 1] = pack2(ll[j - 1], ll[j]); }
-                        const int gc = gc0 + j;
-                        const bool in_upper = gr <= gc;
-                        if (in_upper) r_mx1 = fmaxf(r_mx1, fabsf(s));
-                        if (conv0) {
-                            const float w = gr < gc ? 2.f : (gr == gc ? 1.f : 0.f);
-                            const float dlt = old[j] - x;
-                            f_f1 = fmaf(w * dlt, dlt, f_f1);
-                        }
-                    }
-                    if (!diag) {
-#pragma unroll
-                        for (int j = 0; j < 32; j += 4)
-                            st_f4(s1_new + (size_t)gr * ld + gc0 + j, nw[j], nw[j + 1], nw[j + 2], nw[j + 3]);
-                        st_h32(o1h + (size_t)gr * ld + gc0, ph);
-                        st_h32(o1l + (size_t)gr * ld + gc0, pl);
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) {
-                            const size_t m = (size_t)(gc0 + j) * ld + gr;
-                            s1_new[m] = nw[j];
-                            o1h[m] = hh[j];
-                            o1l[m] = ll[j];
-                        }
-                    } else {
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) {
-                            const int gc = gc0 + j;
-                            if (gr <= gc) {
-                                const size_t dct = (size_t)gr * ld + gc;
-                                s1_new[dct] = nw[j]; o1h[dct] = hh[j]; o1l[dct] = ll[j];
-                            }
-                            if (gr < gc) {
-                                const size_t m = (size_t)gc * ld + gr;
-                                s1_new[m] = nw[j]; o1h[m] = hh[j]; o1l[m] = ll[j];
-                            }
-                        }
-                    }
+                    for (int j = 0; j < 16; ++j) a1[g * 16 + j] += __uint_as_float(v[j]);
                 }
-                r_tr += (double)f_tr;
-                r_fs0 += (double)f_fs0;
-                r_f0 += (double)f_f0;
-                r_f1 += (double)f_f1;
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(tempty_bar(acc));
+                if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
             }
-            // accumulators drained: hand the TMEM stage back to the MMA issuer
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(tempty_bar(acc));
-            if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
+            // ---- branch, update, re-split, reductions
+            const bool diag = ti == tj;
+            if (with_p0)
+                final_epilogue<0>(a0, o0, ld, gr, gc_base, diag, upd0, sig, unscale0, scale0, !upd0, r_tr, r_fs0,
+                                  r_f0, r_mx_dummy);
+            final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale1, scale1, conv0, r_dummy, r_dummy,
+                              r_f1, r_mx1);
         }
         // per-warp partials, fixed slot per (CTA, warp): the finalizer sums them in a fixed order
         r_tr = warp_sum(r_tr);
@@ -423,6 +440,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         if (lane == 0) {
             DmptCtl nc = *p.ctl;
             nc.ticket = 0;
+            nc.wave = 0;
             control_finalize(nc, p.logs, p.pb, red);
             *p.ctl = nc;
         }
