@@ -73,7 +73,10 @@ typedef struct dmpt_result {
     double fro_err0;           /* FroErr0 = ||S0 - S0^2||_F at the D0 stop layer        */
     double ms_total;           /* CUDA-event time of the whole run (bounds + transform + split + loop) */
     double ms_loop;            /* CUDA-event time of the layer loop alone ("time for main loop", Eq. 82)*/
-    double reserved_d[4];
+    double ms_bounds;          /* a1: Gershgorin kernel (+ scalar set-up)                                */
+    double ms_transform;       /* a2: initial transform kernel (+ first decision)                        */
+    double ms_split;           /* a3: the two initial split kernels                                      */
+    double reserved_d[1];
     /* Per-layer records, entry n-1 for layer n.  Caller-allocated HOST arrays of max_layers
      * entries each, or NULL to skip.  Entries the run did not reach are left untouched. */
     int8_t *sigma;             /* sigma_n                                         */
@@ -118,6 +121,22 @@ int dmpt_run_host(dmpt_ctx *ctx, const float *h_h0, const float *h_h1, int ld_in
  * stopping test).  Uses the context's workspace; invalidates nothing the caller owns. */
 int dmpt_layer_products(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, int ld,
                         float *d_x0, float *d_x1, int ld_out);
+
+/* The three HBM-bound steps on their own (tests and micro-benchmarks; dmpt_run does not call these
+ * entry points but launches the same kernels).  All run on the context's stream and return after it
+ * drained.  Matrices are n x n (n of dmpt_create), row-major, leading dimensions in elements.
+ *   a1  Gershgorin discs of d_h0 -> *h_eps_min, *h_eps_max (host).
+ *   a2  S0 = (eps_max I - H0)/W, S1 = -H1/W, W = eps_max - eps_min (Eq. 34, 493), each
+ *       element formed in fp64 and rounded once to fp32; *h_tr_s0 (host, may be NULL) = Tr S0.
+ *   a3  hi = fp16(2^shift x), lo = fp16(2^shift x - hi), round-to-nearest-even (Eq. 13);
+ *       d_hi, d_lo are device fp16 (uint16_t bit patterns), leading dimension ld_out.  diag_half != 0
+ *       splits x - I/2 instead (the form the order-0 operands take). */
+int dmpt_spectral_bounds(dmpt_ctx *ctx, const float *d_h0, int ld, double *h_eps_min, double *h_eps_max);
+int dmpt_initial_transform(dmpt_ctx *ctx, const float *d_h0, const float *d_h1, int ld,
+                           double eps_min, double eps_max, float *d_s0, float *d_s1, int ld_out,
+                           double *h_tr_s0);
+int dmpt_split(dmpt_ctx *ctx, const float *d_x, int ld, int shift, int diag_half,
+               uint16_t *d_hi, uint16_t *d_lo, int ld_out);
 
 int dmpt_destroy(dmpt_ctx *ctx);
 

@@ -18,6 +18,9 @@ from .binding import (  # noqa: F401
     dmpt_run,
     dmpt_run_host,
     dmpt_set_hamiltonian,
+    dmpt_spectral_bounds,
+    dmpt_initial_transform,
+    dmpt_split,
     dmpt_strerror,
     dmpt_workspace_bytes,
     lib,

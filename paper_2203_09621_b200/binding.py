@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libdmpt.so")
 EXPORTED_SYMBOLS = (
     "dmpt_default_options", "dmpt_workspace_bytes", "dmpt_create", "dmpt_set_hamiltonian",
     "dmpt_run", "dmpt_run_host", "dmpt_layer_products", "dmpt_destroy", "dmpt_strerror",
-    "dmpt_last_cuda_error",
+    "dmpt_last_cuda_error", "dmpt_spectral_bounds", "dmpt_initial_transform", "dmpt_split",
 )
 
 DMPT_OK, DMPT_EINVAL, DMPT_ESTATE, DMPT_ECUDA = 0, -1, -2, -3
@@ -36,7 +36,8 @@ class _CResult(C.Structure):
         ("status", C.c_int), ("layers", C.c_int), ("layers_d0", C.c_int), ("layers_d1", C.c_int),
         ("launches", C.c_int), ("reserved_i", C.c_int * 3),
         ("eps_min", C.c_double), ("eps_max", C.c_double), ("fro_err0", C.c_double),
-        ("ms_total", C.c_double), ("ms_loop", C.c_double), ("reserved_d", C.c_double * 4),
+        ("ms_total", C.c_double), ("ms_loop", C.c_double), ("ms_bounds", C.c_double),
+        ("ms_transform", C.c_double), ("ms_split", C.c_double), ("reserved_d", C.c_double * 1),
         ("sigma", C.POINTER(C.c_int8)), ("tr_s", C.POINTER(C.c_double)), ("tr_x", C.POINTER(C.c_double)),
         ("id_err", C.POINTER(C.c_double)), ("fro_err1", C.POINTER(C.c_double)),
         ("fro_err2", C.POINTER(C.c_double)),
@@ -81,6 +82,14 @@ def lib():
         L.dmpt_layer_products.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
                                           C.c_void_p, C.c_int]
         L.dmpt_layer_products.restype = C.c_int
+        L.dmpt_spectral_bounds.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double),
+                                           C.POINTER(C.c_double)]
+        L.dmpt_spectral_bounds.restype = C.c_int
+        L.dmpt_initial_transform.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_double,
+                                             C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double)]
+        L.dmpt_initial_transform.restype = C.c_int
+        L.dmpt_split.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int]
+        L.dmpt_split.restype = C.c_int
         L.dmpt_destroy.argtypes = [C.c_void_p]
         L.dmpt_destroy.restype = C.c_int
         L.dmpt_strerror.argtypes = [C.c_int]
@@ -141,6 +150,25 @@ def dmpt_layer_products(ctx, s0_ptr, s1_ptr, ld, x0_ptr, x1_ptr, ld_out) -> int:
                                          C.c_void_p(x0_ptr), C.c_void_p(x1_ptr), int(ld_out)))
 
 
+def dmpt_spectral_bounds(ctx, h0_ptr, ld):
+    lo, hi = C.c_double(), C.c_double()
+    rc = int(lib().dmpt_spectral_bounds(ctx, C.c_void_p(h0_ptr), int(ld), C.byref(lo), C.byref(hi)))
+    return rc, lo.value, hi.value
+
+
+def dmpt_initial_transform(ctx, h0_ptr, h1_ptr, ld, eps_min, eps_max, s0_ptr, s1_ptr, ld_out):
+    tr = C.c_double()
+    rc = int(lib().dmpt_initial_transform(ctx, C.c_void_p(h0_ptr), C.c_void_p(h1_ptr), int(ld), float(eps_min),
+                                          float(eps_max), C.c_void_p(s0_ptr), C.c_void_p(s1_ptr), int(ld_out),
+                                          C.byref(tr)))
+    return rc, tr.value
+
+
+def dmpt_split(ctx, x_ptr, ld, shift, diag_half, hi_ptr, lo_ptr, ld_out) -> int:
+    return int(lib().dmpt_split(ctx, C.c_void_p(x_ptr), int(ld), int(shift), int(diag_half), C.c_void_p(hi_ptr),
+                                C.c_void_p(lo_ptr), int(ld_out)))
+
+
 def dmpt_destroy(ctx) -> None:
     lib().dmpt_destroy(ctx)
 
@@ -158,6 +186,9 @@ class DmptResult:
     fro_err0: float
     ms_total: float
     ms_loop: float
+    ms_bounds: float = 0.0
+    ms_transform: float = 0.0
+    ms_split: float = 0.0
     sigma: list = field(default_factory=list)
     tr_s: list = field(default_factory=list)
     tr_x: list = field(default_factory=list)
@@ -224,7 +255,8 @@ class Dmpt:
         nl = max(0, int(r.layers))
         return DmptResult(status=rc, layers=r.layers, layers_d0=r.layers_d0, layers_d1=r.layers_d1,
                           launches=r.launches, eps_min=r.eps_min, eps_max=r.eps_max, fro_err0=r.fro_err0,
-                          ms_total=r.ms_total, ms_loop=r.ms_loop,
+                          ms_total=r.ms_total, ms_loop=r.ms_loop, ms_bounds=r.ms_bounds,
+                          ms_transform=r.ms_transform, ms_split=r.ms_split,
                           sigma=list(bufs["sigma"][:nl]), tr_s=list(bufs["tr_s"][:nl]),
                           tr_x=list(bufs["tr_x"][:nl]), id_err=list(bufs["id_err"][:nl]),
                           fro_err1=list(bufs["fro_err1"][:nl]), d0=d0, d1=d1, d2=d2)
@@ -268,6 +300,32 @@ class Dmpt:
         if rc != DMPT_OK:
             raise DmptError(rc, "dmpt_layer_products", dmpt_last_cuda_error(self.ctx))
         return x0, x1
+
+    def spectral_bounds(self, h0):
+        rc, lo, hi = dmpt_spectral_bounds(self.ctx, h0.data_ptr(), h0.stride(0))
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_spectral_bounds", dmpt_last_cuda_error(self.ctx))
+        return lo, hi
+
+    def initial_transform(self, h0, h1, eps_min, eps_max):
+        t = self.torch
+        s0 = t.empty((self.n, self.n), dtype=t.float32, device=self.device)
+        s1 = t.empty((self.n, self.n), dtype=t.float32, device=self.device)
+        rc, tr = dmpt_initial_transform(self.ctx, h0.data_ptr(), h1.data_ptr(), h0.stride(0), eps_min, eps_max,
+                                        s0.data_ptr(), s1.data_ptr(), self.n)
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_initial_transform", dmpt_last_cuda_error(self.ctx))
+        return s0, s1, tr
+
+    def split(self, x, shift=0, diag_half=False):
+        t = self.torch
+        hi = t.empty((self.n, self.n), dtype=t.float16, device=self.device)
+        lo = t.empty((self.n, self.n), dtype=t.float16, device=self.device)
+        rc = dmpt_split(self.ctx, x.data_ptr(), x.stride(0), shift, 1 if diag_half else 0, hi.data_ptr(),
+                        lo.data_ptr(), self.n)
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_split", dmpt_last_cuda_error(self.ctx))
+        return hi, lo
 
     def close(self):
         if getattr(self, "ctx", None) is not None:

@@ -114,7 +114,7 @@ struct dmpt_ctx {
     int s0_shift = 14;
     LayerParams lp{};
     cudaEvent_t ev[kNumEvents]{};
-    cudaEvent_t ev_t[4]{};
+    cudaEvent_t ev_t[6]{};       // 0 start, 1 loop start, 2 loop end, 3 end, 4 after bounds, 5 after transform
     int* h_flags = nullptr;      // pinned
     DmptCtl* h_ctl = nullptr;    // pinned
     char err[256] = {0};
@@ -351,16 +351,18 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     }
     dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, ctl, ctx->opt.bounds, ctx->opt.eps_min, ctx->opt.eps_max);
     CK(cudaGetLastError());
+    CK(cudaEventRecord(ctx->ev_t[4], st));
     const int tgrid = elementwise_grid(ctx, (long long)np * (np / 4), 256);
     dmpt_transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, d_h1, n, ld, np, ctx->lp.s0, ctx->lp.s1[0], ctl, partials);
     CK(cudaGetLastError());
     dmpt_control_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.logs, ctx->lp.pb, partials, tgrid);
     CK(cudaGetLastError());
+    CK(cudaEventRecord(ctx->ev_t[5], st));
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
     CK(cudaGetLastError());
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
     CK(cudaGetLastError());
     *launches += 6;
     CK(cudaEventRecord(ctx->ev_t[1], st));
@@ -415,6 +417,12 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
         res->ms_total = ms;
         CK(cudaEventElapsedTime(&ms, ctx->ev_t[1], ctx->ev_t[2]));
         res->ms_loop = ms;
+        CK(cudaEventElapsedTime(&ms, ctx->ev_t[0], ctx->ev_t[4]));
+        res->ms_bounds = ms;
+        CK(cudaEventElapsedTime(&ms, ctx->ev_t[4], ctx->ev_t[5]));
+        res->ms_transform = ms;
+        CK(cudaEventElapsedTime(&ms, ctx->ev_t[5], ctx->ev_t[1]));
+        res->ms_split = ms;
         const int nl = c.layers;
         if (nl > 0) {
             std::vector<int> sg(nl);
@@ -518,14 +526,91 @@ extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
     CK(cudaGetLastError());
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
     CK(cudaGetLastError());
     int rc = launch_layer(ctx);
     if (rc) return rc;
     CK(cudaMemcpy2DAsync(d_x0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpy2DAsync(d_x1, (size_t)ld_out * 4, ctx->lp.s1[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    return DMPT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1-a3 on their own: the same kernels dmpt_run launches, on caller matrices
+// ---------------------------------------------------------------------------------------------
+extern "C" int dmpt_spectral_bounds(dmpt_ctx* ctx, const float* d_h0, int ld, double* h_eps_min,
+                                    double* h_eps_max) {
+    if (!ctx || !d_h0 || !h_eps_min || !h_eps_max || ld < ctx->n) return DMPT_EINVAL;
+    const int n = ctx->n;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(ctx->L.ctl);
+    long long* bounds = ctx->at<long long>(ctx->L.bounds);
+    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    CK(cudaGetLastError());
+    const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
+    dmpt_gershgorin_kernel<<<grid, 256, 0, st>>>(d_h0, n, ld, bounds);
+    CK(cudaGetLastError());
+    long long hb[2];
+    CK(cudaMemcpyAsync(hb, bounds, sizeof hb, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    *h_eps_min = ordered_to_dbl(hb[0]);
+    *h_eps_max = ordered_to_dbl(hb[1]);
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_initial_transform(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
+                                      double eps_min, double eps_max, float* d_s0, float* d_s1, int ld_out,
+                                      double* h_tr_s0) {
+    if (!ctx || !d_h0 || !d_h1 || !d_s0 || !d_s1 || ld < ctx->n || ld_out < ctx->n) return DMPT_EINVAL;
+    const double w = eps_max - eps_min;
+    if (!(w > 0.0) || !isfinite(w)) return DMPT_EDEGENERATE;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    long long* bounds = ctx->at<long long>(L.bounds);
+    double* partials = ctx->at<double>(L.partials);
+    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    CK(cudaGetLastError());
+    dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, ctl, 1, eps_min, eps_max);
+    CK(cudaGetLastError());
+    const int tgrid = elementwise_grid(ctx, (long long)np * (np / 4), 256);
+    dmpt_transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, d_h1, (int)n, ld, (int)np, ctx->lp.s0, ctx->lp.s1[0], ctl, partials);
+    CK(cudaGetLastError());
+    CK(cudaMemcpy2DAsync(d_s0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpy2DAsync(d_s1, (size_t)ld_out * 4, ctx->lp.s1[0], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
+    std::vector<double> hp((size_t)tgrid * 3);
+    CK(cudaMemcpyAsync(hp.data(), partials, hp.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (h_tr_s0) {
+        double t = 0.0;
+        for (int b = 0; b < tgrid; ++b) t += hp[(size_t)b * 3];
+        *h_tr_s0 = t;
+    }
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_split(dmpt_ctx* ctx, const float* d_x, int ld, int shift, int diag_half, uint16_t* d_hi,
+                          uint16_t* d_lo, int ld_out) {
+    if (!ctx || !d_x || !d_hi || !d_lo || ld < ctx->n || ld_out < ctx->n || shift < 0 || shift > 15) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    double* partials = ctx->at<double>(L.partials);
+    const int grid = elementwise_grid(ctx, (long long)np * np, 256);
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_x, (int)n, ld, (int)np, ctx->lp.s0, partials);
+    CK(cudaGetLastError());
+    const long long c8 = (long long)np * np / 8;
+    const int sgrid = elementwise_grid(ctx, c8, 256);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, shift,
+                                             diag_half ? 1 : 0);
+    CK(cudaGetLastError());
+    CK(cudaMemcpy2DAsync(d_hi, (size_t)ld_out * 2, ctx->lp.h[0][0], np * 2, n * 2, n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpy2DAsync(d_lo, (size_t)ld_out * 2, ctx->lp.h[0][1], np * 2, n * 2, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaStreamSynchronize(st));
     return DMPT_OK;
 }

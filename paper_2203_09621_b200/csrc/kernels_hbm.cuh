@@ -235,7 +235,7 @@ __global__ void dmpt_control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProble
 //     (readings R12/R17): hi = fp16(2^e x), lo = fp16(2^e x - hi), round-to-nearest-even.
 //     8 elements per thread: two 128-bit loads, one 128-bit store per output.
 //     `which` selects the exponent on the device: 0 -> s0_shift, 1 -> ctl->e1_in, 2 -> ctl->e2_in.
-//     For which == 0 the matrix split is M = S0 - I/2 (residual form, layer_kernel.cuh).
+//     With diag_half the matrix split is M = S0 - I/2 (residual form, layer_kernel.cuh).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void split_scaled(float x, float scale, __half& hi, __half& lo) {
     const float t = x * scale;              // exact: scale is a power of two (barring overflow)
@@ -245,10 +245,11 @@ __device__ __forceinline__ void split_scaled(float x, float scale, __half& hi, _
 
 __global__ void __launch_bounds__(256) dmpt_split_kernel(const float* __restrict__ x, long long count8, int n_pad,
                                                          __half* __restrict__ hi, __half* __restrict__ lo,
-                                                         const DmptCtl* __restrict__ ctl, int which, int s0_shift) {
+                                                         const DmptCtl* __restrict__ ctl, int which, int s0_shift,
+                                                         int diag_half) {
     const int e = which == 0 ? s0_shift : (which == 1 ? ctl->e1_in : ctl->e2_in);
     const float scale = exp2f((float)e);
-    const float diag_shift = which == 0 ? 0.5f : 0.f;      // order 0: the operands hold M = S0 - I/2
+    const float diag_shift = diag_half ? 0.5f : 0.f;       // order 0: the operands hold M = S0 - I/2
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < count8;
          i += (long long)gridDim.x * blockDim.x) {
         const float4 v0 = ldg_stream4(x + i * 8);
