@@ -68,7 +68,8 @@ typedef struct dmpt_result {
     int layers_d0;     /* layer at which the D0 test fired (Algorithm 2); 0 if it never did           */
     int layers_d1;     /* layer at which the D1 test fired (Algorithm 3); 0 if it never did           */
     int launches;      /* kernels this run launched (all of them this library's own)                  */
-    int reserved_i[3];
+    int layers_d2;     /* order 2: layer at which the D2 test fired (R15); 0 otherwise            */
+    int reserved_i[2];
     double eps_min, eps_max;   /* spectral bounds used                                 */
     double fro_err0;           /* FroErr0 = ||S0 - S0^2||_F at the D0 stop layer        */
     double ms_total;           /* CUDA-event time of the whole run (bounds + transform + split + loop) */
@@ -121,6 +122,13 @@ int dmpt_run_host(dmpt_ctx *ctx, const float *h_h0, const float *h_h1, int ld_in
  * stopping test).  Uses the context's workspace; invalidates nothing the caller owns. */
 int dmpt_layer_products(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, int ld,
                         float *d_x0, float *d_x1, int ld_out);
+
+/* The order-2 product of one layer on its own (contexts created with order == 2 only; a9,
+ * PAPER.md:195 Eq. 25 third line, 201 Eq. 26): given symmetric S0, S1, S2 writes
+ * X2 = S0 S2 + S2 S0 + S1 S1, each of the three products in the dual half-precision form, through the
+ * split + tcgen05 path of the order-2 pass of a layer (sigma = +1, no stopping test). */
+int dmpt_layer_products2(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, const float *d_s2, int ld,
+                         float *d_x2, int ld_out);
 
 /* The three HBM-bound steps on their own (tests and micro-benchmarks; dmpt_run does not call these
  * entry points but launches the same kernels).  All run on the context's stream and return after it

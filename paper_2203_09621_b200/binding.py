@@ -16,6 +16,7 @@ EXPORTED_SYMBOLS = (
     "dmpt_default_options", "dmpt_workspace_bytes", "dmpt_create", "dmpt_set_hamiltonian",
     "dmpt_run", "dmpt_run_host", "dmpt_layer_products", "dmpt_destroy", "dmpt_strerror",
     "dmpt_last_cuda_error", "dmpt_spectral_bounds", "dmpt_initial_transform", "dmpt_split",
+    "dmpt_layer_products2",
 )
 
 DMPT_OK, DMPT_EINVAL, DMPT_ESTATE, DMPT_ECUDA = 0, -1, -2, -3
@@ -34,7 +35,7 @@ class DmptOptions(C.Structure):
 class _CResult(C.Structure):
     _fields_ = [
         ("status", C.c_int), ("layers", C.c_int), ("layers_d0", C.c_int), ("layers_d1", C.c_int),
-        ("launches", C.c_int), ("reserved_i", C.c_int * 3),
+        ("launches", C.c_int), ("layers_d2", C.c_int), ("reserved_i", C.c_int * 2),
         ("eps_min", C.c_double), ("eps_max", C.c_double), ("fro_err0", C.c_double),
         ("ms_total", C.c_double), ("ms_loop", C.c_double), ("ms_bounds", C.c_double),
         ("ms_transform", C.c_double), ("ms_split", C.c_double), ("reserved_d", C.c_double * 1),
@@ -82,6 +83,9 @@ def lib():
         L.dmpt_layer_products.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
                                           C.c_void_p, C.c_int]
         L.dmpt_layer_products.restype = C.c_int
+        L.dmpt_layer_products2.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
+                                           C.c_int]
+        L.dmpt_layer_products2.restype = C.c_int
         L.dmpt_spectral_bounds.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double),
                                            C.POINTER(C.c_double)]
         L.dmpt_spectral_bounds.restype = C.c_int
@@ -150,6 +154,11 @@ def dmpt_layer_products(ctx, s0_ptr, s1_ptr, ld, x0_ptr, x1_ptr, ld_out) -> int:
                                          C.c_void_p(x0_ptr), C.c_void_p(x1_ptr), int(ld_out)))
 
 
+def dmpt_layer_products2(ctx, s0_ptr, s1_ptr, s2_ptr, ld, x2_ptr, ld_out) -> int:
+    return int(lib().dmpt_layer_products2(ctx, C.c_void_p(s0_ptr), C.c_void_p(s1_ptr), C.c_void_p(s2_ptr), int(ld),
+                                          C.c_void_p(x2_ptr), int(ld_out)))
+
+
 def dmpt_spectral_bounds(ctx, h0_ptr, ld):
     lo, hi = C.c_double(), C.c_double()
     rc = int(lib().dmpt_spectral_bounds(ctx, C.c_void_p(h0_ptr), int(ld), C.byref(lo), C.byref(hi)))
@@ -189,11 +198,13 @@ class DmptResult:
     ms_bounds: float = 0.0
     ms_transform: float = 0.0
     ms_split: float = 0.0
+    layers_d2: int = 0
     sigma: list = field(default_factory=list)
     tr_s: list = field(default_factory=list)
     tr_x: list = field(default_factory=list)
     id_err: list = field(default_factory=list)
     fro_err1: list = field(default_factory=list)
+    fro_err2: list = field(default_factory=list)
     d0: object = None
     d1: object = None
     d2: object = None
@@ -259,7 +270,9 @@ class Dmpt:
                           ms_transform=r.ms_transform, ms_split=r.ms_split,
                           sigma=list(bufs["sigma"][:nl]), tr_s=list(bufs["tr_s"][:nl]),
                           tr_x=list(bufs["tr_x"][:nl]), id_err=list(bufs["id_err"][:nl]),
-                          fro_err1=list(bufs["fro_err1"][:nl]), d0=d0, d1=d1, d2=d2)
+                          fro_err1=list(bufs["fro_err1"][:nl]),
+                          fro_err2=list(bufs["fro_err2"][:nl]) if self.order == 2 else [],
+                          layers_d2=r.layers_d2, d0=d0, d1=d1, d2=d2)
 
     def run(self, out=None, check=True) -> DmptResult:
         t = self.torch
@@ -300,6 +313,15 @@ class Dmpt:
         if rc != DMPT_OK:
             raise DmptError(rc, "dmpt_layer_products", dmpt_last_cuda_error(self.ctx))
         return x0, x1
+
+    def layer_products2(self, s0, s1, s2):
+        t = self.torch
+        x2 = t.empty((self.n, self.n), dtype=t.float32, device=self.device)
+        rc = dmpt_layer_products2(self.ctx, s0.data_ptr(), s1.data_ptr(), s2.data_ptr(), s0.stride(0),
+                                  x2.data_ptr(), self.n)
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_layer_products2", dmpt_last_cuda_error(self.ctx))
+        return x2
 
     def spectral_bounds(self, h0):
         rc, lo, hi = dmpt_spectral_bounds(self.ctx, h0.data_ptr(), h0.stride(0))

@@ -52,6 +52,7 @@ struct DmptCtl {
     int single_shot;  // 1: dmpt_layer_products - run one layer, take no decisions
     unsigned int ticket;  // CTA arrival counter of the running launch
     unsigned int wave;    // wave-boundary arrivals of the running launch (LayerParams::wave_sync)
+    unsigned int wave2;   // the same for the order-2 pass of the layer
     double n_s;     // Tr S0_{n-1}
     double n_x;     // ||S0_{n-1}||_F^2
     double fro0;    // FroErr0

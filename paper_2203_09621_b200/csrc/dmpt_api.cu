@@ -37,7 +37,7 @@ struct Carve {
 
 struct Layout {
     int n, n_pad, order, num_tiles;
-    size_t ctl, bounds, sigma, tr_s, tr_x, id_err, fro1, fro2, partials, tiles;
+    size_t ctl, bounds, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, partials, partials2, tiles;
     size_t s0, s1[2], s2[2];
     size_t h[2][6];          // [buffer][S0hi, S0lo, S1hi, S1lo, S2hi, S2lo]
     size_t stage_h0, stage_h1;
@@ -57,6 +57,7 @@ Layout make_layout(int n, int order) {
     Carve c;
     L.ctl = c.take(sizeof(DmptCtl));
     L.bounds = c.take(2 * sizeof(long long));
+    L.s2_est = c.take(sizeof(unsigned long long));
     L.sigma = c.take(kMaxLayersCap * sizeof(int));
     L.tr_s = c.take(kMaxLayersCap * sizeof(double));
     L.tr_x = c.take(kMaxLayersCap * sizeof(double));
@@ -64,6 +65,7 @@ Layout make_layout(int n, int order) {
     L.fro1 = c.take(kMaxLayersCap * sizeof(double));
     L.fro2 = c.take(kMaxLayersCap * sizeof(double));
     L.partials = c.take(kPartialDoubles * sizeof(double));
+    L.partials2 = c.take(kPartialDoubles * sizeof(double));
     L.tiles = c.take((size_t)L.num_tiles * sizeof(uint32_t));
     L.s0 = c.take(np2 * 4);
     L.s1[0] = c.take(np2 * 4);
@@ -179,8 +181,9 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
     const cuuint64_t strides[1] = {(cuuint64_t)L.n_pad * 2};
     const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)kTile};
     const cuuint32_t estr[2] = {1, 1};
+    const int nh = L.order == 2 ? 6 : 4;
     for (int b = 0; b < 2; ++b)
-        for (int m = 0; m < 4; ++m) {
+        for (int m = 0; m < nh; ++m) {
             CUresult r = encode(&ctx->lp.maps[b][m], CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
                                 ctx->at<void>(L.h[b][m]), dims, strides, box, estr,
                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
@@ -203,7 +206,6 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     if (o.max_layers <= 0) o.max_layers = 200;
     if (o.max_layers > kMaxLayersCap) o.max_layers = kMaxLayersCap;
     if (o.s0_shift > 15) return DMPT_EINVAL;
-    if (o.order == 2) return DMPT_EINVAL;   // second order: not built yet (row a9)
     const size_t need = dmpt_workspace_bytes(n, o.order);
     if (need == 0) return DMPT_EINVAL;
     if (workspace_bytes < need || (reinterpret_cast<uintptr_t>(d_workspace) & 255)) return DMPT_EWORKSPACE;
@@ -246,7 +248,8 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     for (auto& e : ctx->ev_t) CKC(cudaEventCreate(&e));
     CKC(cudaHostAlloc(&ctx->h_flags, kFlagSlots * sizeof(int), cudaHostAllocDefault));
     CKC(cudaHostAlloc(&ctx->h_ctl, sizeof(DmptCtl), cudaHostAllocDefault));
-    CKC(cudaFuncSetAttribute(dmpt_layer_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    CKC(cudaFuncSetAttribute(dmpt_layer_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<0>()));
+    CKC(cudaFuncSetAttribute(dmpt_layer_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<1>()));
 
     const Layout& L = ctx->L;
     const int nb = L.n_pad / kTile;
@@ -262,8 +265,11 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.s0 = ctx->at<float>(L.s0);
     lp.s1[0] = ctx->at<float>(L.s1[0]);
     lp.s1[1] = ctx->at<float>(L.s1[1]);
-    for (int b = 0; b < 2; ++b)
-        for (int m = 0; m < 4; ++m) lp.h[b][m] = ctx->at<__half>(L.h[b][m]);
+    const int nh = o.order == 2 ? 6 : 4;
+    for (int b = 0; b < 2; ++b) {
+        lp.s2[b] = o.order == 2 ? ctx->at<float>(L.s2[b]) : nullptr;
+        for (int m = 0; m < 6; ++m) lp.h[b][m] = m < nh ? ctx->at<__half>(L.h[b][m]) : nullptr;
+    }
     lp.tiles = ctx->at<uint32_t>(L.tiles);
     lp.num_tiles = L.num_tiles;
     lp.n_pad = L.n_pad;
@@ -276,6 +282,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.logs.fro1 = ctx->at<double>(L.fro1);
     lp.logs.fro2 = ctx->at<double>(L.fro2);
     lp.partials = ctx->at<double>(L.partials);
+    lp.partials2 = ctx->at<double>(L.partials2);
     lp.pb.n = n;
     lp.pb.n_pad = L.n_pad;
     lp.pb.n_occ = 0;
@@ -311,17 +318,30 @@ extern "C" int dmpt_set_hamiltonian(dmpt_ctx* ctx, const float* d_h0, const floa
     return DMPT_OK;
 }
 
-static int launch_layer(dmpt_ctx* ctx) {
+template <int PASS>
+static int launch_pass(dmpt_ctx* ctx) {
     if (ctx->lp.wave_sync) {
         // the wave barrier needs every CTA resident: a cooperative launch guarantees it or fails
         void* args[] = {&ctx->lp};
-        CK(cudaLaunchCooperativeKernel((const void*)dmpt_layer_kernel, dim3(ctx->grid_layer), dim3(kNumThreads),
-                                       args, kSmemBytes, ctx->stream));
+        CK(cudaLaunchCooperativeKernel((const void*)dmpt_layer_kernel<PASS>, dim3(ctx->grid_layer),
+                                       dim3(kNumThreads), args, smem_bytes<PASS>(), ctx->stream));
     } else {
-        dmpt_layer_kernel<<<ctx->grid_layer, kNumThreads, kSmemBytes, ctx->stream>>>(ctx->lp);
+        dmpt_layer_kernel<PASS><<<ctx->grid_layer, kNumThreads, smem_bytes<PASS>(), ctx->stream>>>(ctx->lp);
         CK(cudaGetLastError());
     }
     return DMPT_OK;
+}
+
+// One layer: at order 2 the S2 pass goes first (it reads the iterates pass 0 is about to replace and
+// leaves its reductions for pass 0's control step).
+static int launch_layer(dmpt_ctx* ctx, int* launches) {
+    if (ctx->opt.order == 2) {
+        int rc = launch_pass<1>(ctx);
+        if (rc) return rc;
+        ++*launches;
+    }
+    ++*launches;
+    return launch_pass<0>(ctx);
 }
 
 static int elementwise_grid(const dmpt_ctx* ctx, long long work_items, int threads) {
@@ -365,6 +385,19 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
     CK(cudaGetLastError());
     *launches += 6;
+    if (ctx->opt.order == 2) {      // S2_0 = 0 (H2 = 0): fp32 iterate and its operands
+        const size_t np2 = (size_t)np * np;
+        CK(cudaMemsetAsync(ctx->lp.s2[0], 0, np2 * 4, st));
+        CK(cudaMemsetAsync(ctx->lp.h[0][4], 0, np2 * 2, st));
+        CK(cudaMemsetAsync(ctx->lp.h[0][5], 0, np2 * 2, st));
+        unsigned long long* est = ctx->at<unsigned long long>(L.s2_est);
+        CK(cudaMemsetAsync(est, 0, sizeof *est, st));
+        dmpt_rowsq_max_kernel<<<elementwise_grid(ctx, (long long)np * 32, 256), 256, 0, st>>>(ctx->lp.s1[0], np, est);
+        CK(cudaGetLastError());
+        dmpt_s2_scale_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, est);
+        CK(cudaGetLastError());
+        *launches += 2;
+    }
     CK(cudaEventRecord(ctx->ev_t[1], st));
 
     // Layer loop.  Launches are enqueued in chunks, two chunks ahead of the GPU; after each chunk a
@@ -374,9 +407,8 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     int launched = 0, chunks = 0;
     auto launch_chunk = [&]() -> int {
         for (int i = 0; i < chunk_len && launched < max_layers; ++i, ++launched) {
-            int rc = launch_layer(ctx);
+            int rc = launch_layer(ctx, launches);
             if (rc) return rc;
-            ++*launches;
         }
         CK(cudaMemcpyAsync(&ctx->h_flags[chunks % kFlagSlots], &ctl->done, sizeof(int), cudaMemcpyDeviceToHost, st));
         CK(cudaEventRecord(ctx->ev[chunks % kNumEvents], st));
@@ -408,6 +440,7 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
         res->layers = c.layers;
         res->layers_d0 = c.n_c;
         res->layers_d1 = c.n_c1;
+        res->layers_d2 = c.n_c2;
         res->launches = launches;
         res->eps_min = c.eps_min;
         res->eps_max = c.eps_max;
@@ -434,6 +467,8 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
             if (res->tr_x) CK(cudaMemcpy(res->tr_x, ctx->at<double>(L.tr_x), nl * sizeof(double), cudaMemcpyDeviceToHost));
             if (res->id_err) CK(cudaMemcpy(res->id_err, ctx->at<double>(L.id_err), nl * sizeof(double), cudaMemcpyDeviceToHost));
             if (res->fro_err1) CK(cudaMemcpy(res->fro_err1, ctx->at<double>(L.fro1), nl * sizeof(double), cudaMemcpyDeviceToHost));
+            if (res->fro_err2 && ctx->opt.order == 2)
+                CK(cudaMemcpy(res->fro_err2, ctx->at<double>(L.fro2), nl * sizeof(double), cudaMemcpyDeviceToHost));
         }
     }
     return status;
@@ -460,6 +495,9 @@ extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, in
     CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
     CK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
                          cudaMemcpyDeviceToDevice, ctx->stream));
+    if (ctx->opt.order == 2)
+        CK(cudaMemcpy2DAsync(d_d2, (size_t)ld * 4, ctx->lp.s2[ctx->h_ctl->s2_buf & 1], np * 4, n * 4, n,
+                             cudaMemcpyDeviceToDevice, ctx->stream));
     return finish(ctx, res, launches);
 }
 
@@ -484,6 +522,9 @@ extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1
     CK(cudaMemcpy2DAsync(h_d0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaMemcpy2DAsync(h_d1, (size_t)ld_out * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
                          cudaMemcpyDeviceToHost, ctx->stream));
+    if (ctx->opt.order == 2)
+        CK(cudaMemcpy2DAsync(h_d2, (size_t)ld_out * 4, ctx->lp.s2[ctx->h_ctl->s2_buf & 1], np * 4, n * 4, n,
+                             cudaMemcpyDeviceToHost, ctx->stream));
     return finish(ctx, res, launches);
 }
 
@@ -492,10 +533,12 @@ extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1
 // ---------------------------------------------------------------------------------------------
 namespace {
 __global__ void single_shot_init_kernel(DmptCtl* ctl, DmptProblem pb, const double* __restrict__ partials,
-                                        int nblocks) {
+                                        const double* __restrict__ partials2 /* max|S2| or NULL */, int nblocks) {
     if (threadIdx.x | blockIdx.x) return;
-    double m = 0.0;
+    double m = 0.0, m2 = 0.0;
     for (int b = 0; b < nblocks; ++b) m = fmax(m, partials[b]);
+    if (partials2)
+        for (int b = 0; b < nblocks; ++b) m2 = fmax(m2, partials2[b]);
     DmptCtl c;
     memset(&c, 0, sizeof c);
     c.layer = 1;
@@ -504,6 +547,8 @@ __global__ void single_shot_init_kernel(DmptCtl* ctl, DmptProblem pb, const doub
     c.single_shot = 1;
     c.s1_max = m;
     c.e1_in = c.e1_out = pb.s1_autoscale ? scale_exponent(m) : 0;
+    c.s2_max = m2;
+    c.e2_in = c.e2_out = pb.s1_autoscale ? scale_exponent(m2) : 0;
     *ctl = c;
 }
 }  // namespace
@@ -522,7 +567,7 @@ extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float
     CK(cudaGetLastError());
     dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s1, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
     CK(cudaGetLastError());
-    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, grid);
+    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, nullptr, grid);
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
@@ -530,10 +575,44 @@ extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float
     CK(cudaGetLastError());
     dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
     CK(cudaGetLastError());
-    int rc = launch_layer(ctx);
+    int rc = launch_pass<0>(ctx);
     if (rc) return rc;
     CK(cudaMemcpy2DAsync(d_x0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpy2DAsync(d_x1, (size_t)ld_out * 4, ctx->lp.s1[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_layer_products2(dmpt_ctx* ctx, const float* d_s0, const float* d_s1, const float* d_s2, int ld,
+                                    float* d_x2, int ld_out) {
+    if (!ctx || !d_s0 || !d_s1 || !d_s2 || !d_x2) return DMPT_EINVAL;
+    if (ld < ctx->n || ld_out < ctx->n || ctx->opt.order != 2) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    double* partials = ctx->at<double>(L.partials);
+    double* partials2 = ctx->at<double>(L.partials2);
+    const int grid = elementwise_grid(ctx, (long long)np * np, 256);
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s0, (int)n, ld, (int)np, ctx->lp.s0, partials);
+    CK(cudaGetLastError());
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s1, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
+    CK(cudaGetLastError());
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s2, (int)n, ld, (int)np, ctx->lp.s2[0], partials2);
+    CK(cudaGetLastError());
+    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, partials2, grid);
+    CK(cudaGetLastError());
+    const long long c8 = (long long)np * np / 8;
+    const int sgrid = elementwise_grid(ctx, c8, 256);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
+    CK(cudaGetLastError());
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
+    CK(cudaGetLastError());
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s2[0], c8, (int)np, ctx->lp.h[0][4], ctx->lp.h[0][5], ctl, 2, ctx->s0_shift, 0);
+    CK(cudaGetLastError());
+    int rc = launch_pass<1>(ctx);
+    if (rc) return rc;
+    CK(cudaMemcpy2DAsync(d_x2, (size_t)ld_out * 4, ctx->lp.s2[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaStreamSynchronize(st));
     return DMPT_OK;
 }

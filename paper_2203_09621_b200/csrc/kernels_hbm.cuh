@@ -231,6 +231,38 @@ __global__ void dmpt_control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProble
 }
 
 // ---------------------------------------------------------------------------------------------
+// Order 2 only: the scale of the FIRST split of S2.  S2_0 = 0, so S2_1 = sigma_1 S1_0 S1_0 and, by
+// Cauchy-Schwarz, max|S2_1| = max_i sum_k (S1_0)_ik^2 (attained on the diagonal).  One warp per row
+// of the padded S1_0; the maximum lands in *est as the bit pattern of a non-negative double
+// (ordered like an unsigned integer).  dmpt_s2_scale_init_kernel then sets e2_out (reading R12).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dmpt_rowsq_max_kernel(const float* __restrict__ s1, int n_pad,
+                                                             unsigned long long* __restrict__ est) {
+    const int warps_per_block = blockDim.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    double mx = 0.0;
+    for (int row = blockIdx.x * warps_per_block + warp; row < n_pad; row += gridDim.x * warps_per_block) {
+        const float* p = s1 + (size_t)row * n_pad;
+        double acc = 0.0;
+        for (int j = lane * 4; j < n_pad; j += 128) {
+            const float4 v = ldg_stream4(p + j);
+            acc += (double)(v.x * v.x + v.y * v.y) + (double)(v.z * v.z + v.w * v.w);
+        }
+        mx = fmax(mx, warp_sum(acc));
+    }
+    if (lane == 0 && mx > 0.0 && isfinite(mx)) atomicMax(est, (unsigned long long)__double_as_longlong(mx));
+}
+
+__global__ void dmpt_s2_scale_init_kernel(DmptCtl* ctl, DmptProblem pb, const unsigned long long* __restrict__ est) {
+    if (threadIdx.x | blockIdx.x) return;
+    const double m = __longlong_as_double((long long)*est);
+    ctl->s2_max = m;
+    ctl->e2_in = 0;
+    ctl->e2_out = pb.s1_autoscale ? scale_exponent(m) : 0;
+}
+
+// ---------------------------------------------------------------------------------------------
 // a3  Split (Eq. 13, 302-307 Eqs. 42-43) after an exact power-of-two scale 2^e
 //     (readings R12/R17): hi = fp16(2^e x), lo = fp16(2^e x - hi), round-to-nearest-even.
 //     8 elements per thread: two 128-bit loads, one 128-bit store per output.

@@ -46,10 +46,12 @@ namespace dmpt {
 constexpr int kTile = 128;                 // output tile edge (rows of panel I x rows of panel J)
 constexpr int kBK = 32;                    // fp16 per k-block: 64-byte rows, SWIZZLE_64B
 constexpr int kRowBytes = kBK * 2;
-constexpr int kStages = 3;
 constexpr int kOpBytes = kTile * kRowBytes;          // 8 KiB per operand tile
-constexpr int kOpsPerStage = 8;
-constexpr int kStageBytes = kOpBytes * kOpsPerStage; // 64 KiB
+// PASS 0 (orders 0 and 1): 8 operand tiles per k-block (64 KiB), 3 stages.
+// PASS 1 (order 2):       12 operand tiles per k-block (96 KiB), 2 stages.
+template <int PASS> struct PassCfg;
+template <> struct PassCfg<0> { static constexpr int kOps = 8, kStages = 3; };
+template <> struct PassCfg<1> { static constexpr int kOps = 12, kStages = 2; };
 constexpr int kChunkK = 128;               // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
@@ -59,16 +61,21 @@ constexpr int kNumEpiWarps = 8;
 constexpr int kNumThreads = 32 * (kEpiWarp0 + kNumEpiWarps);   // 320
 constexpr int kHalfCols = kTile / 2;       // accumulator columns per epilogue thread and product
 constexpr int kSub = 16;                   // columns per step of the final epilogue
-constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+template <int PASS>
+constexpr int smem_bytes() {
+    return PassCfg<PASS>::kStages * PassCfg<PASS>::kOps * kOpBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+}
 
 // operand slots inside a stage (A = row panel I, B = row panel J)
-enum Op : int { AMH = 0, AML = 1, A1H = 2, A1L = 3, BMH = 4, BML = 5, B1H = 6, B1L = 7 };
+enum Op : int { AMH = 0, AML = 1, A1H = 2, A1L = 3, BMH = 4, BML = 5, B1H = 6, B1L = 7,
+                A2H = 8, A2L = 9, B2H = 10, B2L = 11 };
 
 struct LayerParams {
-    CUtensorMap maps[2][4];     // [buffer][Mhi, Mlo, S1hi, S1lo], box = kBK x kTile, SWIZZLE_64B
+    CUtensorMap maps[2][6];     // [buffer][Mhi, Mlo, S1hi, S1lo, S2hi, S2lo], box = kBK x kTile, SWIZZLE_64B
     float* s0;                  // fp32 S0, updated in place, ld = n_pad
     float* s1[2];               // fp32 S1, ping-pong
-    __half* h[2][4];            // fp16 operand matrices the epilogue writes, same order as maps
+    float* s2[2];               // fp32 S2, ping-pong (order 2)
+    __half* h[2][6];            // fp16 operand matrices the epilogue writes, same order as maps
     const uint32_t* tiles;      // (I | J << 16), I <= J, in launch order
     int num_tiles;
     int n_pad;
@@ -76,7 +83,8 @@ struct LayerParams {
     DmptCtl* ctl;
     DmptLogs logs;
     DmptProblem pb;
-    double* partials;           // [gridDim.x][kNumEpiWarps][RED_COUNT]
+    double* partials;           // [gridDim.x][kNumEpiWarps][RED_COUNT], written by PASS 0
+    double* partials2;          // same shape, written by PASS 1 (RED_FRO2, RED_MAX2)
 };
 
 __device__ __forceinline__ uint32_t pack2(__half a, __half b) {
@@ -181,11 +189,25 @@ __device__ __forceinline__ void final_epilogue(float (&acc)[kHalfCols], const Ep
     }
 }
 
+
+// PASS 0: orders 0 and 1 of layer n (P0 = M.M, P1 = M.S1 + S1.M); its last CTA runs Algorithms 2-3.
+// PASS 1: order 2 of layer n (a9, Eq. 25 third line, 201 Eq. 26):
+//             V2 = X2 - S2 = (M.S2 + S2.M) + S1.S1,   S2 <- S2 + sigma V2,
+//         two accumulators again: Q = S1.S1 (3 products, scale 2^(2 e1)) and P2 = M.S2 + S2.M (6 products,
+//         scale 2^(a + e2)), combined in fp32 in the epilogue.  Launched BEFORE pass 0 of the same layer: it
+//         reads the operands of S0_{n-1}, S1_{n-1}, S2_{n-1} and the decision pass 0 of layer n-1 left in
+//         DmptCtl, writes S2_n into the other buffer and leaves ||V2||_F^2, max|S2_n| in partials2.
+template <int PASS>
 __global__ void __launch_bounds__(kNumThreads, 1)
 dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
+    constexpr int kOps = PassCfg<PASS>::kOps;
+    constexpr int kStages = PassCfg<PASS>::kStages;
+    constexpr int kStageBytes = kOps * kOpBytes;
     // ---- the decision for this layer, taken by the previous launch
     const DmptCtl c = *p.ctl;
     if (c.done) return;
+    // order 2 after the D1 stop: S0 and S1 are frozen, pass 0 only runs the control step
+    const bool idle = PASS == 0 && c.conv1 != 0;
 
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -202,12 +224,15 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const int num_chunks = p.n_pad / kChunkK;
-    const bool with_p0 = c.mode0 != MODE_FROZEN;
+    const int num_tiles = idle ? 0 : p.num_tiles;
+    const bool with_p0 = PASS == 1 || c.mode0 != MODE_FROZEN;     // first accumulator in use
+    unsigned int* wave_ctr = PASS == 0 ? &p.ctl->wave : &p.ctl->wave2;
 
     if (warp == 0 && lane == 0) {
         for (int m = 0; m < 2; ++m) {
             prefetch_tensormap(&p.maps[c.s0_buf][m]);
             prefetch_tensormap(&p.maps[c.s1_buf][2 + m]);
+            if (PASS == 1) prefetch_tensormap(&p.maps[c.s2_buf][4 + m]);
         }
         for (int s = 0; s < kStages; ++s) {
             mbar_init(full_bar(s), 1);
@@ -235,20 +260,22 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             const CUtensorMap* mml = &p.maps[c.s0_buf][1];
             const CUtensorMap* m1h = &p.maps[c.s1_buf][2];
             const CUtensorMap* m1l = &p.maps[c.s1_buf][3];
+            const CUtensorMap* m2h = &p.maps[c.s2_buf][4];
+            const CUtensorMap* m2l = &p.maps[c.s2_buf][5];
             const int num_kb = p.n_pad / kBK;
             int stage = 0;
             uint32_t phase = 0;
             unsigned int wave = 0;
-            const unsigned int num_waves = (p.num_tiles + gridDim.x - 1) / gridDim.x;
-            for (int t = blockIdx.x; t < p.num_tiles; t += gridDim.x, ++wave) {
+            const unsigned int num_waves = (num_tiles + gridDim.x - 1) / gridDim.x;
+            for (int t = blockIdx.x; t < num_tiles; t += gridDim.x, ++wave) {
                 if (p.wave_sync && wave > 0) {
                     // re-align the K phase of all CTAs: tiles in flight then stream the same k-blocks of
                     // few row panels at the same time and share them through L2
                     __threadfence();
-                    atomicAdd(&p.ctl->wave, 1u);
+                    atomicAdd(wave_ctr, 1u);
                     const unsigned int target = gridDim.x * wave;
                     unsigned int spins = 0;
-                    while (ld_acquire_u32(&p.ctl->wave) < target) {
+                    while (ld_acquire_u32(wave_ctr) < target) {
                         __nanosleep(64);
                         if (++spins > (1u << 26)) __trap();
                     }
@@ -269,11 +296,17 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                     tma_load_2d(base + B1H * kOpBytes, m1h, fb, k0, row_j);
                     tma_load_2d(base + A1L * kOpBytes, m1l, fb, k0, row_i);
                     tma_load_2d(base + B1L * kOpBytes, m1l, fb, k0, row_j);
+                    if (PASS == 1) {
+                        tma_load_2d(base + A2H * kOpBytes, m2h, fb, k0, row_i);
+                        tma_load_2d(base + B2H * kOpBytes, m2h, fb, k0, row_j);
+                        tma_load_2d(base + A2L * kOpBytes, m2l, fb, k0, row_i);
+                        tma_load_2d(base + B2L * kOpBytes, m2l, fb, k0, row_j);
+                    }
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
             // CTAs with fewer tiles still owe their arrivals to the later waves
-            if (p.wave_sync && wave < num_waves && wave > 0) atomicAdd(&p.ctl->wave, num_waves - wave);
+            if (p.wave_sync && wave < num_waves && wave > 0) atomicAdd(wave_ctr, num_waves - wave);
         }
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
@@ -283,34 +316,46 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             uint32_t phase = 0;
             int acc = 0;
             uint32_t acc_phase = 0;
-            for (int t = blockIdx.x; t < p.num_tiles; t += gridDim.x) {
+            for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
                 for (int ch = 0; ch < num_chunks; ++ch) {
                     mbar_wait(tempty_bar(acc), acc_phase ^ 1);
                     tc_fence_after();
-                    const uint32_t d0 = tmem_base + acc * 256;        // P0 accumulator columns
-                    const uint32_t d1 = d0 + 128;                     // P1 accumulator columns
+                    const uint32_t d0 = tmem_base + acc * 256;        // P0 (pass 1: Q) accumulator columns
+                    const uint32_t d1 = d0 + 128;                     // P1 (pass 1: P2) accumulator columns
                     for (int kb = 0; kb < kKbPerChunk; ++kb) {
                         mbar_wait(full_bar(stage), phase);
                         tc_fence_after();
                         const uint32_t base = smem_base + stage * kStageBytes;
-                        uint64_t d[kOpsPerStage];
+                        uint64_t d[kOps];
 #pragma unroll
-                        for (int o = 0; o < kOpsPerStage; ++o) d[o] = make_smem_desc<kRowBytes>(base + o * kOpBytes);
+                        for (int o = 0; o < kOps; ++o) d[o] = make_smem_desc<kRowBytes>(base + o * kOpBytes);
 #pragma unroll
                         for (int ks = 0; ks < kBK / 16; ++ks) {
                             const uint64_t adv = (uint64_t)(ks * 32 >> 4);     // 16 fp16 = 32 bytes along K
                             const uint32_t first = (kb | ks) != 0;
-                            if (with_p0) {
-                                umma_f16<1>(d0, d[AMH] + adv, d[BMH] + adv, idesc, first);   // hi.hi
-                                umma_f16<1>(d0, d[AMH] + adv, d[BML] + adv, idesc, 1);       // hi.lo
-                                umma_f16<1>(d0, d[AML] + adv, d[BMH] + adv, idesc, 1);       // lo.hi
+                            if (PASS == 0) {
+                                if (with_p0) {
+                                    umma_f16<1>(d0, d[AMH] + adv, d[BMH] + adv, idesc, first);   // hi.hi
+                                    umma_f16<1>(d0, d[AMH] + adv, d[BML] + adv, idesc, 1);       // hi.lo
+                                    umma_f16<1>(d0, d[AML] + adv, d[BMH] + adv, idesc, 1);       // lo.hi
+                                }
+                                umma_f16<1>(d1, d[AMH] + adv, d[B1H] + adv, idesc, first);       // M.S1
+                                umma_f16<1>(d1, d[A1H] + adv, d[BMH] + adv, idesc, 1);           // S1.M
+                                umma_f16<1>(d1, d[AMH] + adv, d[B1L] + adv, idesc, 1);
+                                umma_f16<1>(d1, d[AML] + adv, d[B1H] + adv, idesc, 1);
+                                umma_f16<1>(d1, d[A1H] + adv, d[BML] + adv, idesc, 1);
+                                umma_f16<1>(d1, d[A1L] + adv, d[BMH] + adv, idesc, 1);
+                            } else {
+                                umma_f16<1>(d0, d[A1H] + adv, d[B1H] + adv, idesc, first);       // S1.S1
+                                umma_f16<1>(d0, d[A1H] + adv, d[B1L] + adv, idesc, 1);
+                                umma_f16<1>(d0, d[A1L] + adv, d[B1H] + adv, idesc, 1);
+                                umma_f16<1>(d1, d[AMH] + adv, d[B2H] + adv, idesc, first);       // M.S2
+                                umma_f16<1>(d1, d[A2H] + adv, d[BMH] + adv, idesc, 1);           // S2.M
+                                umma_f16<1>(d1, d[AMH] + adv, d[B2L] + adv, idesc, 1);
+                                umma_f16<1>(d1, d[AML] + adv, d[B2H] + adv, idesc, 1);
+                                umma_f16<1>(d1, d[A2H] + adv, d[BML] + adv, idesc, 1);
+                                umma_f16<1>(d1, d[A2L] + adv, d[BMH] + adv, idesc, 1);
                             }
-                            umma_f16<1>(d1, d[AMH] + adv, d[B1H] + adv, idesc, first);       // M.S1
-                            umma_f16<1>(d1, d[A1H] + adv, d[BMH] + adv, idesc, 1);           // S1.M
-                            umma_f16<1>(d1, d[AMH] + adv, d[B1L] + adv, idesc, 1);
-                            umma_f16<1>(d1, d[AML] + adv, d[B1H] + adv, idesc, 1);
-                            umma_f16<1>(d1, d[A1H] + adv, d[BML] + adv, idesc, 1);
-                            umma_f16<1>(d1, d[A1L] + adv, d[BMH] + adv, idesc, 1);
                         }
                         umma_commit(empty_bar(stage));                 // frees the smem stage
                         if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -330,19 +375,28 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         const float unscale1 = exp2f(-(float)(p.pb.s0_shift + c.e1_in));
         const float scale0 = exp2f((float)p.pb.s0_shift);
         const float scale1 = exp2f((float)c.e1_out);
+        const float unscale_q = exp2f(-2.f * (float)c.e1_in);                     // S1.S1 sums
+        const float unscale2 = exp2f(-(float)(p.pb.s0_shift + c.e2_in));          // M.S2 + S2.M sums
+        const float scale2 = exp2f((float)c.e2_out);
         const bool upd0 = c.mode0 == MODE_ACTIVE;
         const bool conv0 = c.conv0 != 0;                // FroErr1 wanted (stop layer or frozen)
         EpiOut o0, o1;
-        o0.dst = p.s0; o0.old = p.s0;
-        o0.hi = p.h[c.s0_buf ^ 1][0]; o0.lo = p.h[c.s0_buf ^ 1][1];
-        o1.dst = p.s1[c.s1_buf ^ 1]; o1.old = p.s1[c.s1_buf];
-        o1.hi = p.h[c.s1_buf ^ 1][2]; o1.lo = p.h[c.s1_buf ^ 1][3];
+        if (PASS == 0) {
+            o0.dst = p.s0; o0.old = p.s0;
+            o0.hi = p.h[c.s0_buf ^ 1][0]; o0.lo = p.h[c.s0_buf ^ 1][1];
+            o1.dst = p.s1[c.s1_buf ^ 1]; o1.old = p.s1[c.s1_buf];
+            o1.hi = p.h[c.s1_buf ^ 1][2]; o1.lo = p.h[c.s1_buf ^ 1][3];
+        } else {
+            o0.dst = nullptr; o0.old = nullptr; o0.hi = nullptr; o0.lo = nullptr;
+            o1.dst = p.s2[c.s2_buf ^ 1]; o1.old = p.s2[c.s2_buf];
+            o1.hi = p.h[c.s2_buf ^ 1][4]; o1.lo = p.h[c.s2_buf ^ 1][5];
+        }
 
         double r_tr = 0.0, r_fs0 = 0.0, r_f0 = 0.0, r_f1 = 0.0, r_dummy = 0.0;
         float r_mx1 = 0.f, r_mx_dummy = 0.f;
         int acc = 0;
         uint32_t acc_phase = 0;
-        for (int t = blockIdx.x; t < p.num_tiles; t += gridDim.x) {
+        for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
             const uint32_t tl = p.tiles[t];
             const int ti = (int)(tl & 0xFFFF), tj = (int)(tl >> 16);
             const int gr = ti * kTile + q * 32 + lane;  // global row of this thread's TMEM lane
@@ -379,11 +433,19 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             }
             // ---- branch, update, re-split, reductions
             const bool diag = ti == tj;
-            if (with_p0)
-                final_epilogue<0>(a0, o0, ld, gr, gc_base, diag, upd0, sig, unscale0, scale0, !upd0, r_tr, r_fs0,
-                                  r_f0, r_mx_dummy);
-            final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale1, scale1, conv0, r_dummy, r_dummy,
-                              r_f1, r_mx1);
+            if (PASS == 0) {
+                if (with_p0)
+                    final_epilogue<0>(a0, o0, ld, gr, gc_base, diag, upd0, sig, unscale0, scale0, !upd0, r_tr, r_fs0,
+                                      r_f0, r_mx_dummy);
+                final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale1, scale1, conv0, r_dummy,
+                                  r_dummy, r_f1, r_mx1);
+            } else {
+                // V2 = 2^-(a+e2) P2 + 2^-(2 e1) Q: both factors are powers of two, one fp32 rounding per element
+#pragma unroll
+                for (int j = 0; j < kHalfCols; ++j) a1[j] = fmaf(unscale_q, a0[j], unscale2 * a1[j]);
+                final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, 1.f, scale2, true, r_dummy, r_dummy,
+                                  r_f1, r_mx1);
+            }
         }
         // per-warp partials, fixed slot per (CTA, warp): the finalizer sums them in a fixed order
         r_tr = warp_sum(r_tr);
@@ -392,24 +454,28 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         r_f1 = warp_sum(r_f1);
         const double mx1 = warp_max((double)r_mx1);
         if (lane == 0) {
-            double* out = p.partials + ((size_t)blockIdx.x * kNumEpiWarps + (warp - kEpiWarp0)) * RED_COUNT;
+            double* out = (PASS == 0 ? p.partials : p.partials2) +
+                          ((size_t)blockIdx.x * kNumEpiWarps + (warp - kEpiWarp0)) * RED_COUNT;
             out[RED_TR_S0] = r_tr;
             out[RED_FRO_S0] = r_fs0;
             out[RED_FRO0] = r_f0;
-            out[RED_FRO1] = r_f1;
-            out[RED_MAX1] = mx1;
-            out[RED_FRO2] = 0.0;
-            out[RED_MAX2] = 0.0;
+            out[RED_FRO1] = PASS == 0 ? r_f1 : 0.0;
+            out[RED_MAX1] = PASS == 0 ? mx1 : 0.0;
+            out[RED_FRO2] = PASS == 1 ? r_f1 : 0.0;
+            out[RED_MAX2] = PASS == 1 ? mx1 : 0.0;
         }
     }
 
-    // ---- teardown, then the last CTA of the launch runs Algorithms 2-3 for this layer
+    // ---- teardown
     tc_fence_before();
     __syncthreads();
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc<1>(tmem_base, kTmemCols);
     }
+    if (PASS == 1) return;          // pass 0 of the same layer follows on the stream and takes the decisions
+
+    // ---- the last CTA of the launch runs Algorithms 2-3 for this layer
     __shared__ int is_last;
     if (threadIdx.x == 0) {
         __threadfence();
@@ -426,9 +492,12 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         for (int k = 0; k < RED_COUNT; ++k) red[k] = 0.0;
         for (int s = lane; s < nslots; s += 32) {
             const volatile double* in = p.partials + (size_t)s * RED_COUNT;
+            const volatile double* in2 = p.partials2 + (size_t)s * RED_COUNT;
 #pragma unroll
             for (int k = 0; k < RED_COUNT; ++k) {
-                if (k == RED_MAX1 || k == RED_MAX2) red[k] = fmax(red[k], in[k]);
+                if (k == RED_MAX1) red[k] = fmax(red[k], in[k]);
+                else if (k == RED_MAX2) { if (p.pb.order == 2) red[k] = fmax(red[k], in2[k]); }
+                else if (k == RED_FRO2) { if (p.pb.order == 2) red[k] += in2[k]; }
                 else red[k] += in[k];
             }
         }
@@ -441,6 +510,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             DmptCtl nc = *p.ctl;
             nc.ticket = 0;
             nc.wave = 0;
+            nc.wave2 = 0;
             control_finalize(nc, p.logs, p.pb, red);
             *p.ctl = nc;
         }

@@ -387,9 +387,14 @@ def test_error_codes(dev):
     assert r.status == p.binding.DMPT_ENOCONV and r.layers == 5
     assert torch.isfinite(r.d0).all() and torch.isfinite(r.d1).all()
     s.close()
-    # order 2 is not built yet: refused at create time, loudly
+    # the order-2 product entry point needs an order-2 context
+    s = _solver(128, dev)
+    with pytest.raises(p.DmptError) as e:
+        s.layer_products2(h0, h1, h1)
+    assert e.value.code == p.binding.DMPT_EINVAL
+    s.close()
     with pytest.raises(p.DmptError):
-        _solver(128, dev, order=2)
+        _solver(128, dev, order=3)
 
 
 def test_caller_supplied_bounds(dev, config1):
@@ -406,3 +411,83 @@ def test_caller_supplied_bounds(dev, config1):
     assert (res.eps_min, res.eps_max) == bounds
     _check_against(ref.d0, ref.d1, wl.n_occ, d0, d1)
     assert ref.layers - 8 <= res.layers <= ref.layers + 2
+
+
+# ------------------------------------------------------------------------------------------
+# a9: second order
+# ------------------------------------------------------------------------------------------
+TOL_D2 = 5e-4      # relative to max|D2_ref|: the D1 tolerance of north_star carried to the next order
+
+
+@pytest.mark.parametrize("n", [40, 128, 333, 640])
+def test_layer_products2_match_fp64(dev, n):
+    """X2 = S0 S2 + S2 S0 + S1 S1 (Eq. 25 third line, 201 Eq. 26) through the order-2 pass."""
+    rng = np.random.default_rng(13 * n)
+    a = rng.uniform(-1, 1, size=(n, n)) / np.sqrt(n)
+    s0 = ((a + a.T) / 2 + np.diag(rng.uniform(0, 1, size=n))).astype(np.float32)
+    b = rng.standard_normal((n, n))
+    s1 = (0.37 * (b + b.T)).astype(np.float32)
+    c = rng.standard_normal((n, n))
+    s2 = (2.1e-3 * (c + c.T)).astype(np.float32)
+    s = _solver(n, dev, order=2)
+    x2 = s.layer_products2(*(torch.from_numpy(m).to(dev) for m in (s0, s1, s2))).double().cpu().numpy()
+    s.close()
+    s0d, s1d, s2d = (m.astype(np.float64) for m in (s0, s1, s2))
+    p2 = s0d @ s2d
+    ref = p2 + p2.T + s1d @ s1d
+    m = np.abs(s0d - 0.5 * np.eye(n))
+    bound = (C_PROD * (m @ np.abs(s2d) + np.abs(s2d) @ m + np.abs(s1d) @ np.abs(s1d)) + 3e-7 * np.abs(ref)
+             + 1e-7 * np.abs(s2d).max())
+    assert np.all(np.abs(x2 - ref) <= bound), f"X2: worst ratio {np.max(np.abs(x2 - ref) / bound):.2f}"
+    assert np.array_equal(x2, x2.T)
+
+
+def _run2(wl, dev, **kw):
+    s = _solver(wl.n, dev, order=2, **kw)
+    s.set_hamiltonian(torch.from_numpy(wl.h0).to(dev), torch.from_numpy(wl.h1).to(dev), wl.n_occ)
+    res = s.run()
+    out = tuple(m.double().cpu().numpy() for m in (res.d0, res.d1, res.d2))
+    s.close()
+    return res, out
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 256), (5, 512), (5, 1284), (4, 1024)])
+def test_second_order_matches_oracle(dev, cfg, n):
+    """Order 2 at sizes the oracle finishes in seconds: O2 at order 2 (Algorithms 1-3 with the cascaded
+    stop, reading R15) and, through it, the definition O1 (the two agree to 1e-9, test_oracle_pins)."""
+    from oracle.dnn_sp2_pt import dnn_sp2_pt
+    from workloads import make_config
+
+    wl = make_config(cfg, n=n)
+    ref = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, order=2)
+    assert ref.status == "ok"
+    res, (d0, d1, d2) = _run2(wl, dev)
+    assert res.status == 0
+    _check_against(ref.d0, ref.d1, wl.n_occ, d0, d1)
+    e2 = np.abs(d2 - ref.d2).max() / np.abs(ref.d2).max()
+    assert e2 <= TOL_D2, f"max|D2 - ref|/max|D2_ref| = {e2:.3e}"
+    assert np.array_equal(d2, d2.T)
+    assert ref.layers - 8 <= res.layers <= ref.layers + 2
+    # the first-order part of an order-2 run is the order-1 run (same kernels, same decisions)
+    r1, e0, e1 = _run(wl, dev)
+    assert r1.layers == res.layers_d1 and res.layers_d2 == res.layers
+    assert np.array_equal(e0, d0) and np.array_equal(e1, d1)
+    # cascade (R15): D0 stop, then D1 stop >= 2 layers later, then D2 stop >= 2 layers after that
+    assert res.layers_d0 + 2 <= res.layers_d1 and res.layers_d1 + 2 <= res.layers
+    assert len(res.fro_err2) == res.layers and np.isfinite(res.fro_err2[res.layers_d1 - 1])
+
+
+def test_second_order_special_cases(dev):
+    from workloads import make_config
+
+    wl = make_config(1, n=192)
+    # H1 = 0 -> D1 = D2 = 0 exactly
+    wl0 = make_config(1, n=192)
+    wl0.h1 = np.zeros_like(wl.h1)
+    res, (d0, d1, d2) = _run2(wl0, dev)
+    assert res.status == 0 and np.abs(d1).max() == 0.0 and np.abs(d2).max() == 0.0
+    # D2 is quadratic in H1 (exercises the per-layer power-of-two scales of S1 and S2)
+    base = _run2(wl, dev)[1]
+    wl.h1 = (wl.h1 * np.float32(2.0 ** -10)).astype(np.float32)
+    tiny = _run2(wl, dev)[1]
+    assert np.abs(tiny[2] * 2.0 ** 20 - base[2]).max() <= 1e-5 * np.abs(base[2]).max()
