@@ -491,3 +491,80 @@ def test_second_order_special_cases(dev):
     wl.h1 = (wl.h1 * np.float32(2.0 ** -10)).astype(np.float32)
     tiny = _run2(wl, dev)[1]
     assert np.abs(tiny[2] * 2.0 ** 20 - base[2]).max() <= 1e-5 * np.abs(base[2]).max()
+
+
+def _definition2_fp64_on_device(h0_32, h1_32, n_occ, dev, mu=None):
+    """D0, D1, D2 of oracle/closed_form.py restated with torch fp64 on the device (cross-reference, not the
+    oracle; pinned to it in test_fp64_cross_reference_order2_is_pinned_to_the_oracle).  Returns device fp64."""
+    from workloads.linalg import eigh_any
+
+    n = h0_32.shape[0]
+    eps, v = eigh_any(h0_32.to(dev).double(), mu)                 # mu: only read above the solver's size limit
+    vo = v[:, :n_occ]
+    d0 = vo @ vo.T
+    a = v.T @ (h1_32.to(dev).double() @ v)                        # H1 in the eigenbasis of H0
+    y = torch.zeros((n, n), dtype=torch.float64, device=dev)
+    de = eps[:n_occ, None] - eps[None, n_occ:]                    # occupied - virtual level spacings
+    y[:n_occ, n_occ:] = a[:n_occ, n_occ:] / de                    # PAPER.md:371-375 (Eqs. 53-54)
+    y[n_occ:, :n_occ] = y[:n_occ, n_occ:].T
+    d1 = v @ y @ v.T
+    z = torch.zeros((n, n), dtype=torch.float64, device=dev)      # order-2 blocks of D^2 = D, [H, D] = 0
+    you = y[:n_occ, n_occ:]
+    z[:n_occ, :n_occ] = -(you @ you.T)
+    z[n_occ:, n_occ:] = you.T @ you
+    z[:n_occ, n_occ:] = (you @ a[n_occ:, n_occ:] - a[:n_occ, :n_occ] @ you) / de
+    z[n_occ:, :n_occ] = z[:n_occ, n_occ:].T
+    del a, y, you, de
+    d2 = v @ z @ v.T
+    return d0, d1, d2
+
+
+def test_fp64_cross_reference_order2_is_pinned_to_the_oracle(dev, config1):
+    from oracle.closed_form import density_matrices
+
+    wl = config1
+    d0, d1, d2 = density_matrices(wl.h0, wl.h1, wl.n_occ, order=2)
+    x0, x1, x2 = (m.cpu().numpy() for m in
+                  _definition2_fp64_on_device(torch.from_numpy(wl.h0), torch.from_numpy(wl.h1), wl.n_occ, dev))
+    assert np.abs(d0 - x0).max() <= 1e-11 and np.abs(d1 - x1).max() <= 1e-11 * max(1.0, np.abs(d1).max())
+    assert np.abs(d2 - x2).max() <= 1e-10 * max(1.0, np.abs(d2).max())
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("n", [4096, 32768])
+def test_config5_second_order_full_size(dev, n):
+    """Config 5 (N = 32768, N_occ = 16384, order 2; 4096 as a quicker sibling) in the launch configuration
+    of a full run.  The fp64 oracle would need ~15 h there, so the values come from the
+    DEFINITION evaluated with a device fp64 eigendecomposition of the same rounded inputs (cross-reference
+    pinned to oracle O1 above), all three matrices compared element by element on the device."""
+    from workloads import make_config
+
+    wl = make_config(5, n=n, device="cuda")
+    h0 = torch.from_numpy(wl.h0)
+    h1 = torch.from_numpy(wl.h1)
+    s = _solver(wl.n, dev, order=2)
+    s.set_hamiltonian(h0.to(dev), h1.to(dev), wl.n_occ)
+    res = s.run()
+    assert res.status == 0
+    d0, d1, d2 = res.d0, res.d1, res.d2
+    s.close()
+    del s
+    torch.cuda.empty_cache()
+    for m in (d0, d1, d2):
+        assert torch.equal(m, m.T)
+    assert abs(float(torch.diagonal(d0).double().sum()) - wl.n_occ) <= TOL_TR
+    r0, r1, r2 = _definition2_fp64_on_device(h0, h1, wl.n_occ, dev, mu=wl.meta["mu"])
+
+    def maxdiff(x, ref):       # row blocks: no second fp64 copy of a 8 GiB matrix
+        e = 0.0
+        for i in range(0, x.shape[0], 4096):
+            e = max(e, float((x[i:i + 4096].double() - ref[i:i + 4096]).abs().max()))
+        return e
+
+    e0 = maxdiff(d0, r0)
+    e1 = maxdiff(d1, r1) / float(r1.abs().max())
+    e2 = maxdiff(d2, r2) / float(r2.abs().max())
+    print(f"config 5 @ n={n}: layers {res.layers} (D0 {res.layers_d0}, D1 {res.layers_d1}) gap {wl.meta['gap']:.3f} "
+          f"max|D0 err| {e0:.2e} D1 {e1:.2e} D2 {e2:.2e} loop {res.ms_loop:.0f} ms")
+    assert e0 <= TOL_D0 and e1 <= TOL_D1 and e2 <= TOL_D2, (e0, e1, e2)
+    assert res.layers_d0 + 2 <= res.layers_d1 and res.layers_d1 + 2 <= res.layers <= res.layers_d1 + 6

@@ -81,14 +81,29 @@ def _eigh(h: np.ndarray, device):
     return np.linalg.eigh(h)
 
 
-def _sym_round32(h: np.ndarray) -> np.ndarray:
-    """Symmetrise in fp64, round once to fp32; result is exactly symmetric."""
-    h = 0.5 * (h + h.T)
-    h32 = h.astype(np.float32)
-    # (a+b)/2 is commutative in IEEE arithmetic, so h is already bit-symmetric;
+def _mirror_upper(h: np.ndarray, blk: int = 2048) -> None:
+    """Copy the strict upper triangle onto the lower one, in place, block by block."""
+    n = h.shape[0]
+    for r0 in range(0, n, blk):
+        r1 = min(n, r0 + blk)
+        h[r0:r1, :r0] = h[:r0, r0:r1].T
+        d = h[r0:r1, r0:r1]
+        iu = np.triu_indices(r1 - r0, 1)
+        d.T[iu] = d[iu]
+
+
+def _sym_round32(h: np.ndarray, blk: int = 2048) -> np.ndarray:
+    """Symmetrise in fp64, round once to fp32; result is exactly symmetric.
+
+    Row blocks keep the temporaries small (N = 32768: 8 GiB per fp64 matrix)."""
+    n = h.shape[0]
+    h32 = np.empty((n, n), dtype=np.float32)
+    for r0 in range(0, n, blk):
+        r1 = min(n, r0 + blk)
+        h32[r0:r1] = (0.5 * (h[r0:r1] + h[:, r0:r1].T)).astype(np.float32)
+    # (a+b)/2 is commutative in IEEE arithmetic, so h32 is already bit-symmetric;
     # keep the upper triangle anyway so that symmetry never depends on that.
-    iu = np.triu_indices(h32.shape[0], 1)
-    h32.T[iu] = h32[iu]
+    _mirror_upper(h32, blk)
     return h32
 
 
@@ -140,30 +155,45 @@ def tight_binding_cube(rng, n_atoms, density=0.1, decay=1.5, onsite_sigma=0.3, o
         d = pos[atom[r0:r1], None, :] - pos[None, atom, :]
         r = np.sqrt(np.einsum("ijk,ijk->ij", d, d))
         h0[r0:r1, :] = -np.exp(-r / decay) * u
-    iu = np.triu_indices(n, 1)
-    h0.T[iu] = h0[iu]
+    _mirror_upper(h0)
     h0[np.arange(n), np.arange(n)] = onsite
     return h0, pos, atom
 
 
-def _scissor(h0: np.ndarray, n_occ: int, target_gap: float, device):
+def _scissor(h0: np.ndarray, n_occ: int, target_gap: float, device, mu_hint=None):
     """Open the HOMO-LUMO gap to `target_gap`.
 
     H0 <- H0 + delta * (I - 2 V_occ V_occ^T): occupied levels move down by delta and
     virtual levels up by delta, eigenvectors unchanged.  Returns (H0', eps', gap before).
     """
+    if _use_torch(device):
+        # everything on the device; only the shifted matrix comes back (N = 32768: 8 GiB per matrix)
+        import torch
+
+        from .linalg import eigh_any
+
+        ht = torch.from_numpy(h0).to(device)
+        wt, v = eigh_any(ht, mu_hint)
+        w = wt.cpu().numpy()
+        gap0 = float(w[n_occ] - w[n_occ - 1])
+        delta = max(0.0, 0.5 * (target_gap - gap0))
+        if delta > 0.0:
+            vo = v[:, :n_occ]
+            del v
+            ht.addmm_(vo, vo.T, beta=1.0, alpha=-2.0 * delta)
+            ht.diagonal().add_(delta)
+            h0 = ht.cpu().numpy()
+            w[:n_occ] -= delta
+            w[n_occ:] += delta
+        del ht
+        torch.cuda.empty_cache()
+        return h0, w, gap0
     w, v = _eigh(h0, device)
     gap0 = float(w[n_occ] - w[n_occ - 1])
     delta = max(0.0, 0.5 * (target_gap - gap0))
     if delta > 0.0:
         vo = v[:, :n_occ]
-        if _use_torch(device):
-            import torch
-
-            vt = torch.from_numpy(vo).to(device)
-            p = (vt @ vt.T).cpu().numpy()
-        else:
-            p = vo @ vo.T
+        p = vo @ vo.T
         h0 = h0 + delta * (np.eye(h0.shape[0]) - 2.0 * p)
         w = w.copy()
         w[:n_occ] -= delta
@@ -206,6 +236,7 @@ def make_config(index: int, n: int | None = None, device=None, seed: int | None 
         h0, eps, _q = gapped_random_orthogonal(rng, n, n_occ, cfg["occ"], cfg["virt"], device)
         del _q
         meta["gap"] = float(eps[n_occ] - eps[n_occ - 1])
+        meta["mu"] = float(0.5 * (eps[n_occ] + eps[n_occ - 1]))
         meta["spectrum"] = (float(eps[0]), float(eps[-1]))
         pos = atom = None
     else:
@@ -213,9 +244,21 @@ def make_config(index: int, n: int | None = None, device=None, seed: int | None 
             raise ValueError("tight-binding configs need n divisible by 4")
         h0, pos, atom = tight_binding_cube(rng, n // 4)
         if scissor:
-            h0, eps, gap0 = _scissor(h0, n_occ, cfg["gap"], device)
+            mu_hint = None
+            from .linalg import EIGH_DIRECT_MAX
+
+            if _use_torch(device) and n > EIGH_DIRECT_MAX:
+                # the device eigensolver refuses this size (workloads/linalg.py): split the spectrum near
+                # the Fermi level, located on a small sibling of the same generator (same density of states)
+                sib, _, _ = tight_binding_cube(np.random.default_rng(meta["seed"] + 7919), 1024)
+                ws = np.linalg.eigvalsh(sib)
+                k = int(round(cfg["fill"] * ws.shape[0]))
+                mu_hint = 0.5 * (ws[k - 1] + ws[k])
+                del sib
+            h0, eps, gap0 = _scissor(h0, n_occ, cfg["gap"], device, mu_hint)
             meta["gap_literal"] = gap0
             meta["gap"] = float(eps[n_occ] - eps[n_occ - 1])
+            meta["mu"] = float(0.5 * (eps[n_occ] + eps[n_occ - 1]))
             meta["spectrum"] = (float(eps[0]), float(eps[-1]))
         else:
             meta["gap"] = None
@@ -224,11 +267,15 @@ def make_config(index: int, n: int | None = None, device=None, seed: int | None 
         h1 = symmetric_gaussian(rng, n, cfg["h1_scale"])
     else:
         axis = {"dipole_x": 0, "dipole_y": 1, "dipole_z": 2}[cfg["h1"]]
-        h1 = np.diag(pos[atom, axis])
+        h1 = None
 
     h0_32 = _sym_round32(h0)
     del h0
-    h1_32 = _sym_round32(h1)
-    del h1
+    if h1 is None:      # dipole field: diagonal, already symmetric; rounded once like everything else
+        h1_32 = np.zeros((n, n), dtype=np.float32)
+        h1_32[np.arange(n), np.arange(n)] = pos[atom, axis].astype(np.float32)
+    else:
+        h1_32 = _sym_round32(h1)
+        del h1
     return Workload(name=cfg["name"] if n == cfg["n"] else f'{cfg["name"]} @ n={n}',
                     n=n, n_occ=n_occ, order=cfg["order"], h0=h0_32, h1=h1_32, meta=meta)
