@@ -44,13 +44,18 @@ struct Layout {
     size_t total;
 };
 
-int num_tiles_for(int nb) { return nb * (nb + 1) / 2; }
+// pair tiles (IP, J): block rows 2 IP, 2 IP + 1 x block column J >= 2 IP, nb even
+int num_tiles_for(int nb) {
+    int t = 0;
+    for (int ip = 0; ip < nb / 2; ++ip) t += nb - 2 * ip;
+    return t;
+}
 
 Layout make_layout(int n, int order) {
     Layout L{};
     L.n = n;
     L.order = order;
-    L.n_pad = (int)align_up((size_t)n, kTile);
+    L.n_pad = (int)align_up((size_t)n, kPair);
     const int nb = L.n_pad / kTile;
     L.num_tiles = num_tiles_for(nb);
     const size_t np2 = (size_t)L.n_pad * L.n_pad;
@@ -83,15 +88,16 @@ Layout make_layout(int n, int order) {
     return L;
 }
 
-// Launch order of the upper-triangular tiles: bands of `band` block rows, column by column inside
-// a band, so that the ~#SM tiles in flight share few row panels (L2 reuse of the operand panels).
+// Launch order of the upper-triangular pair tiles: bands of `band` pair rows, column by column inside
+// a band, so that the ~#SM/2 pair tiles in flight share few row panels (L2 reuse of the operand panels).
 std::vector<uint32_t> make_tile_order(int nb, int band) {
     std::vector<uint32_t> t;
     t.reserve(num_tiles_for(nb));
-    for (int b0 = 0; b0 < nb; b0 += band) {
-        const int b1 = b0 + band < nb ? b0 + band : nb;
-        for (int j = b0; j < nb; ++j)
-            for (int i = b0; i < b1 && i <= j; ++i) t.push_back((uint32_t)i | ((uint32_t)j << 16));
+    const int nbp = nb / 2;
+    for (int b0 = 0; b0 < nbp; b0 += band) {
+        const int b1 = b0 + band < nbp ? b0 + band : nbp;
+        for (int j = 2 * b0; j < nb; ++j)
+            for (int ip = b0; ip < b1 && 2 * ip <= j; ++ip) t.push_back((uint32_t)ip | ((uint32_t)j << 16));
     }
     return t;
 }
@@ -179,7 +185,7 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
     const Layout& L = ctx->L;
     const cuuint64_t dims[2] = {(cuuint64_t)L.n_pad, (cuuint64_t)L.n_pad};
     const cuuint64_t strides[1] = {(cuuint64_t)L.n_pad * 2};
-    const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)kTile};
+    const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)kBRows};
     const cuuint32_t estr[2] = {1, 1};
     const int nh = L.order == 2 ? 6 : 4;
     for (int b = 0; b < 2; ++b)
@@ -255,11 +261,26 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     const int nb = L.n_pad / kTile;
     int band = 1;
     while ((band + 1) * (band + 1) <= ctx->num_sms) ++band;      // ~sqrt(#SM) block rows per band
+    band = band / 2 > 0 ? band / 2 : 1;                          // ... in pair rows
     std::vector<uint32_t> tiles = make_tile_order(nb, band);
     CKC(cudaMemcpyAsync(ctx->at<void>(L.tiles), tiles.data(), tiles.size() * sizeof(uint32_t),
                         cudaMemcpyHostToDevice, ctx->stream));
     CKC(cudaStreamSynchronize(ctx->stream));
-    ctx->grid_layer = L.num_tiles < ctx->num_sms ? L.num_tiles : ctx->num_sms;
+    // one CTA pair (cluster of 2, one TPC) per pair tile in flight
+    int max_clusters = 0;
+    {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(ctx->num_sms & ~1);
+        cfg.blockDim = dim3(kNumThreads);
+        cfg.dynamicSmemBytes = smem_bytes<1>();
+        CKC(cudaOccupancyMaxActiveClusters(&max_clusters, dmpt_layer_kernel<1>, &cfg));
+    }
+    if (max_clusters < 1) {
+        snprintf(ctx->err, sizeof ctx->err, "no CTA pair of the layer kernel fits this device");
+        return fail(DMPT_ECUDA);
+    }
+    if (max_clusters > ctx->num_sms / 2) max_clusters = ctx->num_sms / 2;
+    ctx->grid_layer = 2 * (L.num_tiles < max_clusters ? L.num_tiles : max_clusters);
 
     LayerParams& lp = ctx->lp;
     lp.s0 = ctx->at<float>(L.s0);
@@ -273,7 +294,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.tiles = ctx->at<uint32_t>(L.tiles);
     lp.num_tiles = L.num_tiles;
     lp.n_pad = L.n_pad;
-    lp.wave_sync = (o.wave_sync && L.num_tiles > ctx->grid_layer) ? 1 : 0;
+    lp.wave_sync = (o.wave_sync && L.num_tiles > ctx->grid_layer / 2) ? 1 : 0;
     lp.ctl = ctx->at<DmptCtl>(L.ctl);
     lp.logs.sigma = ctx->at<int>(L.sigma);
     lp.logs.tr_s = ctx->at<double>(L.tr_s);
@@ -320,15 +341,19 @@ extern "C" int dmpt_set_hamiltonian(dmpt_ctx* ctx, const float* d_h0, const floa
 
 template <int PASS>
 static int launch_pass(dmpt_ctx* ctx) {
-    if (ctx->lp.wave_sync) {
-        // the wave barrier needs every CTA resident: a cooperative launch guarantees it or fails
-        void* args[] = {&ctx->lp};
-        CK(cudaLaunchCooperativeKernel((const void*)dmpt_layer_kernel<PASS>, dim3(ctx->grid_layer),
-                                       dim3(kNumThreads), args, smem_bytes<PASS>(), ctx->stream));
-    } else {
-        dmpt_layer_kernel<PASS><<<ctx->grid_layer, kNumThreads, smem_bytes<PASS>(), ctx->stream>>>(ctx->lp);
-        CK(cudaGetLastError());
-    }
+    // clusters of 2 come from the kernel's __cluster_dims__; the wave barrier needs every CTA resident:
+    // a cooperative launch guarantees it or fails
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(ctx->grid_layer);
+    cfg.blockDim = dim3(kNumThreads);
+    cfg.dynamicSmemBytes = smem_bytes<PASS>();
+    cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = ctx->lp.wave_sync ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    CK(cudaLaunchKernelEx(&cfg, dmpt_layer_kernel<PASS>, ctx->lp));
     return DMPT_OK;
 }
 

@@ -46,13 +46,19 @@ namespace dmpt {
 constexpr int kTile = 128;                 // output tile edge (rows of panel I x rows of panel J)
 constexpr int kBK = 32;                    // fp16 per k-block: 64-byte rows, SWIZZLE_64B
 constexpr int kRowBytes = kBK * 2;
-constexpr int kOpBytes = kTile * kRowBytes;          // 8 KiB per operand tile
-// PASS 0 (orders 0 and 1): 8 operand tiles per k-block (64 KiB), 3 stages.
-// PASS 1 (order 2):       12 operand tiles per k-block (96 KiB), 2 stages.
+constexpr int kPair = 2 * kTile;           // rows of a CTA-pair tile (UMMA M = 256, cta_group::2)
+constexpr int kBRows = kTile / 2;          // rows of the J panel each CTA of the pair stages (half of UMMA N)
+constexpr int kABytes = kTile * kRowBytes;           // 8 KiB per A-side operand tile (this CTA's 128 rows of panel I)
+constexpr int kBBytes = kBRows * kRowBytes;          // 4 KiB per B-side operand tile (this CTA's 64 rows of panel J)
+// Per CTA and k-block: PASS 0 (orders 0 and 1) stages 4 A + 4 B tiles (48 KiB), 4 stages;
+//                      PASS 1 (order 2) stages 6 A + 6 B tiles (72 KiB), 3 stages.
 template <int PASS> struct PassCfg;
-template <> struct PassCfg<0> { static constexpr int kOps = 8, kStages = 3; };
-template <> struct PassCfg<1> { static constexpr int kOps = 12, kStages = 2; };
-constexpr int kChunkK = 128;               // promotion interval along K
+template <> struct PassCfg<0> { static constexpr int kOps = 4, kStages = 4; };
+template <> struct PassCfg<1> { static constexpr int kOps = 6, kStages = 3; };
+#ifndef DMPT_CHUNK_K
+#define DMPT_CHUNK_K 128
+#endif
+constexpr int kChunkK = DMPT_CHUNK_K;      // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;
@@ -63,20 +69,21 @@ constexpr int kHalfCols = kTile / 2;       // accumulator columns per epilogue t
 constexpr int kSub = 16;                   // columns per step of the final epilogue
 template <int PASS>
 constexpr int smem_bytes() {
-    return PassCfg<PASS>::kStages * PassCfg<PASS>::kOps * kOpBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+    return PassCfg<PASS>::kStages * PassCfg<PASS>::kOps * (kABytes + kBBytes) + 1024 /* alignment slack */ +
+           256 /* barriers */;
 }
 
-// operand slots inside a stage (A = row panel I, B = row panel J)
-enum Op : int { AMH = 0, AML = 1, A1H = 2, A1L = 3, BMH = 4, BML = 5, B1H = 6, B1L = 7,
-                A2H = 8, A2L = 9, B2H = 10, B2L = 11 };
+// operand matrices, in the order of LayerParams::maps / ::h; a stage holds the A tiles of the first kOps of
+// them (rows of panel I), then the B tiles (rows of panel J)
+enum Op : int { MH = 0, ML = 1, S1H = 2, S1L = 3, S2H = 4, S2L = 5 };
 
 struct LayerParams {
-    CUtensorMap maps[2][6];     // [buffer][Mhi, Mlo, S1hi, S1lo, S2hi, S2lo], box = kBK x kTile, SWIZZLE_64B
+    CUtensorMap maps[2][6];     // [buffer][Mhi, Mlo, S1hi, S1lo, S2hi, S2lo], box = kBK x kBRows, SWIZZLE_64B
     float* s0;                  // fp32 S0, updated in place, ld = n_pad
     float* s1[2];               // fp32 S1, ping-pong
     float* s2[2];               // fp32 S2, ping-pong (order 2)
     __half* h[2][6];            // fp16 operand matrices the epilogue writes, same order as maps
-    const uint32_t* tiles;      // (I | J << 16), I <= J, in launch order
+    const uint32_t* tiles;      // pair tiles (IP | J << 16): block rows 2 IP, 2 IP + 1 x block column J >= 2 IP
     int num_tiles;
     int n_pad;
     int wave_sync;              // 1: producers of all CTAs re-align at every tile boundary (L2 reuse)
@@ -190,6 +197,14 @@ __device__ __forceinline__ void final_epilogue(float (&acc)[kHalfCols], const Ep
 }
 
 
+// One layer launch.  Clusters of two CTAs (one TPC) work on 256 x 128 pair tiles with
+// tcgen05.mma.cta_group::2: CTA r of the pair owns block row 2 IP + r (its 128 rows of every A-side
+// operand and its 128 TMEM lanes of both accumulators) and stages rows r*64 .. r*64+63 of the J panel
+// (its half of UMMA N = 128).  Per MMA each SM reads 4 KiB (A) + 2 KiB (half of B) from shared memory
+// instead of 8 KiB, and TMA brings 48 KiB instead of 64 KiB per k-block (profiles/: the 1-CTA kernel
+// was bound by the shared-memory pipe).  Only the leader CTA (rank 0) issues MMAs; both run TMA and
+// the epilogue.
+//
 // PASS 0: orders 0 and 1 of layer n (P0 = M.M, P1 = M.S1 + S1.M); its last CTA runs Algorithms 2-3.
 // PASS 1: order 2 of layer n (a9, Eq. 25 third line, 201 Eq. 26):
 //             V2 = X2 - S2 = (M.S2 + S2.M) + S1.S1,   S2 <- S2 + sigma V2,
@@ -198,12 +213,13 @@ __device__ __forceinline__ void final_epilogue(float (&acc)[kHalfCols], const Ep
 //         reads the operands of S0_{n-1}, S1_{n-1}, S2_{n-1} and the decision pass 0 of layer n-1 left in
 //         DmptCtl, writes S2_n into the other buffer and leaves ||V2||_F^2, max|S2_n| in partials2.
 template <int PASS>
-__global__ void __launch_bounds__(kNumThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kNumThreads, 1)
 dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     constexpr int kOps = PassCfg<PASS>::kOps;
     constexpr int kStages = PassCfg<PASS>::kStages;
-    constexpr int kStageBytes = kOps * kOpBytes;
-    // ---- the decision for this layer, taken by the previous launch
+    constexpr int kStageBytes = kOps * (kABytes + kBBytes);
+    constexpr int kBOff = kOps * kABytes;          // B tiles follow the A tiles inside a stage
+    // ---- the decision for this layer, taken by the previous launch (both CTAs of a pair read the same)
     const DmptCtl c = *p.ctl;
     if (c.done) return;
     // order 2 after the D1 stop: S0 and S1 are frozen, pass 0 only runs the control step
@@ -221,8 +237,14 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     volatile uint32_t* tmem_slot_ptr =
         reinterpret_cast<volatile uint32_t*>(smem_gen + kStages * kStageBytes + 8 * (2 * kStages + 2 * kAccStages));
 
-    const int warp = threadIdx.x >> 5;
+    // warp index through a shuffle: the compiler then knows it is warp-uniform, and the single-thread
+    // sections below are entered through elect.sync, so TMA / MMA operands stay in uniform registers
+    // (with `lane == 0` every UTCHMMA / UTMALDG was wrapped in an ELECT + R2UR.BROADCAST + BRA.U.ANY loop)
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();        // 0 = leader of the pair
+    const int pair = blockIdx.x >> 1;
+    const int num_pairs = gridDim.x >> 1;
     const int num_chunks = p.n_pad / kChunkK;
     const int num_tiles = idle ? 0 : p.num_tiles;
     const bool with_p0 = PASS == 1 || c.mode0 != MODE_FROZEN;     // first accumulator in use
@@ -235,88 +257,99 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             if (PASS == 1) prefetch_tensormap(&p.maps[c.s2_buf][4 + m]);
         }
         for (int s = 0; s < kStages; ++s) {
-            mbar_init(full_bar(s), 1);
-            mbar_init(empty_bar(s), 1);
+            mbar_init(full_bar(s), 1);                       // leader's: its producer's arrive + both CTAs' bytes
+            mbar_init(empty_bar(s), 1);                      // MMA commit, multicast to both CTAs
         }
         for (int s = 0; s < kAccStages; ++s) {
-            mbar_init(tfull_bar(s), 1);
-            mbar_init(tempty_bar(s), kNumEpiWarps);
+            mbar_init(tfull_bar(s), 1);                      // MMA commit, multicast to both CTAs
+            mbar_init(tempty_bar(s), 2 * kNumEpiWarps);      // leader's: epilogue warps of both CTAs
         }
         fence_mbar_init();
     }
     if (warp == 1) {
-        tmem_alloc<1>(tmem_slot, kTmemCols);
-        tmem_relinquish<1>();
+        tmem_alloc<2>(tmem_slot, kTmemCols);
+        tmem_relinquish<2>();
     }
     tc_fence_before();
-    __syncthreads();
+    cluster_sync_all();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     if (warp == 0) {
-        // =========================== TMA producer ===========================
-        if (lane == 0) {
-            const CUtensorMap* mmh = &p.maps[c.s0_buf][0];
-            const CUtensorMap* mml = &p.maps[c.s0_buf][1];
-            const CUtensorMap* m1h = &p.maps[c.s1_buf][2];
-            const CUtensorMap* m1l = &p.maps[c.s1_buf][3];
-            const CUtensorMap* m2h = &p.maps[c.s2_buf][4];
-            const CUtensorMap* m2l = &p.maps[c.s2_buf][5];
+        // =========================== TMA producer (both CTAs) ===========================
+        {
+            const CUtensorMap* maps[6] = {&p.maps[c.s0_buf][MH],  &p.maps[c.s0_buf][ML],  &p.maps[c.s1_buf][S1H],
+                                          &p.maps[c.s1_buf][S1L], &p.maps[c.s2_buf][S2H], &p.maps[c.s2_buf][S2L]};
             const int num_kb = p.n_pad / kBK;
             int stage = 0;
             uint32_t phase = 0;
             unsigned int wave = 0;
-            const unsigned int num_waves = (num_tiles + gridDim.x - 1) / gridDim.x;
-            for (int t = blockIdx.x; t < num_tiles; t += gridDim.x, ++wave) {
+            const unsigned int num_waves = (num_tiles + num_pairs - 1) / num_pairs;
+            for (int t = pair; t < num_tiles; t += num_pairs, ++wave) {
                 if (p.wave_sync && wave > 0) {
                     // re-align the K phase of all CTAs: tiles in flight then stream the same k-blocks of
                     // few row panels at the same time and share them through L2
-                    __threadfence();
-                    atomicAdd(wave_ctr, 1u);
-                    const unsigned int target = gridDim.x * wave;
-                    unsigned int spins = 0;
-                    while (ld_acquire_u32(wave_ctr) < target) {
-                        __nanosleep(64);
-                        if (++spins > (1u << 26)) __trap();
+                    if (lane == 0) {
+                        __threadfence();
+                        atomicAdd(wave_ctr, 1u);
+                        const unsigned int target = gridDim.x * wave;
+                        unsigned int spins = 0;
+                        while (ld_acquire_u32(wave_ctr) < target) {
+                            __nanosleep(64);
+                            if (++spins > (1u << 26)) __trap();
+                        }
                     }
+                    __syncwarp();
                 }
                 const uint32_t tl = p.tiles[t];
-                const int row_i = (int)(tl & 0xFFFF) * kTile, row_j = (int)(tl >> 16) * kTile;
+                const int row_a = (2 * (int)(tl & 0xFFFF) + (int)rank) * kTile;
+                const int row_b = (int)(tl >> 16) * kTile + (int)rank * kBRows;
                 for (int kb = 0; kb < num_kb; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1);
-                    const uint32_t fb = full_bar(stage);
+                    const uint32_t fb = full_bar(stage);      // completion is counted on the LEADER's barrier
                     const uint32_t base = smem_base + stage * kStageBytes;
-                    mbar_arrive_expect_tx(fb, kStageBytes);
+#ifdef DMPT_DBG_NOLOAD
+                    if (rank == 0 && elect_one()) mbar_arrive(fb);
+                    __syncwarp();
+                    if (++stage == kStages) { stage = 0; phase ^= 1; }
+                    continue;
+#endif
+                    if (elect_one()) {
+#ifdef DMPT_DBG_AONLY
+                    if (rank == 0) mbar_arrive_expect_tx(fb, 2 * kOps * kABytes);
+#else
+                    if (rank == 0) mbar_arrive_expect_tx(fb, 2 * kStageBytes);
+#endif
+#ifdef DMPT_DBG_K0
+                    const int k0 = (kb & 15) * kBK;
+#else
                     const int k0 = kb * kBK;
-                    tma_load_2d(base + AMH * kOpBytes, mmh, fb, k0, row_i);
-                    tma_load_2d(base + BMH * kOpBytes, mmh, fb, k0, row_j);
-                    tma_load_2d(base + AML * kOpBytes, mml, fb, k0, row_i);
-                    tma_load_2d(base + BML * kOpBytes, mml, fb, k0, row_j);
-                    tma_load_2d(base + A1H * kOpBytes, m1h, fb, k0, row_i);
-                    tma_load_2d(base + B1H * kOpBytes, m1h, fb, k0, row_j);
-                    tma_load_2d(base + A1L * kOpBytes, m1l, fb, k0, row_i);
-                    tma_load_2d(base + B1L * kOpBytes, m1l, fb, k0, row_j);
-                    if (PASS == 1) {
-                        tma_load_2d(base + A2H * kOpBytes, m2h, fb, k0, row_i);
-                        tma_load_2d(base + B2H * kOpBytes, m2h, fb, k0, row_j);
-                        tma_load_2d(base + A2L * kOpBytes, m2l, fb, k0, row_i);
-                        tma_load_2d(base + B2L * kOpBytes, m2l, fb, k0, row_j);
+#endif
+#pragma unroll
+                    for (int o = 0; o < kOps; ++o) {
+                        tma_load_2d_2sm(base + o * kABytes, maps[o], fb, k0, row_a);
+                        tma_load_2d_2sm(base + o * kABytes + kBBytes, maps[o], fb, k0, row_a + kBRows);
+#ifndef DMPT_DBG_AONLY
+                        tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[o], fb, k0, row_b);
+#endif
                     }
+                    }
+                    __syncwarp();
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
             }
             // CTAs with fewer tiles still owe their arrivals to the later waves
-            if (p.wave_sync && wave < num_waves && wave > 0) atomicAdd(wave_ctr, num_waves - wave);
+            if (p.wave_sync && wave < num_waves && wave > 0 && lane == 0) atomicAdd(wave_ctr, num_waves - wave);
         }
     } else if (warp == 1) {
-        // =========================== MMA issuer ===========================
-        if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc_f16(kTile, kTile);
+        // =========================== MMA issuer (leader CTA only) ===========================
+        if (rank == 0) {
+            constexpr uint32_t idesc = make_idesc_f16(kPair, kTile);     // M = 256 over the pair, N = 128
             int stage = 0;
             uint32_t phase = 0;
             int acc = 0;
             uint32_t acc_phase = 0;
-            for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+            for (int t = pair; t < num_tiles; t += num_pairs) {
                 for (int ch = 0; ch < num_chunks; ++ch) {
                     mbar_wait(tempty_bar(acc), acc_phase ^ 1);
                     tc_fence_after();
@@ -326,47 +359,54 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                         mbar_wait(full_bar(stage), phase);
                         tc_fence_after();
                         const uint32_t base = smem_base + stage * kStageBytes;
-                        uint64_t d[kOps];
+                        if (elect_one()) {
+                        uint64_t a[kOps], b[kOps];
 #pragma unroll
-                        for (int o = 0; o < kOps; ++o) d[o] = make_smem_desc<kRowBytes>(base + o * kOpBytes);
+                        for (int o = 0; o < kOps; ++o) {
+                            a[o] = make_smem_desc<kRowBytes>(base + o * kABytes);
+                            b[o] = make_smem_desc<kRowBytes>(base + kBOff + o * kBBytes);
+                        }
 #pragma unroll
                         for (int ks = 0; ks < kBK / 16; ++ks) {
                             const uint64_t adv = (uint64_t)(ks * 32 >> 4);     // 16 fp16 = 32 bytes along K
-                            const uint32_t first = (kb | ks) != 0;
+                            const uint32_t accum = (kb | ks) != 0;             // 0: start the chunk from zero
                             if (PASS == 0) {
                                 if (with_p0) {
-                                    umma_f16<1>(d0, d[AMH] + adv, d[BMH] + adv, idesc, first);   // hi.hi
-                                    umma_f16<1>(d0, d[AMH] + adv, d[BML] + adv, idesc, 1);       // hi.lo
-                                    umma_f16<1>(d0, d[AML] + adv, d[BMH] + adv, idesc, 1);       // lo.hi
+                                    umma_f16<2>(d0, a[MH] + adv, b[MH] + adv, idesc, accum);     // hi.hi
+                                    umma_f16<2>(d0, a[MH] + adv, b[ML] + adv, idesc, 1);         // hi.lo
+                                    umma_f16<2>(d0, a[ML] + adv, b[MH] + adv, idesc, 1);         // lo.hi
                                 }
-                                umma_f16<1>(d1, d[AMH] + adv, d[B1H] + adv, idesc, first);       // M.S1
-                                umma_f16<1>(d1, d[A1H] + adv, d[BMH] + adv, idesc, 1);           // S1.M
-                                umma_f16<1>(d1, d[AMH] + adv, d[B1L] + adv, idesc, 1);
-                                umma_f16<1>(d1, d[AML] + adv, d[B1H] + adv, idesc, 1);
-                                umma_f16<1>(d1, d[A1H] + adv, d[BML] + adv, idesc, 1);
-                                umma_f16<1>(d1, d[A1L] + adv, d[BMH] + adv, idesc, 1);
+                                umma_f16<2>(d1, a[MH] + adv, b[S1H] + adv, idesc, accum);        // M.S1
+                                umma_f16<2>(d1, a[S1H] + adv, b[MH] + adv, idesc, 1);            // S1.M
+                                umma_f16<2>(d1, a[MH] + adv, b[S1L] + adv, idesc, 1);
+                                umma_f16<2>(d1, a[ML] + adv, b[S1H] + adv, idesc, 1);
+                                umma_f16<2>(d1, a[S1H] + adv, b[ML] + adv, idesc, 1);
+                                umma_f16<2>(d1, a[S1L] + adv, b[MH] + adv, idesc, 1);
                             } else {
-                                umma_f16<1>(d0, d[A1H] + adv, d[B1H] + adv, idesc, first);       // S1.S1
-                                umma_f16<1>(d0, d[A1H] + adv, d[B1L] + adv, idesc, 1);
-                                umma_f16<1>(d0, d[A1L] + adv, d[B1H] + adv, idesc, 1);
-                                umma_f16<1>(d1, d[AMH] + adv, d[B2H] + adv, idesc, first);       // M.S2
-                                umma_f16<1>(d1, d[A2H] + adv, d[BMH] + adv, idesc, 1);           // S2.M
-                                umma_f16<1>(d1, d[AMH] + adv, d[B2L] + adv, idesc, 1);
-                                umma_f16<1>(d1, d[AML] + adv, d[B2H] + adv, idesc, 1);
-                                umma_f16<1>(d1, d[A2H] + adv, d[BML] + adv, idesc, 1);
-                                umma_f16<1>(d1, d[A2L] + adv, d[BMH] + adv, idesc, 1);
+                                umma_f16<2>(d0, a[S1H] + adv, b[S1H] + adv, idesc, accum);       // S1.S1
+                                umma_f16<2>(d0, a[S1H] + adv, b[S1L] + adv, idesc, 1);
+                                umma_f16<2>(d0, a[S1L] + adv, b[S1H] + adv, idesc, 1);
+                                umma_f16<2>(d1, a[MH] + adv, b[S2H] + adv, idesc, accum);        // M.S2
+                                umma_f16<2>(d1, a[S2H] + adv, b[MH] + adv, idesc, 1);            // S2.M
+                                umma_f16<2>(d1, a[MH] + adv, b[S2L] + adv, idesc, 1);
+                                umma_f16<2>(d1, a[ML] + adv, b[S2H] + adv, idesc, 1);
+                                umma_f16<2>(d1, a[S2H] + adv, b[ML] + adv, idesc, 1);
+                                umma_f16<2>(d1, a[S2L] + adv, b[MH] + adv, idesc, 1);
                             }
                         }
-                        umma_commit(empty_bar(stage));                 // frees the smem stage
+                        umma_commit_2sm(empty_bar(stage), 0b11);       // frees the smem stage in both CTAs
+                        if (kb == kKbPerChunk - 1)
+                            umma_commit_2sm(tfull_bar(acc), 0b11);     // chunk accumulators complete, both CTAs
+                        }
+                        __syncwarp();
                         if (++stage == kStages) { stage = 0; phase ^= 1; }
                     }
-                    umma_commit(tfull_bar(acc));                       // chunk accumulators complete
                     if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
                 }
             }
         }
     } else {
-        // =========================== epilogue ===========================
+        // =========================== epilogue (both CTAs) ===========================
         const int q = warp & 3;                         // TMEM lane quadrant this warp may read
         const int half = (warp - kEpiWarp0) >> 2;       // which 64 accumulator columns
         const int ld = p.n_pad;
@@ -383,24 +423,27 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         EpiOut o0, o1;
         if (PASS == 0) {
             o0.dst = p.s0; o0.old = p.s0;
-            o0.hi = p.h[c.s0_buf ^ 1][0]; o0.lo = p.h[c.s0_buf ^ 1][1];
+            o0.hi = p.h[c.s0_buf ^ 1][MH]; o0.lo = p.h[c.s0_buf ^ 1][ML];
             o1.dst = p.s1[c.s1_buf ^ 1]; o1.old = p.s1[c.s1_buf];
-            o1.hi = p.h[c.s1_buf ^ 1][2]; o1.lo = p.h[c.s1_buf ^ 1][3];
+            o1.hi = p.h[c.s1_buf ^ 1][S1H]; o1.lo = p.h[c.s1_buf ^ 1][S1L];
         } else {
             o0.dst = nullptr; o0.old = nullptr; o0.hi = nullptr; o0.lo = nullptr;
             o1.dst = p.s2[c.s2_buf ^ 1]; o1.old = p.s2[c.s2_buf];
-            o1.hi = p.h[c.s2_buf ^ 1][4]; o1.lo = p.h[c.s2_buf ^ 1][5];
+            o1.hi = p.h[c.s2_buf ^ 1][S2H]; o1.lo = p.h[c.s2_buf ^ 1][S2L];
         }
 
         double r_tr = 0.0, r_fs0 = 0.0, r_f0 = 0.0, r_f1 = 0.0, r_dummy = 0.0;
         float r_mx1 = 0.f, r_mx_dummy = 0.f;
         int acc = 0;
         uint32_t acc_phase = 0;
-        for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+        for (int t = pair; t < num_tiles; t += num_pairs) {
             const uint32_t tl = p.tiles[t];
-            const int ti = (int)(tl & 0xFFFF), tj = (int)(tl >> 16);
+            const int ti = 2 * (int)(tl & 0xFFFF) + (int)rank, tj = (int)(tl >> 16);
             const int gr = ti * kTile + q * 32 + lane;  // global row of this thread's TMEM lane
             const int gc_base = tj * kTile + half * kHalfCols;
+            // the pair tile (IP, J = 2 IP) holds block (2 IP + 1, 2 IP) below the diagonal: its mirror is
+            // computed by the pair tile (IP, 2 IP + 1), so the peer CTA only drains it
+            const bool live = ti <= tj;
             float a0[kHalfCols], a1[kHalfCols];
 #pragma unroll
             for (int j = 0; j < kHalfCols; ++j) { a0[j] = 0.f; a1[j] = 0.f; }
@@ -410,27 +453,37 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 tc_fence_after();
                 const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + acc * 256 + half * kHalfCols;
                 uint32_t v[16];
-                if (with_p0) {
+#ifdef DMPT_DBG_NODRAIN
+                if (false) {
+#else
+                if (live) {
+#endif
+                    if (with_p0) {
+#pragma unroll
+                        for (int g = 0; g < kHalfCols / 16; ++g) {
+                            tmem_ld_32x16(trow + g * 16, v);
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int j = 0; j < 16; ++j) a0[g * 16 + j] += __uint_as_float(v[j]);
+                        }
+                    }
 #pragma unroll
                     for (int g = 0; g < kHalfCols / 16; ++g) {
-                        tmem_ld_32x16(trow + g * 16, v);
+                        tmem_ld_32x16(trow + 128 + g * 16, v);
                         tmem_ld_wait();
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) a0[g * 16 + j] += __uint_as_float(v[j]);
+                        for (int j = 0; j < 16; ++j) a1[g * 16 + j] += __uint_as_float(v[j]);
                     }
-                }
-#pragma unroll
-                for (int g = 0; g < kHalfCols / 16; ++g) {
-                    tmem_ld_32x16(trow + 128 + g * 16, v);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) a1[g * 16 + j] += __uint_as_float(v[j]);
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(tempty_bar(acc));
+                if (lane == 0) mbar_arrive_cluster(tempty_bar(acc), 0);      // on the leader's barrier
                 if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
             }
+#ifdef DMPT_DBG_NOEPI
+            continue;
+#endif
+            if (!live) continue;
             // ---- branch, update, re-split, reductions
             const bool diag = ti == tj;
             if (PASS == 0) {
@@ -466,12 +519,12 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         }
     }
 
-    // ---- teardown
+    // ---- teardown: neither CTA may leave while its peer can still read its smem or signal its barriers
     tc_fence_before();
-    __syncthreads();
+    cluster_sync_all();
     if (warp == 1) {
         tc_fence_after();
-        tmem_dealloc<1>(tmem_base, kTmemCols);
+        tmem_dealloc<2>(tmem_base, kTmemCols);
     }
     if (PASS == 1) return;          // pass 0 of the same layer follows on the stream and takes the decisions
 
