@@ -55,10 +55,7 @@ constexpr int kBBytes = kBRows * kRowBytes;          // 4 KiB per B-side operand
 template <int PASS> struct PassCfg;
 template <> struct PassCfg<0> { static constexpr int kOps = 4, kStages = 4; };
 template <> struct PassCfg<1> { static constexpr int kOps = 6, kStages = 3; };
-#ifndef DMPT_CHUNK_K
-#define DMPT_CHUNK_K 128
-#endif
-constexpr int kChunkK = DMPT_CHUNK_K;      // promotion interval along K
+constexpr int kChunkK = 128;               // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;
@@ -308,31 +305,15 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                     mbar_wait(empty_bar(stage), phase ^ 1);
                     const uint32_t fb = full_bar(stage);      // completion is counted on the LEADER's barrier
                     const uint32_t base = smem_base + stage * kStageBytes;
-#ifdef DMPT_DBG_NOLOAD
-                    if (rank == 0 && elect_one()) mbar_arrive(fb);
-                    __syncwarp();
-                    if (++stage == kStages) { stage = 0; phase ^= 1; }
-                    continue;
-#endif
                     if (elect_one()) {
-#ifdef DMPT_DBG_AONLY
-                    if (rank == 0) mbar_arrive_expect_tx(fb, 2 * kOps * kABytes);
-#else
-                    if (rank == 0) mbar_arrive_expect_tx(fb, 2 * kStageBytes);
-#endif
-#ifdef DMPT_DBG_K0
-                    const int k0 = (kb & 15) * kBK;
-#else
-                    const int k0 = kb * kBK;
-#endif
+                        if (rank == 0) mbar_arrive_expect_tx(fb, 2 * kStageBytes);
+                        const int k0 = kb * kBK;
 #pragma unroll
-                    for (int o = 0; o < kOps; ++o) {
-                        tma_load_2d_2sm(base + o * kABytes, maps[o], fb, k0, row_a);
-                        tma_load_2d_2sm(base + o * kABytes + kBBytes, maps[o], fb, k0, row_a + kBRows);
-#ifndef DMPT_DBG_AONLY
-                        tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[o], fb, k0, row_b);
-#endif
-                    }
+                        for (int o = 0; o < kOps; ++o) {
+                            tma_load_2d_2sm(base + o * kABytes, maps[o], fb, k0, row_a);
+                            tma_load_2d_2sm(base + o * kABytes + kBBytes, maps[o], fb, k0, row_a + kBRows);
+                            tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[o], fb, k0, row_b);
+                        }
                     }
                     __syncwarp();
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -360,43 +341,43 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                         tc_fence_after();
                         const uint32_t base = smem_base + stage * kStageBytes;
                         if (elect_one()) {
-                        uint64_t a[kOps], b[kOps];
+                            uint64_t a[kOps], b[kOps];
 #pragma unroll
-                        for (int o = 0; o < kOps; ++o) {
-                            a[o] = make_smem_desc<kRowBytes>(base + o * kABytes);
-                            b[o] = make_smem_desc<kRowBytes>(base + kBOff + o * kBBytes);
-                        }
-#pragma unroll
-                        for (int ks = 0; ks < kBK / 16; ++ks) {
-                            const uint64_t adv = (uint64_t)(ks * 32 >> 4);     // 16 fp16 = 32 bytes along K
-                            const uint32_t accum = (kb | ks) != 0;             // 0: start the chunk from zero
-                            if (PASS == 0) {
-                                if (with_p0) {
-                                    umma_f16<2>(d0, a[MH] + adv, b[MH] + adv, idesc, accum);     // hi.hi
-                                    umma_f16<2>(d0, a[MH] + adv, b[ML] + adv, idesc, 1);         // hi.lo
-                                    umma_f16<2>(d0, a[ML] + adv, b[MH] + adv, idesc, 1);         // lo.hi
-                                }
-                                umma_f16<2>(d1, a[MH] + adv, b[S1H] + adv, idesc, accum);        // M.S1
-                                umma_f16<2>(d1, a[S1H] + adv, b[MH] + adv, idesc, 1);            // S1.M
-                                umma_f16<2>(d1, a[MH] + adv, b[S1L] + adv, idesc, 1);
-                                umma_f16<2>(d1, a[ML] + adv, b[S1H] + adv, idesc, 1);
-                                umma_f16<2>(d1, a[S1H] + adv, b[ML] + adv, idesc, 1);
-                                umma_f16<2>(d1, a[S1L] + adv, b[MH] + adv, idesc, 1);
-                            } else {
-                                umma_f16<2>(d0, a[S1H] + adv, b[S1H] + adv, idesc, accum);       // S1.S1
-                                umma_f16<2>(d0, a[S1H] + adv, b[S1L] + adv, idesc, 1);
-                                umma_f16<2>(d0, a[S1L] + adv, b[S1H] + adv, idesc, 1);
-                                umma_f16<2>(d1, a[MH] + adv, b[S2H] + adv, idesc, accum);        // M.S2
-                                umma_f16<2>(d1, a[S2H] + adv, b[MH] + adv, idesc, 1);            // S2.M
-                                umma_f16<2>(d1, a[MH] + adv, b[S2L] + adv, idesc, 1);
-                                umma_f16<2>(d1, a[ML] + adv, b[S2H] + adv, idesc, 1);
-                                umma_f16<2>(d1, a[S2H] + adv, b[ML] + adv, idesc, 1);
-                                umma_f16<2>(d1, a[S2L] + adv, b[MH] + adv, idesc, 1);
+                            for (int o = 0; o < kOps; ++o) {
+                                a[o] = make_smem_desc<kRowBytes>(base + o * kABytes);
+                                b[o] = make_smem_desc<kRowBytes>(base + kBOff + o * kBBytes);
                             }
-                        }
-                        umma_commit_2sm(empty_bar(stage), 0b11);       // frees the smem stage in both CTAs
-                        if (kb == kKbPerChunk - 1)
-                            umma_commit_2sm(tfull_bar(acc), 0b11);     // chunk accumulators complete, both CTAs
+#pragma unroll
+                            for (int ks = 0; ks < kBK / 16; ++ks) {
+                                const uint64_t adv = (uint64_t)(ks * 32 >> 4);     // 16 fp16 = 32 bytes along K
+                                const uint32_t accum = (kb | ks) != 0;             // 0: start the chunk from zero
+                                if (PASS == 0) {
+                                    if (with_p0) {
+                                        umma_f16<2>(d0, a[MH] + adv, b[MH] + adv, idesc, accum);     // hi.hi
+                                        umma_f16<2>(d0, a[MH] + adv, b[ML] + adv, idesc, 1);         // hi.lo
+                                        umma_f16<2>(d0, a[ML] + adv, b[MH] + adv, idesc, 1);         // lo.hi
+                                    }
+                                    umma_f16<2>(d1, a[MH] + adv, b[S1H] + adv, idesc, accum);        // M.S1
+                                    umma_f16<2>(d1, a[S1H] + adv, b[MH] + adv, idesc, 1);            // S1.M
+                                    umma_f16<2>(d1, a[MH] + adv, b[S1L] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[ML] + adv, b[S1H] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[S1H] + adv, b[ML] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[S1L] + adv, b[MH] + adv, idesc, 1);
+                                } else {
+                                    umma_f16<2>(d0, a[S1H] + adv, b[S1H] + adv, idesc, accum);       // S1.S1
+                                    umma_f16<2>(d0, a[S1H] + adv, b[S1L] + adv, idesc, 1);
+                                    umma_f16<2>(d0, a[S1L] + adv, b[S1H] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[MH] + adv, b[S2H] + adv, idesc, accum);        // M.S2
+                                    umma_f16<2>(d1, a[S2H] + adv, b[MH] + adv, idesc, 1);            // S2.M
+                                    umma_f16<2>(d1, a[MH] + adv, b[S2L] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[ML] + adv, b[S2H] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[S2H] + adv, b[ML] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[S2L] + adv, b[MH] + adv, idesc, 1);
+                                }
+                            }
+                            umma_commit_2sm(empty_bar(stage), 0b11);       // frees the smem stage in both CTAs
+                            if (kb == kKbPerChunk - 1)
+                                umma_commit_2sm(tfull_bar(acc), 0b11);     // chunk accumulators complete, both CTAs
                         }
                         __syncwarp();
                         if (++stage == kStages) { stage = 0; phase ^= 1; }
@@ -453,11 +434,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 tc_fence_after();
                 const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + acc * 256 + half * kHalfCols;
                 uint32_t v[16];
-#ifdef DMPT_DBG_NODRAIN
-                if (false) {
-#else
                 if (live) {
-#endif
                     if (with_p0) {
 #pragma unroll
                         for (int g = 0; g < kHalfCols / 16; ++g) {
@@ -480,9 +457,6 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 if (lane == 0) mbar_arrive_cluster(tempty_bar(acc), 0);      // on the leader's barrier
                 if (++acc == kAccStages) { acc = 0; acc_phase ^= 1; }
             }
-#ifdef DMPT_DBG_NOEPI
-            continue;
-#endif
             if (!live) continue;
             // ---- branch, update, re-split, reductions
             const bool diag = ti == tj;

@@ -38,12 +38,16 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// arrive on the barrier at the same smem offset in CTA `cta` of the cluster
+// arrive on the barrier at the same smem offset in CTA `cta` of the cluster.  Default (CTA-scope
+// release) semantics, as CUTLASS' ClusterBarrier::arrive: the `.release.cluster` form compiles to
+// MEMBAR.ALL.GPU + ERRBAR in front of every arrive and waits for the epilogue's global stores.  What
+// the arrive has to order here are tcgen05.ld results, and tcgen05.wait::ld + fence::before_thread_sync
+// do that.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t cta) {
     asm volatile(
         "{\n\t.reg .b32 remote;\n\t"
         "mapa.shared::cluster.u32 remote, %0, %1;\n\t"
-        "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [remote];\n\t}"
+        "mbarrier.arrive.shared::cluster.b64 _, [remote];\n\t}"
         ::"r"(bar), "r"(cta) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx_cluster(uint32_t bar, uint32_t bytes, uint32_t cta) {
