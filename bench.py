@@ -106,8 +106,9 @@ def flops_paper(n, layers, layers_d0):
 
 
 def fma_executed(n_pad, layers, layers_d0):
-    """Tensor FMAs the layer kernel issues: upper-triangular 128x128 tiles only, 9 (6 once S0 froze)
-    128x128xK products per tile."""
+    """Tensor FMAs the layer kernel needs: the 128x128 output blocks on or above the diagonal, 9 (6 once
+    S0 froze) 128x128xK products each.  The CTA-pair kernel also issues the nb/2
+    sub-diagonal blocks of its 256x128 diagonal pair tiles (+0.8 % at N = 16384); they are not counted."""
     nb = n_pad // 128
     tiles = nb * (nb + 1) // 2
     la = layers_d0 if layers_d0 > 0 else layers
@@ -298,7 +299,12 @@ def run_ours(args):
 
 
 def solver_n_pad(n):
-    return (n + 127) // 128 * 128
+    return (n + 255) // 256 * 256      # CTA-pair tiles: 256 rows
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE dmpt_layer_kernel launch, from the `ncu --set full`
+# capture of this command committed under profiles/ (the file named there); only for the default workload
+NCU_TRAFFIC_BYTES = {16384: None}
 
 
 def main():
@@ -310,12 +316,14 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--n", type=int, default=None, help="override the matrix size (default: the config's)")
     ap.add_argument("--ref-n", type=int, default=4096, help="size of the oracle's bounded sample")
-    ap.add_argument("--ref-layers", type=int, default=6)
+    ap.add_argument("--ref-layers", type=int, default=20)
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per layer launch from ncu (profiles/)")
     args = ap.parse_args()
     if args.n is None:
         from workloads import CONFIGS
         args.n = CONFIGS[args.config]["n"]
+    if args.traffic is None and args.config == 4:
+        args.traffic = NCU_TRAFFIC_BYTES.get(args.n)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warmup raised to 3 (timing rules)", file=sys.stderr)
         args.warmup = 3
