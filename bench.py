@@ -304,7 +304,7 @@ def solver_n_pad(n):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE dmpt_layer_kernel launch, from the `ncu --set full`
 # capture of this command committed under profiles/ (the file named there); only for the default workload
-NCU_TRAFFIC_BYTES = {16384: None}
+NCU_TRAFFIC_BYTES = {16384: 30.65e9}      # profiles/r01_layer_kernel_v3.md: 26.18 GB read + 4.47 GB written
 
 
 def main():
