@@ -135,8 +135,9 @@ def oracle_sample(config, n_sample, layers):
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    from paper_2203_09621_b200 import replicas
+
+    if replicas.env_ranks()[0] != 0:          # under torchrun rank 0 alone runs and prints the oracle's line
         return 0
     n_s, layers = args.ref_n, args.ref_layers
     for _ in range(args.warmup and 1):          # one untimed pass pages numpy/BLAS in
@@ -179,9 +180,9 @@ def run_ours(args):
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product has no CPU path")
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2203_09621_b200 import replicas
+
+    rank, local, world = replicas.env_ranks()
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
@@ -189,7 +190,7 @@ def run_ours(args):
 
     # Replicas only: every rank solves its own seeded problem of the same
     # configuration; there is no data-path collective.
-    wl = make_config(args.config, n=args.n, device=str(dev), seed=None if rank == 0 else 20220309 + args.config + 1000 * rank)
+    wl = make_config(args.config, n=args.n, device=str(dev), seed=replicas.replica_seed(args.config, rank))
     n = wl.n
     h0_host = torch.from_numpy(wl.h0).pin_memory()
     h1_host = torch.from_numpy(wl.h1).pin_memory()
@@ -208,18 +209,10 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(x, dev)
 
     def sum_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return replicas.sum_over_ranks(x, dev)
 
     for _ in range(args.warmup):
         res = solver.run(out=(d0, d1))
