@@ -99,15 +99,14 @@ __global__ void __launch_bounds__(256) dmpt_transform_kernel(const float* __rest
     const double emax = ctl->eps_max;
     const double inv_w = 1.0 / (ctl->eps_max - ctl->eps_min);
     const int q_per_row = n_pad >> 2;
-    const long long total = (long long)n_pad * q_per_row;
     const bool vec = ((ld & 3) == 0) && ((reinterpret_cast<uintptr_t>(h0) & 15) == 0) &&
                      ((reinterpret_cast<uintptr_t>(h1) & 15) == 0);
     double tr = 0.0, fro = 0.0;
     float mx = 0.f;
-    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < total;
-         q += (long long)gridDim.x * blockDim.x) {
-        const int row = (int)(q / q_per_row);
-        const int col = (int)(q - (long long)row * q_per_row) << 2;
+    // block per row (grid-stride), threads along the row: no 64-bit division per element
+    for (int row = blockIdx.x; row < n_pad; row += gridDim.x)
+    for (int qc = threadIdx.x; qc < q_per_row; qc += blockDim.x) {
+        const int col = qc << 2;
         float a[4] = {0.f, 0.f, 0.f, 0.f}, b[4] = {0.f, 0.f, 0.f, 0.f};
         if (row < n) {
             if (vec && col + 3 < n) {
