@@ -213,6 +213,26 @@ def test_reduced_configs_match_oracle(dev, cfg, n):
     assert ref.layers - 8 <= res.layers <= ref.layers + 2
 
 
+@pytest.mark.parametrize("n,order", [(2, 1), (3, 1), (5, 2), (17, 1), (17, 2), (255, 1), (257, 2)])
+def test_smallest_and_off_by_one_sizes(dev, n, order):
+    """Degenerate sizes: a 2 x 2 problem (one occupied level), sizes far below one tile, and one row either
+    side of the 256-row pair tile (n_pad = 256 vs 512: the padded rows must stay exactly inert)."""
+    from oracle.dnn_sp2_pt import dnn_sp2_pt
+    from workloads import make_config
+
+    wl = make_config(1, n=n)
+    ref = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, order=order)
+    assert ref.status == "ok"
+    if order == 1:
+        res, d0, d1 = _run(wl, dev)
+    else:
+        res, (d0, d1, d2) = _run2(wl, dev)
+        assert np.abs(d2 - ref.d2).max() <= TOL_D2 * np.abs(ref.d2).max()
+    assert res.status == 0
+    _check_against(ref.d0, ref.d1, wl.n_occ, d0, d1)
+    assert ref.layers - 8 <= res.layers <= ref.layers + 2
+
+
 def test_config2_full_size_matches_oracle(dev):
     from oracle.dnn_sp2_pt import dnn_sp2_pt
     from workloads import make_config
@@ -475,6 +495,23 @@ def test_second_order_matches_oracle(dev, cfg, n):
     # cascade (R15): D0 stop, then D1 stop >= 2 layers later, then D2 stop >= 2 layers after that
     assert res.layers_d0 + 2 <= res.layers_d1 and res.layers_d1 + 2 <= res.layers
     assert len(res.fro_err2) == res.layers and np.isfinite(res.fro_err2[res.layers_d1 - 1])
+
+
+def test_second_order_is_deterministic_and_run_host_returns_d2(dev):
+    from workloads import make_config
+
+    wl = make_config(5, n=1284)
+    a = _run2(wl, dev)
+    b = _run2(wl, dev, wave_sync=False)
+    assert a[0].layers == b[0].layers
+    for x, y in zip(a[1], b[1]):
+        assert np.array_equal(x, y)
+    s = _solver(wl.n, dev, order=2)
+    r = s.run_host(torch.from_numpy(wl.h0).pin_memory(), torch.from_numpy(wl.h1).pin_memory(), wl.n_occ)
+    assert r.status == 0 and r.layers == a[0].layers
+    for x, y in zip((r.d0, r.d1, r.d2), a[1]):
+        assert np.array_equal(x.double().numpy(), y)
+    s.close()
 
 
 def test_second_order_special_cases(dev):
