@@ -98,23 +98,30 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def flops_paper(n, layers, layers_d0):
-    """Eq. 82 with the layers after S0 froze counted as 3 N^3 (SURVEY.md 8(d) accounting rules)."""
+def _layer_split(layers, layers_d0, layers_d1, order):
+    """(layers with S0 active, layers with S0 frozen and S1 active, layers with only S2 active)."""
     la = layers_d0 if layers_d0 > 0 else layers
-    lf = layers - la
-    return (5.0 * la + 3.0 * lf) * float(n) ** 3
+    l1 = (layers_d1 if (order == 2 and layers_d1 > 0) else layers) - la
+    return la, l1, layers - la - l1
 
 
-def fma_executed(n_pad, layers, layers_d0):
+def flops_paper(n, layers, layers_d0, order=1, layers_d1=0):
+    """Eq. 82 with the layers after S0 froze counted as 3 N^3 (SURVEY.md 8(d) accounting rules); order 2 adds
+    3 N^3 (S0.S2) + 2 N^3 (S1.S1) per layer, and after the D1 stop only those remain."""
+    la, l1, l2 = _layer_split(layers, layers_d0, layers_d1, order)
+    per = (5.0 * la + 3.0 * l1) + (5.0 * layers if order == 2 else 0.0)
+    return per * float(n) ** 3
+
+
+def fma_executed(n_pad, layers, layers_d0, order=1, layers_d1=0):
     """Tensor FMAs the layer kernel needs: the 128x128 output blocks on or above the diagonal, 9 (6 once
     S0 froze) 128x128xK products each.  The CTA-pair kernel also issues the nb/2
     sub-diagonal blocks of its 256x128 diagonal pair tiles (+0.8 % at N = 16384); they are not counted."""
     nb = n_pad // 128
     tiles = nb * (nb + 1) // 2
-    la = layers_d0 if layers_d0 > 0 else layers
-    lf = layers - la
+    la, l1, l2 = _layer_split(layers, layers_d0, layers_d1, order)
     per_mma = 128.0 * 128.0 * n_pad
-    return tiles * per_mma * (9.0 * la + 6.0 * lf)
+    return tiles * per_mma * (9.0 * la + 6.0 * l1 + (9.0 * layers if order == 2 else 0.0))
 
 
 # ---------------------------------------------------------------------------------------------
@@ -164,7 +171,9 @@ def run_reference(args):
 
 
 def workload_name(args):
-    return (f"BASELINE.json configs[{args.config - 1}] (config {args.config}): N={args.n}, first-order response, "
+    from workloads import CONFIGS
+    order = {1: "first", 2: "second"}[CONFIGS[args.config]["order"]]
+    return (f"BASELINE.json configs[{args.config - 1}] (config {args.config}): N={args.n}, {order}-order response, "
             "seeded synthetic gapped Hamiltonian")
 
 
@@ -196,12 +205,16 @@ def run_ours(args):
     h1_host = torch.from_numpy(wl.h1).pin_memory()
     h0 = h0_host.to(dev)
     h1 = h1_host.to(dev)
-    solver = Dmpt(n, device=dev)
+    order = wl.order
+    solver = Dmpt(n, order=order, device=dev)
     solver.set_hamiltonian(h0, h1, wl.n_occ)
     d0 = torch.empty((n, n), dtype=torch.float32, device=dev)
     d1 = torch.empty((n, n), dtype=torch.float32, device=dev)
     d0_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
     d1_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
+    n_out = 2 + (order == 2)
+    outs = (d0, d1) + ((torch.empty((n, n), dtype=torch.float32, device=dev),) if order == 2 else ())
+    outs_host = (d0_host, d1_host) + ((torch.empty((n, n), dtype=torch.float32).pin_memory(),) if order == 2 else ())
 
     def barrier():
         if world > 1:
@@ -215,7 +228,7 @@ def run_ours(args):
         return replicas.sum_over_ranks(x, dev)
 
     for _ in range(args.warmup):
-        res = solver.run(out=(d0, d1))
+        res = solver.run(out=outs)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -226,9 +239,9 @@ def run_ours(args):
     flops = fma = ms_loop = 0.0
     launches = layers_total = 0
     for _ in range(args.steps):
-        res = solver.run(out=(d0, d1))
-        flops += flops_paper(n, res.layers, res.layers_d0)
-        fma += fma_executed(solver_n_pad(n), res.layers, res.layers_d0)
+        res = solver.run(out=outs)
+        flops += flops_paper(n, res.layers, res.layers_d0, order, res.layers_d1)
+        fma += fma_executed(solver_n_pad(n), res.layers, res.layers_d0, order, res.layers_d1)
         ms_loop += res.ms_loop
         launches += res.launches
         layers_total += res.layers
@@ -241,13 +254,13 @@ def run_ours(args):
 
     # ---- end-to-end arm: host buffers through dmpt_run_host, copies inside the timed region
     for _ in range(1):
-        solver.run_host(h0_host, h1_host, wl.n_occ, out=(d0_host, d1_host))
+        solver.run_host(h0_host, h1_host, wl.n_occ, out=outs_host)
     barrier()
     ev0.record()
     e2e_flops = 0.0
     for _ in range(args.steps):
-        r2 = solver.run_host(h0_host, h1_host, wl.n_occ, out=(d0_host, d1_host))
-        e2e_flops += flops_paper(n, r2.layers, r2.layers_d0)
+        r2 = solver.run_host(h0_host, h1_host, wl.n_occ, out=outs_host)
+        e2e_flops += flops_paper(n, r2.layers, r2.layers_d0, order, r2.layers_d1)
     ev1.record()
     barrier()
     ms_e2e = max_over_ranks(ev0.elapsed_time(ev1))
@@ -264,17 +277,17 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f16 x f16 -> f32 (dual-half), f64 scalars",
             "data": "synthetic", "gpu_launches": launches,
-            "config": {"workload": workload_name(args), "n": n, "n_occ": wl.n_occ, "order": 1,
+            "config": {"workload": workload_name(args), "n": n, "n_occ": wl.n_occ, "order": order,
                        "layers": res.layers, "layers_d0": res.layers_d0, "gap": wl.meta.get("gap"),
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2": "inputs larger than L2 (1 GiB per matrix at N=16384); no flush needed",
+                       "l2": f"inputs larger than L2 ({n * n * 4 / 2**30:.2f} GiB per matrix); no flush needed",
                        "time_to_d1_ms": ms / args.steps, "loop_ms": ms_loop / args.steps,
                        "tflops_fma1_loop_only": flops / (ms_loop * 1e-3) / 1e12,
                        "frac_nominal_fp16_peak_fma1": value / NOMINAL_FP16_TFMA,
                        "paper_context": "~120 Tflops (FMA=1) on one A100, N=19008 (PAPER.md:546); another machine"},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
-                    "h2d_bytes_per_step": 2 * n * n * 4, "d2h_bytes_per_step": 2 * n * n * 4},
+                    "h2d_bytes_per_step": 2 * n * n * 4, "d2h_bytes_per_step": n_out * n * n * 4},
             "roofline": {"bound": "tensor", "kernel": "dmpt_layer_kernel", "achieved": achieved_tf, "peak": peak_tf,
                          "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": args.traffic,
                          "peak_kind": f"bf16_tflops_sustained, {peaks_kind} (fp16 = bf16 rate), 2 flops per FMA",

@@ -282,7 +282,12 @@ class Dmpt:
             d1 = t.empty((n, n), dtype=t.float32, device=self.device)
         else:
             d0, d1 = out[0], out[1]
-        d2 = t.empty((n, n), dtype=t.float32, device=self.device) if self.order == 2 else None
+        if self.order != 2:
+            d2 = None
+        elif out is not None and len(out) > 2:
+            d2 = out[2]
+        else:
+            d2 = t.empty((n, n), dtype=t.float32, device=self.device)
         r, bufs = self._new_result()
         rc = dmpt_run(self.ctx, d0.data_ptr(), d1.data_ptr(), d2.data_ptr() if d2 is not None else 0,
                       d0.stride(0), r)
@@ -297,7 +302,12 @@ class Dmpt:
             d1 = t.empty((n, n), dtype=t.float32, pin_memory=True)
         else:
             d0, d1 = out[0], out[1]
-        d2 = t.empty((n, n), dtype=t.float32, pin_memory=True) if self.order == 2 else None
+        if self.order != 2:
+            d2 = None
+        elif out is not None and len(out) > 2:
+            d2 = out[2]
+        else:
+            d2 = t.empty((n, n), dtype=t.float32, pin_memory=True)
         r, bufs = self._new_result()
         rc = dmpt_run_host(self.ctx, h0.data_ptr(), h1.data_ptr(), h0.stride(0), n_occ, d0.data_ptr(),
                            d1.data_ptr(), d2.data_ptr() if d2 is not None else 0, d0.stride(0), r)
