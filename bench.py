@@ -135,9 +135,9 @@ def oracle_sample(config, n_sample, layers):
 
     wl = make_config(config, n=n_sample)
     t0 = time.perf_counter()
-    res = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, max_layers=layers)
+    res = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, order=wl.order, max_layers=layers)
     dt = time.perf_counter() - t0
-    fl = flops_paper(n_sample, res.layers, res.layers_d0)
+    fl = flops_paper(n_sample, res.layers, res.layers_d0, wl.order, res.layers_d1)
     return fl / dt / 1e12, dt, len(os.sched_getaffinity(0))
 
 
