@@ -37,7 +37,7 @@ extern "C" {
 #endif
 
 #define DMPT_OK            0
-#define DMPT_EINVAL       -1   /* null pointer, n <= 0, n_occ outside (0, n), ld < n, order not 1|2   */
+#define DMPT_EINVAL       -1   /* null pointer, n <= 0, n_occ outside (0, n), ld < n, order not 0|1|2 */
 #define DMPT_ESTATE       -2   /* dmpt_run before dmpt_set_hamiltonian                                */
 #define DMPT_ECUDA        -3   /* CUDA error (text via dmpt_strerror / dmpt_last_cuda_error)          */
 #define DMPT_EDEGENERATE  -4   /* eps_max - eps_min not positive and finite                           */
@@ -49,7 +49,9 @@ typedef struct dmpt_ctx dmpt_ctx;
 
 typedef struct dmpt_options {
     int max_layers;    /* cap on the while loop of Algorithm 1 (the paper has none); default 200       */
-    int order;         /* 1: D0, D1.  2: also D2 (Eq. 25 third line)                    */
+    int order;         /* 1: D0, D1.  2: also D2 (Eq. 25 third line).  0: D0 only - the       */
+                       /* ground-state DNN-SP2 recursion with Algorithm 2 as its stop (PAPER.md:176-186,   */
+                       /* 515-519); pass NULL for every H1 / D1 argument                                  */
     int s0_shift;      /* a >= 0: S0 is split as hi = fp16(2^a S0), lo = fp16(2^a S0 - hi) and 2^-2a   */
                        /* is folded back in fp32 (exact).  0 = Eq. 13 verbatim.  -1 = default (14).    */
     int s1_autoscale;  /* 1 (default): the response iterates are split after an exact power-of-two     */
@@ -64,14 +66,15 @@ typedef struct dmpt_options {
 
 typedef struct dmpt_result {
     int status;        /* same as the return code of dmpt_run                                         */
-    int layers;        /* passes of the while loop of Algorithm 1                  */
+    int layers;        /* passes of the while loop of Algorithm 1; at order 0 the pass   */
+                       /* on which Algorithm 2 fired is counted but its product is not formed            */
     int layers_d0;     /* layer at which the D0 test fired (Algorithm 2); 0 if it never did           */
     int layers_d1;     /* layer at which the D1 test fired (Algorithm 3); 0 if it never did           */
     int launches;      /* kernels this run launched (all of them this library's own)                  */
     int layers_d2;     /* order 2: layer at which the D2 test fired (R15); 0 otherwise            */
     int reserved_i[2];
     double eps_min, eps_max;   /* spectral bounds used                                 */
-    double fro_err0;           /* FroErr0 = ||S0 - S0^2||_F at the D0 stop layer        */
+    double fro_err0;           /* FroErr0 = ||S0 - S0^2||_F at the D0 stop layer; NaN at order 0 */
     double ms_total;           /* CUDA-event time of the whole run (bounds + transform + split + loop) */
     double ms_loop;            /* CUDA-event time of the layer loop alone ("time for main loop", Eq. 82)*/
     double ms_bounds;          /* a1: Gershgorin kernel (+ scalar set-up)                                */

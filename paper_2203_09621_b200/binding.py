@@ -245,10 +245,12 @@ class Dmpt:
     def set_hamiltonian(self, h0, h1, n_occ):
         t = self.torch
         for m in (h0, h1):
-            if not (m.is_cuda and m.dtype == t.float32 and m.dim() == 2 and m.stride(1) == 1):
+            if m is None and self.order == 0:
+                continue                # ground-state mode takes no perturbation
+            if m is None or not (m.is_cuda and m.dtype == t.float32 and m.dim() == 2 and m.stride(1) == 1):
                 raise DmptError(DMPT_EINVAL, "set_hamiltonian", "need row-major fp32 CUDA matrices")
         self._h = (h0, h1)          # keep the storage alive
-        dmpt_set_hamiltonian(self.ctx, h0.data_ptr(), h1.data_ptr(), h0.stride(0), n_occ)
+        dmpt_set_hamiltonian(self.ctx, h0.data_ptr(), h1.data_ptr() if h1 is not None else 0, h0.stride(0), n_occ)
 
     def _new_result(self):
         ml = self.max_layers
@@ -279,9 +281,9 @@ class Dmpt:
         n = self.n
         if out is None:
             d0 = t.empty((n, n), dtype=t.float32, device=self.device)
-            d1 = t.empty((n, n), dtype=t.float32, device=self.device)
+            d1 = t.empty((n, n), dtype=t.float32, device=self.device) if self.order >= 1 else None
         else:
-            d0, d1 = out[0], out[1]
+            d0, d1 = out[0], (out[1] if len(out) > 1 else None)
         if self.order != 2:
             d2 = None
         elif out is not None and len(out) > 2:
@@ -289,8 +291,8 @@ class Dmpt:
         else:
             d2 = t.empty((n, n), dtype=t.float32, device=self.device)
         r, bufs = self._new_result()
-        rc = dmpt_run(self.ctx, d0.data_ptr(), d1.data_ptr(), d2.data_ptr() if d2 is not None else 0,
-                      d0.stride(0), r)
+        rc = dmpt_run(self.ctx, d0.data_ptr(), d1.data_ptr() if d1 is not None else 0,
+                      d2.data_ptr() if d2 is not None else 0, d0.stride(0), r)
         return self._wrap(rc, r, bufs, d0, d1, d2, check)
 
     def run_host(self, h0, h1, n_occ, out=None, check=True) -> DmptResult:
@@ -299,9 +301,9 @@ class Dmpt:
         n = self.n
         if out is None:
             d0 = t.empty((n, n), dtype=t.float32, pin_memory=True)
-            d1 = t.empty((n, n), dtype=t.float32, pin_memory=True)
+            d1 = t.empty((n, n), dtype=t.float32, pin_memory=True) if self.order >= 1 else None
         else:
-            d0, d1 = out[0], out[1]
+            d0, d1 = out[0], (out[1] if len(out) > 1 else None)
         if self.order != 2:
             d2 = None
         elif out is not None and len(out) > 2:
@@ -309,8 +311,9 @@ class Dmpt:
         else:
             d2 = t.empty((n, n), dtype=t.float32, pin_memory=True)
         r, bufs = self._new_result()
-        rc = dmpt_run_host(self.ctx, h0.data_ptr(), h1.data_ptr(), h0.stride(0), n_occ, d0.data_ptr(),
-                           d1.data_ptr(), d2.data_ptr() if d2 is not None else 0, d0.stride(0), r)
+        rc = dmpt_run_host(self.ctx, h0.data_ptr(), h1.data_ptr() if h1 is not None else 0, h0.stride(0), n_occ,
+                           d0.data_ptr(), d1.data_ptr() if d1 is not None else 0,
+                           d2.data_ptr() if d2 is not None else 0, d0.stride(0), r)
         return self._wrap(rc, r, bufs, d0, d1, d2, check)
 
     def layer_products(self, s0, s1):

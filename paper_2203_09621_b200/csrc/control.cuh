@@ -112,6 +112,11 @@ __device__ inline void control_decide(DmptCtl& c, const DmptLogs& L, const DmptP
             c.conv0 = 1;
             c.n_c = n;
             c.mode0 = MODE_STOP;      // X0 is still formed once, for FroErr0 (R4)
+            if (pb.order == 0) {      // ground-state mode: D0 = S0_{n-1} is the answer, nothing left to measure
+                c.layers = n;         // counted like the oracle's loop: the pass on which the test fired
+                c.fro0 = nan("");
+                c.done = 1;
+            }
         } else {
             c.mode0 = MODE_ACTIVE;
         }
@@ -144,7 +149,7 @@ __device__ inline void control_finalize(DmptCtl& c, const DmptLogs& L, const Dmp
     }
     const double nanv = nan("");
     // ---- first order
-    if (!c.conv1) {
+    if (pb.order >= 1 && !c.conv1) {
         if (c.conv0) {
             const double f1 = sqrt(red[RED_FRO1]);
             L.fro1[n - 1] = f1;
@@ -191,7 +196,7 @@ __device__ inline void control_finalize(DmptCtl& c, const DmptLogs& L, const Dmp
         c.done = 1;
         return;
     }
-    if (pb.order == 2 ? c.conv2 : c.conv1) {
+    if (pb.order == 2 ? c.conv2 : (pb.order == 1 && c.conv1)) {
         c.done = 1;
         return;
     }

@@ -153,7 +153,7 @@ extern "C" void dmpt_default_options(dmpt_options* opt) {
 }
 
 extern "C" size_t dmpt_workspace_bytes(int n, int order) {
-    if (n <= 0 || (order != 1 && order != 2) || n > 65535 * kTile) return 0;
+    if (n <= 0 || order < 0 || order > 2 || n > 65535 * kTile) return 0;
     return make_layout(n, order).total;
 }
 
@@ -208,7 +208,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     *out = nullptr;
     dmpt_options o;
     if (opt) o = *opt; else dmpt_default_options(&o);
-    if (n <= 0 || (o.order != 1 && o.order != 2) || !d_workspace) return DMPT_EINVAL;
+    if (n <= 0 || o.order < 0 || o.order > 2 || !d_workspace) return DMPT_EINVAL;
     if (o.max_layers <= 0) o.max_layers = 200;
     if (o.max_layers > kMaxLayersCap) o.max_layers = kMaxLayersCap;
     if (o.s0_shift > 15) return DMPT_EINVAL;
@@ -329,7 +329,7 @@ extern "C" int dmpt_destroy(dmpt_ctx* ctx) {
 }
 
 extern "C" int dmpt_set_hamiltonian(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld, int n_occ) {
-    if (!ctx || !d_h0 || !d_h1) return DMPT_EINVAL;
+    if (!ctx || !d_h0 || (!d_h1 && ctx->opt.order != 0)) return DMPT_EINVAL;     // order 0 takes no perturbation
     if (ld < ctx->n || n_occ <= 0 || n_occ >= ctx->n) return DMPT_EINVAL;
     ctx->d_h0 = d_h0;
     ctx->d_h1 = d_h1;
@@ -407,9 +407,12 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     const int sgrid = elementwise_grid(ctx, c8, 256);
     dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
     CK(cudaGetLastError());
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
-    CK(cudaGetLastError());
-    *launches += 6;
+    if (ctx->opt.order >= 1) {      // order 0 (ground state only) has no response operands
+        dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
+        CK(cudaGetLastError());
+        ++*launches;
+    }
+    *launches += 5;
     if (ctx->opt.order == 2) {      // S2_0 = 0 (H2 = 0): fp32 iterate and its operands
         const size_t np2 = (size_t)np * np;
         CK(cudaMemsetAsync(ctx->lp.s2[0], 0, np2 * 4, st));
@@ -507,7 +510,7 @@ static int fetch_ctl(dmpt_ctx* ctx) {
 }
 
 extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, int ld, dmpt_result* res) {
-    if (!ctx || !d_d0 || !d_d1) return DMPT_EINVAL;
+    if (!ctx || !d_d0 || (!d_d1 && ctx->opt.order != 0)) return DMPT_EINVAL;
     if (!ctx->d_h0) return DMPT_ESTATE;
     if (ld < ctx->n || (ctx->opt.order == 2 && !d_d2)) return DMPT_EINVAL;
     const Layout& L = ctx->L;
@@ -518,8 +521,9 @@ extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, in
     if (rc) return rc;
     if ((rc = fetch_ctl(ctx))) return rc;
     CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
-    CK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
-                         cudaMemcpyDeviceToDevice, ctx->stream));
+    if (ctx->opt.order >= 1)
+        CK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
+                             cudaMemcpyDeviceToDevice, ctx->stream));
     if (ctx->opt.order == 2)
         CK(cudaMemcpy2DAsync(d_d2, (size_t)ld * 4, ctx->lp.s2[ctx->h_ctl->s2_buf & 1], np * 4, n * 4, n,
                              cudaMemcpyDeviceToDevice, ctx->stream));
@@ -528,7 +532,8 @@ extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, in
 
 extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1, int ld_in, int n_occ,
                              float* h_d0, float* h_d1, float* h_d2, int ld_out, dmpt_result* res) {
-    if (!ctx || !h_h0 || !h_h1 || !h_d0 || !h_d1) return DMPT_EINVAL;
+    if (!ctx || !h_h0 || !h_d0) return DMPT_EINVAL;
+    if (ctx->opt.order != 0 && (!h_h1 || !h_d1)) return DMPT_EINVAL;
     if (ld_in < ctx->n || ld_out < ctx->n || n_occ <= 0 || n_occ >= ctx->n) return DMPT_EINVAL;
     if (ctx->opt.order == 2 && !h_d2) return DMPT_EINVAL;
     const Layout& L = ctx->L;
@@ -540,13 +545,15 @@ extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1
     int launches = 0;
     CK(cudaEventRecord(ctx->ev_t[0], ctx->stream));
     CK(cudaMemcpy2DAsync(s_h0, n * 4, h_h0, (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, ctx->stream));
-    CK(cudaMemcpy2DAsync(s_h1, n * 4, h_h1, (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, ctx->stream));
-    int rc = run_core(ctx, s_h0, s_h1, (int)n, &launches);
+    if (ctx->opt.order >= 1)
+        CK(cudaMemcpy2DAsync(s_h1, n * 4, h_h1, (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, ctx->stream));
+    int rc = run_core(ctx, s_h0, ctx->opt.order >= 1 ? s_h1 : nullptr, (int)n, &launches);
     if (rc) return rc;
     if ((rc = fetch_ctl(ctx))) return rc;
     CK(cudaMemcpy2DAsync(h_d0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToHost, ctx->stream));
-    CK(cudaMemcpy2DAsync(h_d1, (size_t)ld_out * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
-                         cudaMemcpyDeviceToHost, ctx->stream));
+    if (ctx->opt.order >= 1)
+        CK(cudaMemcpy2DAsync(h_d1, (size_t)ld_out * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
+                             cudaMemcpyDeviceToHost, ctx->stream));
     if (ctx->opt.order == 2)
         CK(cudaMemcpy2DAsync(h_d2, (size_t)ld_out * 4, ctx->lp.s2[ctx->h_ctl->s2_buf & 1], np * 4, n * 4, n,
                              cudaMemcpyDeviceToHost, ctx->stream));

@@ -99,6 +99,7 @@ __global__ void __launch_bounds__(256) dmpt_transform_kernel(const float* __rest
     const double emax = ctl->eps_max;
     const double inv_w = 1.0 / (ctl->eps_max - ctl->eps_min);
     const int q_per_row = n_pad >> 2;
+    const bool with_h1 = h1 != nullptr;        // order 0 (ground state only): S1 = 0
     const bool vec = ((ld & 3) == 0) && ((reinterpret_cast<uintptr_t>(h0) & 15) == 0) &&
                      ((reinterpret_cast<uintptr_t>(h1) & 15) == 0);
     double tr = 0.0, fro = 0.0;
@@ -111,7 +112,7 @@ __global__ void __launch_bounds__(256) dmpt_transform_kernel(const float* __rest
         if (row < n) {
             if (vec && col + 3 < n) {
                 float4 va = ldg_stream4(h0 + (size_t)row * ld + col);
-                float4 vb = ldg_stream4(h1 + (size_t)row * ld + col);
+                float4 vb = with_h1 ? ldg_stream4(h1 + (size_t)row * ld + col) : make_float4(0.f, 0.f, 0.f, 0.f);
                 a[0] = va.x; a[1] = va.y; a[2] = va.z; a[3] = va.w;
                 b[0] = vb.x; b[1] = vb.y; b[2] = vb.z; b[3] = vb.w;
             } else {
@@ -119,7 +120,7 @@ __global__ void __launch_bounds__(256) dmpt_transform_kernel(const float* __rest
                 for (int t = 0; t < 4; ++t)
                     if (col + t < n) {
                         a[t] = h0[(size_t)row * ld + col + t];
-                        b[t] = h1[(size_t)row * ld + col + t];
+                        b[t] = with_h1 ? h1[(size_t)row * ld + col + t] : 0.f;
                     }
             }
         }

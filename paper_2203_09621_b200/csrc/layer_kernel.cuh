@@ -245,6 +245,8 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     const int num_chunks = p.n_pad / kChunkK;
     const int num_tiles = idle ? 0 : p.num_tiles;
     const bool with_p0 = PASS == 1 || c.mode0 != MODE_FROZEN;     // first accumulator in use
+    const bool with_p1 = PASS == 1 || p.pb.order >= 1;            // order 0 (ground state only): no response product
+    const int nops = with_p1 ? kOps : 2;                          // order 0 stages Mhi, Mlo only
     unsigned int* wave_ctr = PASS == 0 ? &p.ctl->wave : &p.ctl->wave2;
 
     if (warp == 0 && lane == 0) {
@@ -306,13 +308,15 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                     const uint32_t fb = full_bar(stage);      // completion is counted on the LEADER's barrier
                     const uint32_t base = smem_base + stage * kStageBytes;
                     if (elect_one()) {
-                        if (rank == 0) mbar_arrive_expect_tx(fb, 2 * kStageBytes);
+                        if (rank == 0) mbar_arrive_expect_tx(fb, 2 * nops * (kABytes + kBBytes));
                         const int k0 = kb * kBK;
 #pragma unroll
                         for (int o = 0; o < kOps; ++o) {
-                            tma_load_2d_2sm(base + o * kABytes, maps[o], fb, k0, row_a);
-                            tma_load_2d_2sm(base + o * kABytes + kBBytes, maps[o], fb, k0, row_a + kBRows);
-                            tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[o], fb, k0, row_b);
+                            if (o < nops) {
+                                tma_load_2d_2sm(base + o * kABytes, maps[o], fb, k0, row_a);
+                                tma_load_2d_2sm(base + o * kABytes + kBBytes, maps[o], fb, k0, row_a + kBRows);
+                                tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[o], fb, k0, row_b);
+                            }
                         }
                     }
                     __syncwarp();
@@ -357,12 +361,14 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                                         umma_f16<2>(d0, a[MH] + adv, b[ML] + adv, idesc, 1);         // hi.lo
                                         umma_f16<2>(d0, a[ML] + adv, b[MH] + adv, idesc, 1);         // lo.hi
                                     }
-                                    umma_f16<2>(d1, a[MH] + adv, b[S1H] + adv, idesc, accum);        // M.S1
-                                    umma_f16<2>(d1, a[S1H] + adv, b[MH] + adv, idesc, 1);            // S1.M
-                                    umma_f16<2>(d1, a[MH] + adv, b[S1L] + adv, idesc, 1);
-                                    umma_f16<2>(d1, a[ML] + adv, b[S1H] + adv, idesc, 1);
-                                    umma_f16<2>(d1, a[S1H] + adv, b[ML] + adv, idesc, 1);
-                                    umma_f16<2>(d1, a[S1L] + adv, b[MH] + adv, idesc, 1);
+                                    if (with_p1) {
+                                        umma_f16<2>(d1, a[MH] + adv, b[S1H] + adv, idesc, accum);    // M.S1
+                                        umma_f16<2>(d1, a[S1H] + adv, b[MH] + adv, idesc, 1);        // S1.M
+                                        umma_f16<2>(d1, a[MH] + adv, b[S1L] + adv, idesc, 1);
+                                        umma_f16<2>(d1, a[ML] + adv, b[S1H] + adv, idesc, 1);
+                                        umma_f16<2>(d1, a[S1H] + adv, b[ML] + adv, idesc, 1);
+                                        umma_f16<2>(d1, a[S1L] + adv, b[MH] + adv, idesc, 1);
+                                    }
                                 } else {
                                     umma_f16<2>(d0, a[S1H] + adv, b[S1H] + adv, idesc, accum);       // S1.S1
                                     umma_f16<2>(d0, a[S1H] + adv, b[S1L] + adv, idesc, 1);
@@ -444,12 +450,14 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                             for (int j = 0; j < 16; ++j) a0[g * 16 + j] += __uint_as_float(v[j]);
                         }
                     }
+                    if (with_p1) {
 #pragma unroll
-                    for (int g = 0; g < kHalfCols / 16; ++g) {
-                        tmem_ld_32x16(trow + 128 + g * 16, v);
-                        tmem_ld_wait();
+                        for (int g = 0; g < kHalfCols / 16; ++g) {
+                            tmem_ld_32x16(trow + 128 + g * 16, v);
+                            tmem_ld_wait();
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) a1[g * 16 + j] += __uint_as_float(v[j]);
+                            for (int j = 0; j < 16; ++j) a1[g * 16 + j] += __uint_as_float(v[j]);
+                        }
                     }
                 }
                 tc_fence_before();
@@ -464,8 +472,9 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 if (with_p0)
                     final_epilogue<0>(a0, o0, ld, gr, gc_base, diag, upd0, sig, unscale0, scale0, !upd0, r_tr, r_fs0,
                                       r_f0, r_mx_dummy);
-                final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale1, scale1, conv0, r_dummy,
-                                  r_dummy, r_f1, r_mx1);
+                if (with_p1)
+                    final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale1, scale1, conv0, r_dummy,
+                                      r_dummy, r_f1, r_mx1);
             } else {
                 // V2 = 2^-(a+e2) P2 + 2^-(2 e1) Q: both factors are powers of two, one fp32 rounding per element
 #pragma unroll

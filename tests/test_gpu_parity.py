@@ -605,3 +605,48 @@ def test_config5_second_order_full_size(dev, n):
           f"max|D0 err| {e0:.2e} D1 {e1:.2e} D2 {e2:.2e} loop {res.ms_loop:.0f} ms")
     assert e0 <= TOL_D0 and e1 <= TOL_D1 and e2 <= TOL_D2, (e0, e1, e2)
     assert res.layers_d0 + 2 <= res.layers_d1 and res.layers_d1 + 2 <= res.layers <= res.layers_d1 + 6
+
+
+# ------------------------------------------------------------------------------------------
+# order 0: the ground-state DNN-SP2 recursion on its own
+# ------------------------------------------------------------------------------------------
+def _run0(h0, n_occ, dev, **kw):
+    s = _solver(h0.shape[0], dev, order=0, **kw)
+    s.set_hamiltonian(torch.from_numpy(h0).to(dev), None, n_occ)
+    res = s.run()
+    d0 = res.d0.double().cpu().numpy()
+    s.close()
+    return res, d0
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 256), (2, 512), (4, 1024), (3, 332), (1, 3)])
+def test_ground_state_mode_matches_oracle(dev, cfg, n):
+    from oracle.dnn_sp2_pt import dnn_sp2
+    from workloads import make_config
+
+    wl = make_config(cfg, n=n)
+    ref0, ref_layers = dnn_sp2(wl.h0, wl.n_occ)
+    res, d0 = _run0(wl.h0, wl.n_occ, dev)
+    assert res.status == 0 and res.d1 is None
+    assert np.abs(d0 - ref0).max() <= TOL_D0 and abs(np.trace(d0) - wl.n_occ) <= TOL_TR
+    assert np.array_equal(d0, d0.T)
+    assert ref_layers - 8 <= res.layers <= ref_layers + 2 and res.layers_d0 == res.layers
+    # the ground-state part of a response run is the same computation: same D0, same stop layer
+    r1, e0, _ = _run(wl, dev)
+    assert r1.layers_d0 == res.layers and np.array_equal(e0, d0)
+
+
+def test_finite_difference_of_ground_state_runs_gives_the_response(dev, config1):
+    """PAPER.md:562-566 (Eq. 83): D1 ~ [D0(H0 + h H1) - D0(H0 - h H1)] / 2h.  Two order-0 runs against the
+    order-1 run of the same library - the paper's own validation of the perturbation recursion (Fig. 5)."""
+    wl = config1
+    r1, _, d1 = _run(wl, dev)
+    h = 0.1                                                # truncation 1.2e-3 |D1|max (exact arithmetic), noise 2e-6/h
+    b = (r1.eps_min - 0.1, r1.eps_max + 0.1)               # common bounds: both runs take the same layers
+    hp = (wl.h0.astype(np.float64) + h * wl.h1).astype(np.float32)
+    hm = (wl.h0.astype(np.float64) - h * wl.h1).astype(np.float32)
+    _, dp = _run0(hp, wl.n_occ, dev, bounds=b)
+    _, dm = _run0(hm, wl.n_occ, dev, bounds=b)
+    fd = (dp - dm) / (2 * h)
+    # O(h^2) truncation (third-order response) + 2 x D0 noise / 2h
+    assert np.abs(fd - d1).max() <= 3e-3 * np.abs(d1).max(), np.abs(fd - d1).max() / np.abs(d1).max()

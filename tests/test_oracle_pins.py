@@ -343,3 +343,18 @@ def test_workloads_are_seeded_symmetric_and_gapped():
     lit = make_config(2, n=256, scissor=False)
     w = np.linalg.eigvalsh(lit.h0.astype(np.float64))
     assert w[lit.n_occ] - w[lit.n_occ - 1] < 0.2                                # W2: nearly gapless
+
+
+def test_ground_state_sp2_matches_the_definition():
+    """O2 with the response lines removed (oracle.dnn_sp2, the reference of the order-0 mode): D0 is the
+    projector onto the N_occ lowest eigenstates (Eq. 5), and its layer count is the D0 stop
+    layer of the full recursion (the ground-state part of Algorithm 1 does not depend on H1)."""
+    from workloads import make_config
+
+    for cfg, n in ((1, 96), (2, 128), (4, 160)):
+        wl = make_config(cfg, n=n)
+        d0, layers = O2.dnn_sp2(wl.h0, wl.n_occ)
+        ref0, _ = O1.density_matrices(wl.h0, wl.h1, wl.n_occ)
+        assert np.abs(d0 - ref0).max() < 1e-10
+        assert abs(np.trace(d0) - wl.n_occ) < 1e-9
+        assert layers == O2.dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ).layers_d0
