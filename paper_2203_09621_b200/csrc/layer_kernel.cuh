@@ -30,10 +30,16 @@
 // tiles loaded, against 1 per 2 for a plain GEMM.  Executed tensor work per layer is
 // 4.5 N^3 FMA (3 N^3 once S0 froze) against the paper's 5 N^3 (3 N^3).
 //
-// Warp roles: warp 0 TMA producer, warp 1 MMA issuer (one elected lane) and TMEM owner,
-// warps 2-9 epilogue: warp w owns TMEM lane quadrant w % 4 and column half (w - 2) / 4 of both
-// accumulators (64 + 64 fp32 registers per thread).  TMEM holds two accumulator stages
+// CTA pairs: a cluster of two CTAs (one TPC) shares a 256 x 128 pair tile through
+// tcgen05.mma.cta_group::2 (see the comment on the kernel).
+//
+// Warp roles (per CTA): warp 0 TMA producer, warp 1 MMA issuer (leader CTA, one elected lane) and
+// TMEM owner, warps 2-9 epilogue: warp w owns TMEM lane quadrant w % 4 and column half (w - 2) / 4
+// of both accumulators (64 + 64 fp32 registers per thread).  TMEM holds two accumulator stages
 // (2 x [P0 | P1] x 128 columns): the drain of chunk c overlaps the MMAs of chunk c + 1.
+//
+// Orders: PASS 0 of the kernel does orders 0 and 1 (order 0 alone when the context was created
+// with order = 0: ground-state mode); PASS 1 is the order-2 pass of a layer (a9).
 #pragma once
 #include <cuda_fp16.h>
 
