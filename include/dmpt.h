@@ -61,7 +61,10 @@ typedef struct dmpt_options {
     double eps_max;
     int wave_sync;     /* 1 (default): the CTAs of a layer launch re-align at every tile boundary so that   */
                        /* tiles in flight share operand panels through L2 (cooperative launch); 0: free run */
-    int reserved[7];   /* must be 0                                                                   */
+    int num_fields;    /* 1 (default; 0 reads as 1) .. 3 perturbations H1_a sharing H0, first order only:      */
+                       /* D1_a for each in one run - S0^2 once per layer, S0.S1_a per field (the x, y, z       */
+                       /* fields of the polarizability, Eq. 79).  Use the *_fields entry points.  */
+    int reserved[6];   /* must be 0                                                                   */
 } dmpt_options;
 
 typedef struct dmpt_result {
@@ -72,7 +75,8 @@ typedef struct dmpt_result {
     int layers_d1;     /* layer at which the D1 test fired (Algorithm 3); 0 if it never did           */
     int launches;      /* kernels this run launched (all of them this library's own)                  */
     int layers_d2;     /* order 2: layer at which the D2 test fired (R15); 0 otherwise            */
-    int reserved_i[2];
+    int layers_d3;     /* multi-field runs: stop layer of field 3 (layers_d2: field 2, layers_d1: field 1)   */
+    int reserved_i[1];
     double eps_min, eps_max;   /* spectral bounds used                                 */
     double fro_err0;           /* FroErr0 = ||S0 - S0^2||_F at the D0 stop layer; NaN at order 0 */
     double ms_total;           /* CUDA-event time of the whole run (bounds + transform + split + loop) */
@@ -88,15 +92,19 @@ typedef struct dmpt_result {
     double *tr_x;              /* N_X = Tr (S0_{n-1})^2, evaluated as ||S0_{n-1}||_F^2 (R9) */
     double *id_err;            /* IdErr_n = N_S - N_X; NaN once S0 froze                              */
     double *fro_err1;          /* FroErr1_n; NaN before D0 converged                   */
-    double *fro_err2;          /* FroErr2_n (order 2); NaN before D1 converged                        */
+    double *fro_err2;          /* FroErr2_n (order 2); NaN before D1 converged.  Multi-field: FroErr1 of field 2 */
+    double *fro_err3;          /* multi-field: FroErr1 of field 3 (else untouched)                    */
 } dmpt_result;
 
-/* Defaults: max_layers 200, order 1, s0_shift -1, s1_autoscale 1, bounds 0, wave_sync 1. */
+/* Defaults: max_layers 200, order 1, s0_shift -1, s1_autoscale 1, bounds 0, wave_sync 1, num_fields 1. */
 void dmpt_default_options(dmpt_options *opt);
 
 /* Bytes of device workspace dmpt_create() needs for matrices of size n at response order `order`
  * (0 on invalid arguments).  Layout is private; see DESIGN.md "HBM layout". */
 size_t dmpt_workspace_bytes(int n, int order);
+
+/* The same for a first-order context with num_fields (1..3) perturbations sharing H0. */
+size_t dmpt_workspace_bytes_fields(int n, int num_fields);
 
 /* Create a context for n x n problems.  `d_workspace` (device, >= dmpt_workspace_bytes(), 256-byte
  * aligned) stays owned by the caller and must outlive the context.  `cuda_stream` is a cudaStream_t
@@ -113,6 +121,15 @@ int dmpt_set_hamiltonian(dmpt_ctx *ctx, const float *d_h0, const float *d_h1, in
  * with leading dimension ld >= n.  `res` may be NULL.  On DMPT_ENOCONV the outputs hold the last
  * iterate.  Safe to call repeatedly. */
 int dmpt_run(dmpt_ctx *ctx, float *d_d0, float *d_d1, float *d_d2, int ld, dmpt_result *res);
+
+/* Multi-field variants (contexts created with order == 1 and num_fields >= 1).
+ * d_h1 / d_d1 are HOST arrays of num_fields DEVICE matrix pointers, all with leading dimension ld.
+ * Every field runs Algorithm 3 on its own (its own stop layer, its own power-of-two scale); the run ends
+ * when all have stopped.  Each D1_a is bit-identical to the single-field run of (H0, H1_a).  Per layer the
+ * tensor work is 3 + 6 num_fields products per tile instead of 9 num_fields.  res->layers_d1/_d2/_d3 and
+ * fro_err1/2/3 belong to fields 1/2/3. */
+int dmpt_set_hamiltonian_fields(dmpt_ctx *ctx, const float *d_h0, const float *const *d_h1, int ld, int n_occ);
+int dmpt_run_fields(dmpt_ctx *ctx, float *d_d0, float *const *d_d1, int ld, dmpt_result *res);
 
 /* The same call with HOST matrices (pinned memory recommended): copies H0, H1 to the device, runs,
  * and copies D0, D1 (D2) back, all on the context's stream.  ms_total then covers the copies too. */

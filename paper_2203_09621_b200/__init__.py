@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     DmptResult,
     dmpt_create,
     dmpt_default_options,
+    dmpt_workspace_bytes_fields,
     dmpt_destroy,
     dmpt_last_cuda_error,
     dmpt_layer_products,

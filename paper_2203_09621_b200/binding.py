@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = (
     "dmpt_default_options", "dmpt_workspace_bytes", "dmpt_create", "dmpt_set_hamiltonian",
     "dmpt_run", "dmpt_run_host", "dmpt_layer_products", "dmpt_destroy", "dmpt_strerror",
     "dmpt_last_cuda_error", "dmpt_spectral_bounds", "dmpt_initial_transform", "dmpt_split",
-    "dmpt_layer_products2",
+    "dmpt_layer_products2", "dmpt_workspace_bytes_fields", "dmpt_set_hamiltonian_fields", "dmpt_run_fields",
 )
 
 DMPT_OK, DMPT_EINVAL, DMPT_ESTATE, DMPT_ECUDA = 0, -1, -2, -3
@@ -28,20 +28,20 @@ class DmptOptions(C.Structure):
         ("max_layers", C.c_int), ("order", C.c_int), ("s0_shift", C.c_int),
         ("s1_autoscale", C.c_int), ("bounds", C.c_int),
         ("eps_min", C.c_double), ("eps_max", C.c_double),
-        ("wave_sync", C.c_int), ("reserved", C.c_int * 7),
+        ("wave_sync", C.c_int), ("num_fields", C.c_int), ("reserved", C.c_int * 6),
     ]
 
 
 class _CResult(C.Structure):
     _fields_ = [
         ("status", C.c_int), ("layers", C.c_int), ("layers_d0", C.c_int), ("layers_d1", C.c_int),
-        ("launches", C.c_int), ("layers_d2", C.c_int), ("reserved_i", C.c_int * 2),
+        ("launches", C.c_int), ("layers_d2", C.c_int), ("layers_d3", C.c_int), ("reserved_i", C.c_int * 1),
         ("eps_min", C.c_double), ("eps_max", C.c_double), ("fro_err0", C.c_double),
         ("ms_total", C.c_double), ("ms_loop", C.c_double), ("ms_bounds", C.c_double),
         ("ms_transform", C.c_double), ("ms_split", C.c_double), ("reserved_d", C.c_double * 1),
         ("sigma", C.POINTER(C.c_int8)), ("tr_s", C.POINTER(C.c_double)), ("tr_x", C.POINTER(C.c_double)),
         ("id_err", C.POINTER(C.c_double)), ("fro_err1", C.POINTER(C.c_double)),
-        ("fro_err2", C.POINTER(C.c_double)),
+        ("fro_err2", C.POINTER(C.c_double)), ("fro_err3", C.POINTER(C.c_double)),
     ]
 
 
@@ -70,6 +70,12 @@ def lib():
         L.dmpt_default_options.restype = None
         L.dmpt_workspace_bytes.argtypes = [C.c_int, C.c_int]
         L.dmpt_workspace_bytes.restype = C.c_size_t
+        L.dmpt_workspace_bytes_fields.argtypes = [C.c_int, C.c_int]
+        L.dmpt_workspace_bytes_fields.restype = C.c_size_t
+        L.dmpt_set_hamiltonian_fields.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_int, C.c_int]
+        L.dmpt_set_hamiltonian_fields.restype = C.c_int
+        L.dmpt_run_fields.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_int, C.POINTER(_CResult)]
+        L.dmpt_run_fields.restype = C.c_int
         L.dmpt_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.POINTER(DmptOptions), C.c_void_p,
                                   C.c_size_t, C.c_void_p]
         L.dmpt_create.restype = C.c_int
@@ -113,6 +119,22 @@ def dmpt_default_options() -> DmptOptions:
 
 def dmpt_workspace_bytes(n: int, order: int = 1) -> int:
     return int(lib().dmpt_workspace_bytes(int(n), int(order)))
+
+
+def dmpt_workspace_bytes_fields(n: int, num_fields: int) -> int:
+    return int(lib().dmpt_workspace_bytes_fields(int(n), int(num_fields)))
+
+
+def dmpt_set_hamiltonian_fields(ctx, h0_ptr: int, h1_ptrs, ld: int, n_occ: int) -> None:
+    arr = (C.c_void_p * len(h1_ptrs))(*[C.c_void_p(p) for p in h1_ptrs])
+    rc = lib().dmpt_set_hamiltonian_fields(ctx, C.c_void_p(h0_ptr), arr, int(ld), int(n_occ))
+    if rc != DMPT_OK:
+        raise DmptError(rc, "dmpt_set_hamiltonian_fields")
+
+
+def dmpt_run_fields(ctx, d0_ptr: int, d1_ptrs, ld: int, res) -> int:
+    arr = (C.c_void_p * len(d1_ptrs))(*[C.c_void_p(p) for p in d1_ptrs])
+    return int(lib().dmpt_run_fields(ctx, C.c_void_p(d0_ptr), arr, int(ld), C.byref(res) if res is not None else None))
 
 
 def dmpt_strerror(code: int) -> str:
@@ -205,6 +227,8 @@ class DmptResult:
     id_err: list = field(default_factory=list)
     fro_err1: list = field(default_factory=list)
     fro_err2: list = field(default_factory=list)
+    fro_err3: list = field(default_factory=list)
+    layers_d3: int = 0
     d0: object = None
     d1: object = None
     d2: object = None
@@ -214,7 +238,7 @@ class Dmpt:
     """Owns a dmpt_ctx plus the torch-allocated workspace.  Marshalling only."""
 
     def __init__(self, n, order=1, max_layers=200, s0_shift=-1, s1_autoscale=True, bounds=None,
-                 device="cuda:0", stream=None, wave_sync=True):
+                 device="cuda:0", stream=None, wave_sync=True, num_fields=1):
         import torch
 
         self.torch = torch
@@ -229,11 +253,14 @@ class Dmpt:
         opt.s0_shift = int(s0_shift)
         opt.s1_autoscale = 1 if s1_autoscale else 0
         opt.wave_sync = 1 if wave_sync else 0
+        opt.num_fields = int(num_fields)
+        self.num_fields = int(num_fields)
         if bounds is not None:
             opt.bounds = 1
             opt.eps_min, opt.eps_max = float(bounds[0]), float(bounds[1])
         self.max_layers = opt.max_layers
-        nbytes = dmpt_workspace_bytes(self.n, self.order)
+        nbytes = (dmpt_workspace_bytes_fields(self.n, self.num_fields) if self.num_fields > 1
+                  else dmpt_workspace_bytes(self.n, self.order))
         if nbytes == 0:
             raise DmptError(DMPT_EINVAL, "dmpt_workspace_bytes")
         with torch.cuda.device(self.device):
@@ -255,10 +282,11 @@ class Dmpt:
     def _new_result(self):
         ml = self.max_layers
         bufs = dict(sigma=(C.c_int8 * ml)(), tr_s=(C.c_double * ml)(), tr_x=(C.c_double * ml)(),
-                    id_err=(C.c_double * ml)(), fro_err1=(C.c_double * ml)(), fro_err2=(C.c_double * ml)())
+                    id_err=(C.c_double * ml)(), fro_err1=(C.c_double * ml)(), fro_err2=(C.c_double * ml)(),
+                    fro_err3=(C.c_double * ml)())
         r = _CResult()
         r.sigma = C.cast(bufs["sigma"], C.POINTER(C.c_int8))
-        for k in ("tr_s", "tr_x", "id_err", "fro_err1", "fro_err2"):
+        for k in ("tr_s", "tr_x", "id_err", "fro_err1", "fro_err2", "fro_err3"):
             setattr(r, k, C.cast(bufs[k], C.POINTER(C.c_double)))
         return r, bufs
 
@@ -273,8 +301,9 @@ class Dmpt:
                           sigma=list(bufs["sigma"][:nl]), tr_s=list(bufs["tr_s"][:nl]),
                           tr_x=list(bufs["tr_x"][:nl]), id_err=list(bufs["id_err"][:nl]),
                           fro_err1=list(bufs["fro_err1"][:nl]),
-                          fro_err2=list(bufs["fro_err2"][:nl]) if self.order == 2 else [],
-                          layers_d2=r.layers_d2, d0=d0, d1=d1, d2=d2)
+                          fro_err2=list(bufs["fro_err2"][:nl]) if (self.order == 2 or self.num_fields > 1) else [],
+                          fro_err3=list(bufs["fro_err3"][:nl]) if self.num_fields > 2 else [],
+                          layers_d2=r.layers_d2, layers_d3=r.layers_d3, d0=d0, d1=d1, d2=d2)
 
     def run(self, out=None, check=True) -> DmptResult:
         t = self.torch
@@ -294,6 +323,29 @@ class Dmpt:
         rc = dmpt_run(self.ctx, d0.data_ptr(), d1.data_ptr() if d1 is not None else 0,
                       d2.data_ptr() if d2 is not None else 0, d0.stride(0), r)
         return self._wrap(rc, r, bufs, d0, d1, d2, check)
+
+    def set_hamiltonian_fields(self, h0, h1s, n_occ):
+        """h1s: num_fields perturbations sharing h0 (row-major fp32 CUDA matrices with h0's leading dimension)."""
+        t = self.torch
+        h1s = list(h1s)
+        for m in [h0] + h1s:
+            if not (m.is_cuda and m.dtype == t.float32 and m.dim() == 2 and m.stride(1) == 1
+                    and m.stride(0) == h0.stride(0)):
+                raise DmptError(DMPT_EINVAL, "set_hamiltonian_fields", "need row-major fp32 CUDA matrices, one ld")
+        if len(h1s) != self.num_fields:
+            raise DmptError(DMPT_EINVAL, "set_hamiltonian_fields", f"need {self.num_fields} perturbations")
+        self._h = (h0, h1s)
+        dmpt_set_hamiltonian_fields(self.ctx, h0.data_ptr(), [m.data_ptr() for m in h1s], h0.stride(0), n_occ)
+
+    def run_fields(self, check=True) -> DmptResult:
+        """D0 and one D1 per field; the result's d1 is the list of them."""
+        t = self.torch
+        n = self.n
+        d0 = t.empty((n, n), dtype=t.float32, device=self.device)
+        d1s = [t.empty((n, n), dtype=t.float32, device=self.device) for _ in range(self.num_fields)]
+        r, bufs = self._new_result()
+        rc = dmpt_run_fields(self.ctx, d0.data_ptr(), [m.data_ptr() for m in d1s], n, r)
+        return self._wrap(rc, r, bufs, d0, d1s, None, check)
 
     def run_host(self, h0, h1, n_occ, out=None, check=True) -> DmptResult:
         """h0, h1: CPU fp32 tensors (pinned recommended); outputs are CPU tensors."""

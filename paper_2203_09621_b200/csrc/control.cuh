@@ -27,8 +27,13 @@ enum Red : int {
     RED_MAX1 = 4,    // max |new S1|                                    -> next S1 scale
     RED_FRO2 = 5,    // sum (S2 - X2)^2 once D1 converged (order 2)     -> FroErr2_n^2
     RED_MAX2 = 6,    // max |new S2|
-    RED_COUNT = 8
+    RED_FRO3 = 7,    // third response slot (multi-field runs only)
+    RED_MAX3 = 8,
+    RED_COUNT = 10
 };
+// Response slots.  Slot 1 is S1 of the (first) perturbation.  Slot 2 is S2 at order 2, or S1 of a SECOND
+// perturbation sharing H0 in a multi-field first-order run (the x, y, z fields of the
+// polarizability, Eq. 79); slot 3 is S1 of a third perturbation.
 
 enum Mode0 : int { MODE_ACTIVE = 0, MODE_STOP = 1, MODE_FROZEN = 2 };
 
@@ -42,12 +47,14 @@ struct DmptCtl {
     int s0_buf;     // hi/lo buffer holding S0_{n-1}
     int s1_buf;     // fp32 + hi/lo buffer holding S1_{n-1}
     int s2_buf;
+    int s3_buf;
     int e1_in;      // S1 operand buffers hold fp16(2^e1_in S1_{n-1})
     int e1_out;     // scale for the split of S1_n
     int e2_in, e2_out;
+    int e3_in, e3_out;
     // ---- state of Algorithms 1-3
-    int conv0, conv1, conv2;
-    int n_c, n_c1, n_c2;
+    int conv0, conv1, conv2, conv3;
+    int n_c, n_c1, n_c2, n_c3;
     int layers;     // layers executed so far
     int single_shot;  // 1: dmpt_layer_products - run one layer, take no decisions
     unsigned int ticket;  // CTA arrival counter of the running launch
@@ -57,7 +64,7 @@ struct DmptCtl {
     double n_x;     // ||S0_{n-1}||_F^2
     double fro0;    // FroErr0
     double eps_min, eps_max;
-    double s1_max, s2_max;
+    double s1_max, s2_max, s3_max;
 };
 
 struct DmptLogs {   // device arrays, max_layers entries, entry n-1 for layer n
@@ -67,10 +74,12 @@ struct DmptLogs {   // device arrays, max_layers entries, entry n-1 for layer n
     double* id_err;
     double* fro1;
     double* fro2;
+    double* fro3;
 };
 
 struct DmptProblem {
     int n, n_pad, n_occ, order, max_layers, s0_shift, s1_autoscale;
+    int nfields;     // 1..3 perturbations sharing H0 (order 1 only above 1)
 };
 
 // exact power of two 2^e bringing m into [8, 16); 0 when m is 0 or not finite
@@ -130,6 +139,37 @@ __device__ inline void control_decide(DmptCtl& c, const DmptLogs& L, const DmptP
     }
 }
 
+// One response slot after layer n: record FroErr_n = ||S - X||_F once its gate opened (D0 converged for a
+// first-order slot, D1 converged for the second-order slot), run the test of Algorithm 3 from
+// `gate_layer + 2` on (R5, R6), and accept the new iterate unless the test fired.
+__device__ inline void response_step(DmptCtl& c, const DmptProblem& pb, int n, bool gate, int gate_layer, int& conv,
+                                     int& n_conv, int& buf, int& e_in, int& e_out, double& mx, double fro_sq,
+                                     double max_new, double* log) {
+    const double nanv = nan("");
+    if (conv) {
+        log[n - 1] = nanv;
+        return;
+    }
+    if (gate) {
+        const double f = sqrt(fro_sq);
+        log[n - 1] = f;
+        if (n - 2 >= gate_layer && !(f < kCPT * c.fro0 * log[n - 3])) {
+            conv = 1;
+            n_conv = n;
+        }
+        if (!isfinite(f) || !isfinite(c.fro0)) c.status = -6;
+    } else {
+        log[n - 1] = nanv;
+    }
+    if (!conv) {   // accept the new iterate
+        buf ^= 1;
+        e_in = e_out;
+        mx = max_new;
+        if (pb.s1_autoscale) e_out = scale_exponent(mx);
+        if (!isfinite(mx)) c.status = -6;
+    }
+}
+
 // After layer n = ctl.layer ran: fold its reductions into the state, apply Algorithm 3
 // (cascade for order 2, reading R15) and decide layer n+1.
 __device__ inline void control_finalize(DmptCtl& c, const DmptLogs& L, const DmptProblem& pb,
@@ -147,56 +187,30 @@ __device__ inline void control_finalize(DmptCtl& c, const DmptLogs& L, const Dmp
     } else if (c.mode0 == MODE_STOP) {
         c.fro0 = sqrt(red[RED_FRO0]);
     }
-    const double nanv = nan("");
-    // ---- first order
-    if (pb.order >= 1 && !c.conv1) {
-        if (c.conv0) {
-            const double f1 = sqrt(red[RED_FRO1]);
-            L.fro1[n - 1] = f1;
-            if (n - 2 >= c.n_c && !(f1 < kCPT * c.fro0 * L.fro1[n - 3])) {     // R5, R6
-                c.conv1 = 1;
-                c.n_c1 = n;
-            }
-            if (!isfinite(f1) || !isfinite(c.fro0)) c.status = -6;
-        } else {
-            L.fro1[n - 1] = nanv;
-        }
-        if (!c.conv1) {   // accept S1_n
-            c.s1_buf ^= 1;
-            c.e1_in = c.e1_out;
-            c.s1_max = red[RED_MAX1];
-            if (pb.s1_autoscale) c.e1_out = scale_exponent(c.s1_max);
-            if (!isfinite(c.s1_max)) c.status = -6;
-        }
-    } else {
-        L.fro1[n - 1] = nanv;
-    }
-    // ---- second order
-    if (pb.order == 2 && !c.conv2) {
-        if (c.conv1) {
-            const double f2 = sqrt(red[RED_FRO2]);
-            L.fro2[n - 1] = f2;
-            if (n - 2 >= c.n_c1 && !(f2 < kCPT * c.fro0 * L.fro2[n - 3])) {
-                c.conv2 = 1;
-                c.n_c2 = n;
-            }
-            if (!isfinite(f2)) c.status = -6;
-        } else {
-            L.fro2[n - 1] = nanv;
-        }
-        if (!c.conv2) {
-            c.s2_buf ^= 1;
-            c.e2_in = c.e2_out;
-            c.s2_max = red[RED_MAX2];
-            if (pb.s1_autoscale) c.e2_out = scale_exponent(c.s2_max);
-            if (!isfinite(c.s2_max)) c.status = -6;
-        }
+    // ---- first order (slot 1): Algorithm 3, tested from layer n_c + 2 on
+    if (pb.order >= 1)
+        response_step(c, pb, n, c.conv0 != 0, c.n_c, c.conv1, c.n_c1, c.s1_buf, c.e1_in, c.e1_out, c.s1_max,
+                      red[RED_FRO1], red[RED_MAX1], L.fro1);
+    else
+        L.fro1[n - 1] = nan("");
+    if (pb.order == 2) {
+        // ---- second order (slot 2): the same test cascaded behind the D1 stop (reading R15)
+        response_step(c, pb, n, c.conv1 != 0, c.n_c1, c.conv2, c.n_c2, c.s2_buf, c.e2_in, c.e2_out, c.s2_max,
+                      red[RED_FRO2], red[RED_MAX2], L.fro2);
+    } else if (pb.nfields >= 2) {
+        // ---- further first-order fields (slots 2, 3): each runs Algorithm 3 on its own, like slot 1
+        response_step(c, pb, n, c.conv0 != 0, c.n_c, c.conv2, c.n_c2, c.s2_buf, c.e2_in, c.e2_out, c.s2_max,
+                      red[RED_FRO2], red[RED_MAX2], L.fro2);
+        if (pb.nfields >= 3)
+            response_step(c, pb, n, c.conv0 != 0, c.n_c, c.conv3, c.n_c3, c.s3_buf, c.e3_in, c.e3_out, c.s3_max,
+                          red[RED_FRO3], red[RED_MAX3], L.fro3);
     }
     if (c.status != 0) {
         c.done = 1;
         return;
     }
-    if (pb.order == 2 ? c.conv2 : (pb.order == 1 && c.conv1)) {
+    const bool all_fields = c.conv1 && (pb.nfields < 2 || c.conv2) && (pb.nfields < 3 || c.conv3);
+    if (pb.order == 2 ? c.conv2 != 0 : (pb.order == 1 && all_fields)) {
         c.done = 1;
         return;
     }

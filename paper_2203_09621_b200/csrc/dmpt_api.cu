@@ -36,10 +36,10 @@ struct Carve {
 };
 
 struct Layout {
-    int n, n_pad, order, num_tiles;
-    size_t ctl, bounds, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, partials, partials2, tiles;
-    size_t s0, s1[2], s2[2];
-    size_t h[2][6];          // [buffer][S0hi, S0lo, S1hi, S1lo, S2hi, S2lo]
+    int n, n_pad, order, nfields, num_tiles;
+    size_t ctl, bounds, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, fro3, partials, partials2, tiles;
+    size_t s0, s1[2], s2[2], s3[2];
+    size_t h[2][8];          // [buffer][S0hi, S0lo, S1hi, S1lo, slot-2 hi, lo, slot-3 hi, lo]
     size_t stage_h0, stage_h1;
     size_t total;
 };
@@ -51,10 +51,14 @@ int num_tiles_for(int nb) {
     return t;
 }
 
-Layout make_layout(int n, int order) {
+// response slots in use: 1 (order 1), 2 (order 2, or two fields), 3 (three fields); 0 at order 0
+int num_slots(int order, int nfields) { return order == 2 ? 2 : (order == 1 ? nfields : 0); }
+
+Layout make_layout(int n, int order, int nfields) {
     Layout L{};
     L.n = n;
     L.order = order;
+    L.nfields = nfields;
     L.n_pad = (int)align_up((size_t)n, kPair);
     const int nb = L.n_pad / kTile;
     L.num_tiles = num_tiles_for(nb);
@@ -69,17 +73,23 @@ Layout make_layout(int n, int order) {
     L.id_err = c.take(kMaxLayersCap * sizeof(double));
     L.fro1 = c.take(kMaxLayersCap * sizeof(double));
     L.fro2 = c.take(kMaxLayersCap * sizeof(double));
+    L.fro3 = c.take(kMaxLayersCap * sizeof(double));
     L.partials = c.take(kPartialDoubles * sizeof(double));
     L.partials2 = c.take(kPartialDoubles * sizeof(double));
     L.tiles = c.take((size_t)L.num_tiles * sizeof(uint32_t));
     L.s0 = c.take(np2 * 4);
     L.s1[0] = c.take(np2 * 4);
     L.s1[1] = c.take(np2 * 4);
-    if (order == 2) {
+    const int slots = num_slots(order, nfields);
+    if (slots >= 2) {
         L.s2[0] = c.take(np2 * 4);
         L.s2[1] = c.take(np2 * 4);
     }
-    const int nh = order == 2 ? 6 : 4;
+    if (slots >= 3) {
+        L.s3[0] = c.take(np2 * 4);
+        L.s3[1] = c.take(np2 * 4);
+    }
+    const int nh = 2 + 2 * (slots < 1 ? 1 : slots);
     for (int b = 0; b < 2; ++b)
         for (int m = 0; m < nh; ++m) L.h[b][m] = c.take(np2 * 2);
     L.stage_h0 = c.take((size_t)n * n * 4);
@@ -116,7 +126,8 @@ struct dmpt_ctx {
     uint8_t* ws = nullptr;
     cudaStream_t stream = nullptr;
     const float* d_h0 = nullptr;
-    const float* d_h1 = nullptr;
+    const float* d_h1 = nullptr;          // field 1
+    const float* d_h1x[2] = {nullptr, nullptr};   // fields 2, 3 (multi-field contexts)
     int num_sms = 0;
     int grid_layer = 0;
     int s0_shift = 14;
@@ -150,11 +161,17 @@ extern "C" void dmpt_default_options(dmpt_options* opt) {
     opt->s1_autoscale = 1;
     opt->bounds = 0;
     opt->wave_sync = 1;
+    opt->num_fields = 1;
 }
 
 extern "C" size_t dmpt_workspace_bytes(int n, int order) {
     if (n <= 0 || order < 0 || order > 2 || n > 65535 * kTile) return 0;
-    return make_layout(n, order).total;
+    return make_layout(n, order, 1).total;
+}
+
+extern "C" size_t dmpt_workspace_bytes_fields(int n, int num_fields) {
+    if (n <= 0 || num_fields < 1 || num_fields > 3 || n > 65535 * kTile) return 0;
+    return make_layout(n, 1, num_fields).total;
 }
 
 extern "C" const char* dmpt_strerror(int code) {
@@ -187,7 +204,8 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
     const cuuint64_t strides[1] = {(cuuint64_t)L.n_pad * 2};
     const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)kBRows};
     const cuuint32_t estr[2] = {1, 1};
-    const int nh = L.order == 2 ? 6 : 4;
+    const int slots = num_slots(L.order, L.nfields);
+    const int nh = 2 + 2 * (slots < 1 ? 1 : slots);
     for (int b = 0; b < 2; ++b)
         for (int m = 0; m < nh; ++m) {
             CUresult r = encode(&ctx->lp.maps[b][m], CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
@@ -212,7 +230,9 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     if (o.max_layers <= 0) o.max_layers = 200;
     if (o.max_layers > kMaxLayersCap) o.max_layers = kMaxLayersCap;
     if (o.s0_shift > 15) return DMPT_EINVAL;
-    const size_t need = dmpt_workspace_bytes(n, o.order);
+    if (o.num_fields == 0) o.num_fields = 1;
+    if (o.num_fields < 1 || o.num_fields > 3 || (o.num_fields > 1 && o.order != 1)) return DMPT_EINVAL;
+    const size_t need = o.num_fields > 1 ? dmpt_workspace_bytes_fields(n, o.num_fields) : dmpt_workspace_bytes(n, o.order);
     if (need == 0) return DMPT_EINVAL;
     if (workspace_bytes < need || (reinterpret_cast<uintptr_t>(d_workspace) & 255)) return DMPT_EWORKSPACE;
 
@@ -220,7 +240,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     ctx->n = n;
     ctx->opt = o;
     ctx->s0_shift = o.s0_shift < 0 ? 14 : o.s0_shift;
-    ctx->L = make_layout(n, o.order);
+    ctx->L = make_layout(n, o.order, o.num_fields);
     ctx->ws = static_cast<uint8_t*>(d_workspace);
     ctx->stream = static_cast<cudaStream_t>(cuda_stream);
     auto fail = [&](int code) {
@@ -256,6 +276,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     CKC(cudaHostAlloc(&ctx->h_ctl, sizeof(DmptCtl), cudaHostAllocDefault));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<0>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<1>()));
+    CKC(cudaFuncSetAttribute(dmpt_layer_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<2>()));
 
     const Layout& L = ctx->L;
     const int nb = L.n_pad / kTile;
@@ -286,10 +307,12 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.s0 = ctx->at<float>(L.s0);
     lp.s1[0] = ctx->at<float>(L.s1[0]);
     lp.s1[1] = ctx->at<float>(L.s1[1]);
-    const int nh = o.order == 2 ? 6 : 4;
+    const int slots = num_slots(o.order, o.num_fields);
+    const int nh = 2 + 2 * (slots < 1 ? 1 : slots);
     for (int b = 0; b < 2; ++b) {
-        lp.s2[b] = o.order == 2 ? ctx->at<float>(L.s2[b]) : nullptr;
-        for (int m = 0; m < 6; ++m) lp.h[b][m] = m < nh ? ctx->at<__half>(L.h[b][m]) : nullptr;
+        lp.s2[b] = slots >= 2 ? ctx->at<float>(L.s2[b]) : nullptr;
+        lp.s3[b] = slots >= 3 ? ctx->at<float>(L.s3[b]) : nullptr;
+        for (int m = 0; m < 8; ++m) lp.h[b][m] = m < nh ? ctx->at<__half>(L.h[b][m]) : nullptr;
     }
     lp.tiles = ctx->at<uint32_t>(L.tiles);
     lp.num_tiles = L.num_tiles;
@@ -302,6 +325,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.logs.id_err = ctx->at<double>(L.id_err);
     lp.logs.fro1 = ctx->at<double>(L.fro1);
     lp.logs.fro2 = ctx->at<double>(L.fro2);
+    lp.logs.fro3 = ctx->at<double>(L.fro3);
     lp.partials = ctx->at<double>(L.partials);
     lp.partials2 = ctx->at<double>(L.partials2);
     lp.pb.n = n;
@@ -311,6 +335,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.pb.max_layers = o.max_layers;
     lp.pb.s0_shift = ctx->s0_shift;
     lp.pb.s1_autoscale = o.s1_autoscale ? 1 : 0;
+    lp.pb.nfields = o.num_fields;
     if (build_tensor_maps(ctx) != DMPT_OK) return fail(DMPT_ECUDA);
 #undef CKC
     *out = ctx;
@@ -359,9 +384,24 @@ static int launch_pass(dmpt_ctx* ctx) {
 
 // One layer: at order 2 the S2 pass goes first (it reads the iterates pass 0 is about to replace and
 // leaves its reductions for pass 0's control step).
+extern "C" int dmpt_set_hamiltonian_fields(dmpt_ctx* ctx, const float* d_h0, const float* const* d_h1, int ld,
+                                           int n_occ) {
+    if (!ctx || !d_h0 || !d_h1 || ctx->opt.order != 1) return DMPT_EINVAL;
+    for (int f = 0; f < ctx->opt.num_fields; ++f)
+        if (!d_h1[f]) return DMPT_EINVAL;
+    int rc = dmpt_set_hamiltonian(ctx, d_h0, d_h1[0], ld, n_occ);
+    if (rc) return rc;
+    for (int f = 1; f < ctx->opt.num_fields; ++f) ctx->d_h1x[f - 1] = d_h1[f];
+    return DMPT_OK;
+}
+
 static int launch_layer(dmpt_ctx* ctx, int* launches) {
     if (ctx->opt.order == 2) {
         int rc = launch_pass<1>(ctx);
+        if (rc) return rc;
+        ++*launches;
+    } else if (ctx->opt.num_fields > 1) {       // fields 2 (and 3): same ordering argument as the order-2 pass
+        int rc = launch_pass<2>(ctx);
         if (rc) return rc;
         ++*launches;
     }
@@ -426,6 +466,19 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
         CK(cudaGetLastError());
         *launches += 2;
     }
+    for (int f = 1; f < ctx->opt.num_fields; ++f) {
+        // fields 2, 3 share H0: the transform kernel is run again for (H0, H1_f) - it rewrites S0 with the
+        // same values and leaves S1 of the field in response slot f + 1 - then the slot's first scale and split
+        float* dst = f == 1 ? ctx->lp.s2[0] : ctx->lp.s3[0];
+        dmpt_transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, ctx->d_h1x[f - 1], n, ld, np, ctx->lp.s0, dst, ctl, partials);
+        CK(cudaGetLastError());
+        dmpt_field_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, tgrid, f + 1);
+        CK(cudaGetLastError());
+        dmpt_split_kernel<<<sgrid, 256, 0, st>>>(dst, c8, (int)np, ctx->lp.h[0][2 + 2 * f], ctx->lp.h[0][3 + 2 * f], ctl,
+                                                 f + 1, ctx->s0_shift, 0);
+        CK(cudaGetLastError());
+        *launches += 3;
+    }
     CK(cudaEventRecord(ctx->ev_t[1], st));
 
     // Layer loop.  Launches are enqueued in chunks, two chunks ahead of the GPU; after each chunk a
@@ -469,6 +522,7 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
         res->layers_d0 = c.n_c;
         res->layers_d1 = c.n_c1;
         res->layers_d2 = c.n_c2;
+        res->layers_d3 = c.n_c3;
         res->launches = launches;
         res->eps_min = c.eps_min;
         res->eps_max = c.eps_max;
@@ -495,8 +549,10 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
             if (res->tr_x) CK(cudaMemcpy(res->tr_x, ctx->at<double>(L.tr_x), nl * sizeof(double), cudaMemcpyDeviceToHost));
             if (res->id_err) CK(cudaMemcpy(res->id_err, ctx->at<double>(L.id_err), nl * sizeof(double), cudaMemcpyDeviceToHost));
             if (res->fro_err1) CK(cudaMemcpy(res->fro_err1, ctx->at<double>(L.fro1), nl * sizeof(double), cudaMemcpyDeviceToHost));
-            if (res->fro_err2 && ctx->opt.order == 2)
+            if (res->fro_err2 && (ctx->opt.order == 2 || ctx->opt.num_fields > 1))
                 CK(cudaMemcpy(res->fro_err2, ctx->at<double>(L.fro2), nl * sizeof(double), cudaMemcpyDeviceToHost));
+            if (res->fro_err3 && ctx->opt.num_fields > 2)
+                CK(cudaMemcpy(res->fro_err3, ctx->at<double>(L.fro3), nl * sizeof(double), cudaMemcpyDeviceToHost));
         }
     }
     return status;
@@ -512,7 +568,7 @@ static int fetch_ctl(dmpt_ctx* ctx) {
 extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, int ld, dmpt_result* res) {
     if (!ctx || !d_d0 || (!d_d1 && ctx->opt.order != 0)) return DMPT_EINVAL;
     if (!ctx->d_h0) return DMPT_ESTATE;
-    if (ld < ctx->n || (ctx->opt.order == 2 && !d_d2)) return DMPT_EINVAL;
+    if (ld < ctx->n || (ctx->opt.order == 2 && !d_d2) || ctx->opt.num_fields > 1) return DMPT_EINVAL;
     const Layout& L = ctx->L;
     const size_t n = ctx->n, np = L.n_pad;
     int launches = 0;
@@ -530,12 +586,35 @@ extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, in
     return finish(ctx, res, launches);
 }
 
+extern "C" int dmpt_run_fields(dmpt_ctx* ctx, float* d_d0, float* const* d_d1, int ld, dmpt_result* res) {
+    if (!ctx || !d_d0 || !d_d1 || ctx->opt.order != 1) return DMPT_EINVAL;
+    const int nf = ctx->opt.num_fields;
+    for (int f = 0; f < nf; ++f)
+        if (!d_d1[f]) return DMPT_EINVAL;
+    if (!ctx->d_h0 || (nf > 1 && !ctx->d_h1x[0]) || (nf > 2 && !ctx->d_h1x[1])) return DMPT_ESTATE;
+    if (ld < ctx->n) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    int launches = 0;
+    CK(cudaEventRecord(ctx->ev_t[0], ctx->stream));
+    int rc = run_core(ctx, ctx->d_h0, ctx->d_h1, ctx->ld_in, &launches);
+    if (rc) return rc;
+    if ((rc = fetch_ctl(ctx))) return rc;
+    const DmptCtl& c = *ctx->h_ctl;
+    const float* src[3] = {ctx->lp.s1[c.s1_buf & 1], nf > 1 ? ctx->lp.s2[c.s2_buf & 1] : nullptr,
+                           nf > 2 ? ctx->lp.s3[c.s3_buf & 1] : nullptr};
+    CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
+    for (int f = 0; f < nf; ++f)
+        CK(cudaMemcpy2DAsync(d_d1[f], (size_t)ld * 4, src[f], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
+    return finish(ctx, res, launches);
+}
+
 extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1, int ld_in, int n_occ,
                              float* h_d0, float* h_d1, float* h_d2, int ld_out, dmpt_result* res) {
     if (!ctx || !h_h0 || !h_d0) return DMPT_EINVAL;
     if (ctx->opt.order != 0 && (!h_h1 || !h_d1)) return DMPT_EINVAL;
     if (ld_in < ctx->n || ld_out < ctx->n || n_occ <= 0 || n_occ >= ctx->n) return DMPT_EINVAL;
-    if (ctx->opt.order == 2 && !h_d2) return DMPT_EINVAL;
+    if ((ctx->opt.order == 2 && !h_d2) || ctx->opt.num_fields > 1) return DMPT_EINVAL;
     const Layout& L = ctx->L;
     const size_t n = ctx->n, np = L.n_pad;
     float* s_h0 = ctx->at<float>(L.stage_h0);

@@ -262,11 +262,23 @@ __global__ void dmpt_s2_scale_init_kernel(DmptCtl* ctl, DmptProblem pb, const un
     ctl->e2_out = pb.s1_autoscale ? scale_exponent(m) : 0;
 }
 
+// Multi-field runs: first scale of response slot 2 or 3 from max|S1_0| of that field (the third of the
+// per-block partials the transform kernel wrote for it).
+__global__ void dmpt_field_init_kernel(DmptCtl* ctl, DmptProblem pb, const double* __restrict__ partials, int nblocks,
+                                       int slot) {
+    if (threadIdx.x | blockIdx.x) return;
+    double m = 0.0;
+    for (int b = 0; b < nblocks; ++b) m = fmax(m, partials[b * 3 + 2]);
+    const int e = pb.s1_autoscale ? scale_exponent(m) : 0;
+    if (slot == 2) { ctl->s2_max = m; ctl->e2_in = ctl->e2_out = e; }
+    else { ctl->s3_max = m; ctl->e3_in = ctl->e3_out = e; }
+}
+
 // ---------------------------------------------------------------------------------------------
 // a3  Split (Eq. 13, 302-307 Eqs. 42-43) after an exact power-of-two scale 2^e
 //     (readings R12/R17): hi = fp16(2^e x), lo = fp16(2^e x - hi), round-to-nearest-even.
 //     8 elements per thread: two 128-bit loads, one 128-bit store per output.
-//     `which` selects the exponent on the device: 0 -> s0_shift, 1 -> ctl->e1_in, 2 -> ctl->e2_in.
+//     `which` selects the exponent on the device: 0 -> s0_shift, 1, 2, 3 -> ctl->e1_in, e2_in, e3_in.
 //     With diag_half the matrix split is M = S0 - I/2 (residual form, layer_kernel.cuh).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void split_scaled(float x, float scale, __half& hi, __half& lo) {
@@ -279,7 +291,7 @@ __global__ void __launch_bounds__(256) dmpt_split_kernel(const float* __restrict
                                                          __half* __restrict__ hi, __half* __restrict__ lo,
                                                          const DmptCtl* __restrict__ ctl, int which, int s0_shift,
                                                          int diag_half) {
-    const int e = which == 0 ? s0_shift : (which == 1 ? ctl->e1_in : ctl->e2_in);
+    const int e = which == 0 ? s0_shift : (which == 1 ? ctl->e1_in : (which == 2 ? ctl->e2_in : ctl->e3_in));
     const float scale = exp2f((float)e);
     const float diag_shift = diag_half ? 0.5f : 0.f;       // order 0: the operands hold M = S0 - I/2
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < count8;

@@ -61,6 +61,7 @@ constexpr int kBBytes = kBRows * kRowBytes;          // 4 KiB per B-side operand
 template <int PASS> struct PassCfg;
 template <> struct PassCfg<0> { static constexpr int kOps = 4, kStages = 4; };
 template <> struct PassCfg<1> { static constexpr int kOps = 6, kStages = 3; };
+template <> struct PassCfg<2> { static constexpr int kOps = 6, kStages = 3; };
 constexpr int kChunkK = 128;               // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
@@ -78,14 +79,17 @@ constexpr int smem_bytes() {
 
 // operand matrices, in the order of LayerParams::maps / ::h; a stage holds the A tiles of the first kOps of
 // them (rows of panel I), then the B tiles (rows of panel J)
-enum Op : int { MH = 0, ML = 1, S1H = 2, S1L = 3, S2H = 4, S2L = 5 };
+enum Op : int { MH = 0, ML = 1, S1H = 2, S1L = 3, S2H = 4, S2L = 5, S3H = 6, S3L = 7 };
+// positions inside a stage of PASS 1 / PASS 2 (M, then two more operand pairs)
+enum Pos : int { PM_H = 0, PM_L = 1, PY_H = 2, PY_L = 3, PZ_H = 4, PZ_L = 5 };
 
 struct LayerParams {
-    CUtensorMap maps[2][6];     // [buffer][Mhi, Mlo, S1hi, S1lo, S2hi, S2lo], box = kBK x kBRows, SWIZZLE_64B
+    CUtensorMap maps[2][8];     // [buffer][Mhi, Mlo, S1hi, S1lo, S2hi, S2lo, S3hi, S3lo], box = kBK x kBRows, SWIZZLE_64B
     float* s0;                  // fp32 S0, updated in place, ld = n_pad
     float* s1[2];               // fp32 S1, ping-pong
-    float* s2[2];               // fp32 S2, ping-pong (order 2)
-    __half* h[2][6];            // fp16 operand matrices the epilogue writes, same order as maps
+    float* s2[2];               // fp32 response slot 2, ping-pong (order 2: S2; multi-field: S1 of field 2)
+    float* s3[2];               // fp32 response slot 3, ping-pong (multi-field: S1 of field 3)
+    __half* h[2][8];            // fp16 operand matrices the epilogue writes, same order as maps
     const uint32_t* tiles;      // pair tiles (IP | J << 16): block rows 2 IP, 2 IP + 1 x block column J >= 2 IP
     int num_tiles;
     int n_pad;
@@ -94,7 +98,7 @@ struct LayerParams {
     DmptLogs logs;
     DmptProblem pb;
     double* partials;           // [gridDim.x][kNumEpiWarps][RED_COUNT], written by PASS 0
-    double* partials2;          // same shape, written by PASS 1 (RED_FRO2, RED_MAX2)
+    double* partials2;          // same shape, written by PASS 1 / PASS 2 (RED_FRO2, RED_MAX2, RED_FRO3, RED_MAX3)
 };
 
 __device__ __forceinline__ uint32_t pack2(__half a, __half b) {
@@ -250,16 +254,19 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     const int num_pairs = gridDim.x >> 1;
     const int num_chunks = p.n_pad / kChunkK;
     const int num_tiles = idle ? 0 : p.num_tiles;
-    const bool with_p0 = PASS == 1 || c.mode0 != MODE_FROZEN;     // first accumulator in use
-    const bool with_p1 = PASS == 1 || p.pb.order >= 1;            // order 0 (ground state only): no response product
-    const int nops = with_p1 ? kOps : 2;                          // order 0 stages Mhi, Mlo only
+    // accumulator 0 / 1 in use.  PASS 0: P0 until S0 froze / P1 unless order 0 (ground state only).
+    // PASS 2: one accumulator per extra field, until that field's stopping test fired.
+    const bool with_p0 = PASS == 0 ? c.mode0 != MODE_FROZEN : (PASS == 1 || c.conv2 == 0);
+    const bool with_p1 = PASS == 0 ? p.pb.order >= 1 : (PASS == 1 || (p.pb.nfields >= 3 && c.conv3 == 0));
+    const int nops = with_p1 ? kOps : kOps - 2;                   // the last operand pair only feeds accumulator 1
     unsigned int* wave_ctr = PASS == 0 ? &p.ctl->wave : &p.ctl->wave2;
 
     if (warp == 0 && lane == 0) {
         for (int m = 0; m < 2; ++m) {
             prefetch_tensormap(&p.maps[c.s0_buf][m]);
             prefetch_tensormap(&p.maps[c.s1_buf][2 + m]);
-            if (PASS == 1) prefetch_tensormap(&p.maps[c.s2_buf][4 + m]);
+            if (PASS >= 1) prefetch_tensormap(&p.maps[c.s2_buf][S2H + m]);
+            if (PASS == 2) prefetch_tensormap(&p.maps[c.s3_buf][S3H + m]);
         }
         for (int s = 0; s < kStages; ++s) {
             mbar_init(full_bar(s), 1);                       // leader's: its producer's arrive + both CTAs' bytes
@@ -283,8 +290,13 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     if (warp == 0) {
         // =========================== TMA producer (both CTAs) ===========================
         {
-            const CUtensorMap* maps[6] = {&p.maps[c.s0_buf][MH],  &p.maps[c.s0_buf][ML],  &p.maps[c.s1_buf][S1H],
-                                          &p.maps[c.s1_buf][S1L], &p.maps[c.s2_buf][S2H], &p.maps[c.s2_buf][S2L]};
+            // staged operand pairs: PASS 0: M, S1;  PASS 1: M, S1, S2;  PASS 2: M, slot 2, slot 3
+            const CUtensorMap* maps[6] = {
+                &p.maps[c.s0_buf][MH], &p.maps[c.s0_buf][ML],
+                PASS == 2 ? &p.maps[c.s2_buf][S2H] : &p.maps[c.s1_buf][S1H],
+                PASS == 2 ? &p.maps[c.s2_buf][S2L] : &p.maps[c.s1_buf][S1L],
+                PASS == 2 ? &p.maps[c.s3_buf][S3H] : &p.maps[c.s2_buf][S2H],
+                PASS == 2 ? &p.maps[c.s3_buf][S3L] : &p.maps[c.s2_buf][S2L]};
             const int num_kb = p.n_pad / kBK;
             int stage = 0;
             uint32_t phase = 0;
@@ -361,30 +373,30 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                             for (int ks = 0; ks < kBK / 16; ++ks) {
                                 const uint64_t adv = (uint64_t)(ks * 32 >> 4);     // 16 fp16 = 32 bytes along K
                                 const uint32_t accum = (kb | ks) != 0;             // 0: start the chunk from zero
-                                if (PASS == 0) {
-                                    if (with_p0) {
-                                        umma_f16<2>(d0, a[MH] + adv, b[MH] + adv, idesc, accum);     // hi.hi
-                                        umma_f16<2>(d0, a[MH] + adv, b[ML] + adv, idesc, 1);         // hi.lo
-                                        umma_f16<2>(d0, a[ML] + adv, b[MH] + adv, idesc, 1);         // lo.hi
-                                    }
-                                    if (with_p1) {
-                                        umma_f16<2>(d1, a[MH] + adv, b[S1H] + adv, idesc, accum);    // M.S1
-                                        umma_f16<2>(d1, a[S1H] + adv, b[MH] + adv, idesc, 1);        // S1.M
-                                        umma_f16<2>(d1, a[MH] + adv, b[S1L] + adv, idesc, 1);
-                                        umma_f16<2>(d1, a[ML] + adv, b[S1H] + adv, idesc, 1);
-                                        umma_f16<2>(d1, a[S1H] + adv, b[ML] + adv, idesc, 1);
-                                        umma_f16<2>(d1, a[S1L] + adv, b[MH] + adv, idesc, 1);
-                                    }
-                                } else {
-                                    umma_f16<2>(d0, a[S1H] + adv, b[S1H] + adv, idesc, accum);       // S1.S1
-                                    umma_f16<2>(d0, a[S1H] + adv, b[S1L] + adv, idesc, 1);
-                                    umma_f16<2>(d0, a[S1L] + adv, b[S1H] + adv, idesc, 1);
-                                    umma_f16<2>(d1, a[MH] + adv, b[S2H] + adv, idesc, accum);        // M.S2
-                                    umma_f16<2>(d1, a[S2H] + adv, b[MH] + adv, idesc, 1);            // S2.M
-                                    umma_f16<2>(d1, a[MH] + adv, b[S2L] + adv, idesc, 1);
-                                    umma_f16<2>(d1, a[ML] + adv, b[S2H] + adv, idesc, 1);
-                                    umma_f16<2>(d1, a[S2H] + adv, b[ML] + adv, idesc, 1);
-                                    umma_f16<2>(d1, a[S2L] + adv, b[MH] + adv, idesc, 1);
+                                // SQUARE(X): X.X = Xhi.Xhi + Xhi.Xlo + Xlo.Xhi              (Eqs. 14-16)
+                                auto square = [&](uint32_t d, int xh, int xl) {
+                                    umma_f16<2>(d, a[xh] + adv, b[xh] + adv, idesc, accum);
+                                    umma_f16<2>(d, a[xh] + adv, b[xl] + adv, idesc, 1);
+                                    umma_f16<2>(d, a[xl] + adv, b[xh] + adv, idesc, 1);
+                                };
+                                // CROSS(M, Y): M.Y + Y.M, three partial products each        (Eqs. 44-46)
+                                auto cross = [&](uint32_t d, int yh, int yl) {
+                                    umma_f16<2>(d, a[PM_H] + adv, b[yh] + adv, idesc, accum);   // Mhi.Yhi
+                                    umma_f16<2>(d, a[yh] + adv, b[PM_H] + adv, idesc, 1);       // Yhi.Mhi
+                                    umma_f16<2>(d, a[PM_H] + adv, b[yl] + adv, idesc, 1);       // Mhi.Ylo
+                                    umma_f16<2>(d, a[PM_L] + adv, b[yh] + adv, idesc, 1);       // Mlo.Yhi
+                                    umma_f16<2>(d, a[yh] + adv, b[PM_L] + adv, idesc, 1);       // Yhi.Mlo
+                                    umma_f16<2>(d, a[yl] + adv, b[PM_H] + adv, idesc, 1);       // Ylo.Mhi
+                                };
+                                if (PASS == 0) {            // P0 = M.M, P1 = M.S1 + S1.M
+                                    if (with_p0) square(d0, PM_H, PM_L);
+                                    if (with_p1) cross(d1, PY_H, PY_L);
+                                } else if (PASS == 1) {     // Q = S1.S1, P2 = M.S2 + S2.M
+                                    square(d0, PY_H, PY_L);
+                                    cross(d1, PZ_H, PZ_L);
+                                } else {                    // two more first-order fields: M.Y + Y.M, M.Z + Z.M
+                                    if (with_p0) cross(d0, PY_H, PY_L);
+                                    if (with_p1) cross(d1, PZ_H, PZ_L);
                                 }
                             }
                             umma_commit_2sm(empty_bar(stage), 0b11);       // frees the smem stage in both CTAs
@@ -411,6 +423,8 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         const float unscale_q = exp2f(-2.f * (float)c.e1_in);                     // S1.S1 sums
         const float unscale2 = exp2f(-(float)(p.pb.s0_shift + c.e2_in));          // M.S2 + S2.M sums
         const float scale2 = exp2f((float)c.e2_out);
+        const float unscale3 = exp2f(-(float)(p.pb.s0_shift + c.e3_in));          // PASS 2: M.Z + Z.M sums
+        const float scale3 = exp2f((float)c.e3_out);
         const bool upd0 = c.mode0 == MODE_ACTIVE;
         const bool conv0 = c.conv0 != 0;                // FroErr1 wanted (stop layer or frozen)
         EpiOut o0, o1;
@@ -419,14 +433,19 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             o0.hi = p.h[c.s0_buf ^ 1][MH]; o0.lo = p.h[c.s0_buf ^ 1][ML];
             o1.dst = p.s1[c.s1_buf ^ 1]; o1.old = p.s1[c.s1_buf];
             o1.hi = p.h[c.s1_buf ^ 1][S1H]; o1.lo = p.h[c.s1_buf ^ 1][S1L];
-        } else {
+        } else if (PASS == 1) {
             o0.dst = nullptr; o0.old = nullptr; o0.hi = nullptr; o0.lo = nullptr;
             o1.dst = p.s2[c.s2_buf ^ 1]; o1.old = p.s2[c.s2_buf];
             o1.hi = p.h[c.s2_buf ^ 1][S2H]; o1.lo = p.h[c.s2_buf ^ 1][S2L];
+        } else {
+            o0.dst = p.s2[c.s2_buf ^ 1]; o0.old = p.s2[c.s2_buf];
+            o0.hi = p.h[c.s2_buf ^ 1][S2H]; o0.lo = p.h[c.s2_buf ^ 1][S2L];
+            o1.dst = p.s3[c.s3_buf ^ 1]; o1.old = p.s3[c.s3_buf];
+            o1.hi = p.h[c.s3_buf ^ 1][S3H]; o1.lo = p.h[c.s3_buf ^ 1][S3L];
         }
 
         double r_tr = 0.0, r_fs0 = 0.0, r_f0 = 0.0, r_f1 = 0.0, r_dummy = 0.0;
-        float r_mx1 = 0.f, r_mx_dummy = 0.f;
+        float r_mx1 = 0.f, r_mx0 = 0.f, r_mx_dummy = 0.f;
         int acc = 0;
         uint32_t acc_phase = 0;
         for (int t = pair; t < num_tiles; t += num_pairs) {
@@ -481,6 +500,14 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 if (with_p1)
                     final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale1, scale1, conv0, r_dummy,
                                       r_dummy, r_f1, r_mx1);
+            } else if (PASS == 2) {
+                // two more first-order fields, each exactly as P1 of pass 0
+                if (with_p0)
+                    final_epilogue<1>(a0, o0, ld, gr, gc_base, diag, true, sig, unscale2, scale2, conv0, r_dummy,
+                                      r_dummy, r_f0, r_mx0);
+                if (with_p1)
+                    final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale3, scale3, conv0, r_dummy,
+                                      r_dummy, r_f1, r_mx1);
             } else {
                 // V2 = 2^-(a+e2) P2 + 2^-(2 e1) Q: both factors are powers of two, one fp32 rounding per element
 #pragma unroll
@@ -495,16 +522,19 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         r_f0 = warp_sum(r_f0);
         r_f1 = warp_sum(r_f1);
         const double mx1 = warp_max((double)r_mx1);
+        const double mx0 = warp_max((double)r_mx0);
         if (lane == 0) {
             double* out = (PASS == 0 ? p.partials : p.partials2) +
                           ((size_t)blockIdx.x * kNumEpiWarps + (warp - kEpiWarp0)) * RED_COUNT;
             out[RED_TR_S0] = r_tr;
             out[RED_FRO_S0] = r_fs0;
-            out[RED_FRO0] = r_f0;
+            out[RED_FRO0] = PASS == 0 ? r_f0 : 0.0;
             out[RED_FRO1] = PASS == 0 ? r_f1 : 0.0;
             out[RED_MAX1] = PASS == 0 ? mx1 : 0.0;
-            out[RED_FRO2] = PASS == 1 ? r_f1 : 0.0;
-            out[RED_MAX2] = PASS == 1 ? mx1 : 0.0;
+            out[RED_FRO2] = PASS == 1 ? r_f1 : (PASS == 2 ? r_f0 : 0.0);      // slot 2: S2, or field 2
+            out[RED_MAX2] = PASS == 1 ? mx1 : (PASS == 2 ? mx0 : 0.0);
+            out[RED_FRO3] = PASS == 2 ? r_f1 : 0.0;                            // slot 3: field 3
+            out[RED_MAX3] = PASS == 2 ? mx1 : 0.0;
         }
     }
 
@@ -515,7 +545,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         tc_fence_after();
         tmem_dealloc<2>(tmem_base, kTmemCols);
     }
-    if (PASS == 1) return;          // pass 0 of the same layer follows on the stream and takes the decisions
+    if (PASS != 0) return;          // pass 0 of the same layer follows on the stream and takes the decisions
 
     // ---- the last CTA of the launch runs Algorithms 2-3 for this layer
     __shared__ int is_last;
@@ -537,15 +567,16 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             const volatile double* in2 = p.partials2 + (size_t)s * RED_COUNT;
 #pragma unroll
             for (int k = 0; k < RED_COUNT; ++k) {
+                const bool second = p.pb.order == 2 || p.pb.nfields >= 2;       // slots 2, 3 come from the other pass
                 if (k == RED_MAX1) red[k] = fmax(red[k], in[k]);
-                else if (k == RED_MAX2) { if (p.pb.order == 2) red[k] = fmax(red[k], in2[k]); }
-                else if (k == RED_FRO2) { if (p.pb.order == 2) red[k] += in2[k]; }
+                else if (k == RED_MAX2 || k == RED_MAX3) { if (second) red[k] = fmax(red[k], in2[k]); }
+                else if (k == RED_FRO2 || k == RED_FRO3) { if (second) red[k] += in2[k]; }
                 else red[k] += in[k];
             }
         }
 #pragma unroll
         for (int k = 0; k < RED_COUNT; ++k) {
-            if (k == RED_MAX1 || k == RED_MAX2) red[k] = warp_max(red[k]);
+            if (k == RED_MAX1 || k == RED_MAX2 || k == RED_MAX3) red[k] = warp_max(red[k]);
             else red[k] = warp_sum(red[k]);
         }
         if (lane == 0) {

@@ -43,10 +43,10 @@ def test_struct_layout_matches_the_header():
 #include "dmpt.h"
 int main(void) {
     printf("%zu %zu %zu %zu %zu\n", sizeof(dmpt_options), offsetof(dmpt_options, bounds),
-           offsetof(dmpt_options, eps_min), offsetof(dmpt_options, wave_sync), offsetof(dmpt_options, reserved));
+           offsetof(dmpt_options, eps_min), offsetof(dmpt_options, num_fields), offsetof(dmpt_options, reserved));
     printf("%zu %zu %zu %zu %zu %zu %zu\n", sizeof(dmpt_result), offsetof(dmpt_result, launches),
            offsetof(dmpt_result, eps_min), offsetof(dmpt_result, ms_loop), offsetof(dmpt_result, ms_split),
-           offsetof(dmpt_result, sigma), offsetof(dmpt_result, fro_err2));
+           offsetof(dmpt_result, sigma), offsetof(dmpt_result, fro_err3));
     return 0;
 }
 '''
@@ -59,17 +59,18 @@ int main(void) {
     o = [int(x) for x in out[0].split()]
     r = [int(x) for x in out[1].split()]
     assert o == [C.sizeof(DmptOptions), DmptOptions.bounds.offset, DmptOptions.eps_min.offset,
-                 DmptOptions.wave_sync.offset, DmptOptions.reserved.offset]
+                 DmptOptions.num_fields.offset, DmptOptions.reserved.offset]
     assert r == [C.sizeof(_CResult), _CResult.launches.offset, _CResult.eps_min.offset, _CResult.ms_loop.offset,
-                 _CResult.ms_split.offset, _CResult.sigma.offset, _CResult.fro_err2.offset]
+                 _CResult.ms_split.offset, _CResult.sigma.offset, _CResult.fro_err3.offset]
 
 
 def test_host_only_entry_points():
     import paper_2203_09621_b200 as p
 
     o = p.dmpt_default_options()
-    assert (o.max_layers, o.order, o.s0_shift, o.s1_autoscale, o.bounds, o.wave_sync) == (200, 1, -1, 1, 0, 1)
-    assert list(o.reserved) == [0] * 7
+    assert (o.max_layers, o.order, o.s0_shift, o.s1_autoscale, o.bounds, o.wave_sync, o.num_fields) == \
+        (200, 1, -1, 1, 0, 1, 1)
+    assert list(o.reserved) == [0] * 6
     assert p.dmpt_strerror(0) == "ok"
     for code in range(-7, 0):
         assert p.dmpt_strerror(code) not in ("ok", "unknown error code")
@@ -77,11 +78,16 @@ def test_host_only_entry_points():
     # workspace: 3 fp32 + 8 fp16 padded matrices + 2 fp32 staging matrices + scalars
     assert p.dmpt_workspace_bytes(0) == 0 and p.dmpt_workspace_bytes(-5) == 0 and p.dmpt_workspace_bytes(64, 3) == 0
     for n in (1, 100, 256, 2048, 16384):
-        npad = (n + 127) // 128 * 128
+        npad = (n + 255) // 256 * 256            # CTA-pair tiles: 256 rows
         need = 3 * npad * npad * 4 + 8 * npad * npad * 2 + 2 * n * n * 4
         got = p.dmpt_workspace_bytes(n, 1)
         assert need <= got <= need + (4 << 20), (n, need, got)
+        assert p.dmpt_workspace_bytes(n, 0) == got and p.dmpt_workspace_bytes_fields(n, 1) == got
+        # each further field: 2 fp32 + 4 fp16 padded matrices
+        per_field = 2 * npad * npad * 4 + 4 * npad * npad * 2
+        assert p.dmpt_workspace_bytes_fields(n, 3) - got == 2 * per_field
     assert p.dmpt_workspace_bytes(2048, 2) > p.dmpt_workspace_bytes(2048, 1)
+    assert p.dmpt_workspace_bytes_fields(64, 0) == 0 and p.dmpt_workspace_bytes_fields(64, 4) == 0
 
 
 def test_invalid_arguments_are_rejected_before_any_cuda_call():

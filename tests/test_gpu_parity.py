@@ -650,3 +650,62 @@ def test_finite_difference_of_ground_state_runs_gives_the_response(dev, config1)
     fd = (dp - dm) / (2 * h)
     # O(h^2) truncation (third-order response) + 2 x D0 noise / 2h
     assert np.abs(fd - d1).max() <= 3e-3 * np.abs(d1).max(), np.abs(fd - d1).max() / np.abs(d1).max()
+
+
+# ------------------------------------------------------------------------------------------
+# several perturbations sharing H0 in one run (Eq. 79)
+# ------------------------------------------------------------------------------------------
+def _fields_workload(n, nf):
+    """Config-2 style system with the dipole fields along x, y, z (the polarizability workload's shape)."""
+    from workloads import make_config
+
+    wl = make_config(2, n=n)                                   # H1 = diag(x)
+    h1s = [wl.h1]
+    rng = np.random.default_rng(99 + n)
+    for f in range(1, nf):                                     # further diagonal fields of different size
+        h1s.append(np.diag(rng.uniform(-1.0, 1.0, size=n) * 10.0 ** (-2 * f)).astype(np.float32))
+    return wl, h1s
+
+
+@pytest.mark.parametrize("n,nf", [(512, 3), (1284, 2), (332, 3)])
+def test_fields_run_equals_single_field_runs_and_the_oracle(dev, n, nf):
+    from oracle.dnn_sp2_pt import dnn_sp2_pt
+
+    wl, h1s = _fields_workload(n, nf)
+    s = _solver(n, dev, num_fields=nf)
+    s.set_hamiltonian_fields(torch.from_numpy(wl.h0).to(dev), [torch.from_numpy(h).to(dev) for h in h1s], wl.n_occ)
+    res = s.run_fields()
+    assert res.status == 0 and len(res.d1) == nf
+    d0 = res.d0.double().cpu().numpy()
+    stops = [res.layers_d1, res.layers_d2, res.layers_d3][:nf]
+    assert res.layers == max(stops)
+    s.close()
+    for f in range(nf):
+        d1 = res.d1[f].double().cpu().numpy()
+        # bit-identical to the single-field run of (H0, H1_f): same kernels, same products, own stopping test
+        wl.h1 = h1s[f]
+        r1, e0, e1 = _run(wl, dev)
+        assert r1.layers == stops[f] and r1.layers_d0 == res.layers_d0
+        assert np.array_equal(e0, d0) and np.array_equal(e1, d1)
+        ref = dnn_sp2_pt(wl.h0, h1s[f], wl.n_occ)
+        _check_against(ref.d0, ref.d1, wl.n_occ, d0, d1)
+
+
+def test_fields_argument_checks(dev):
+    import paper_2203_09621_b200 as p
+
+    wl, h1s = _fields_workload(256, 2)
+    h0 = torch.from_numpy(wl.h0).to(dev)
+    hs = [torch.from_numpy(h).to(dev) for h in h1s]
+    with pytest.raises(p.DmptError):                 # several fields need a first-order context
+        _solver(256, dev, order=2, num_fields=2)
+    with pytest.raises(p.DmptError):
+        _solver(256, dev, num_fields=4)
+    s = _solver(256, dev, num_fields=2)
+    with pytest.raises(p.DmptError):                 # one perturbation short
+        s.set_hamiltonian_fields(h0, hs[:1], wl.n_occ)
+    s.set_hamiltonian_fields(h0, hs, wl.n_occ)
+    r = s.run(check=False)                           # the single-field call on a multi-field context
+    assert r.status == p.binding.DMPT_EINVAL
+    assert s.run_fields().status == 0
+    s.close()
