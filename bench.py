@@ -181,6 +181,7 @@ def workload_name(args):
 # the CUDA arm
 # ---------------------------------------------------------------------------------------------
 def run_ours(args):
+    import numpy as np
     import torch
     import torch.distributed as dist
 
@@ -206,8 +207,19 @@ def run_ours(args):
     h0 = h0_host.to(dev)
     h1 = h1_host.to(dev)
     order = wl.order
-    solver = Dmpt(n, order=order, device=dev)
-    solver.set_hamiltonian(h0, h1, wl.n_occ)
+    nf = args.fields
+    if nf > 1:
+        # several perturbations sharing H0 (DESIGN.md f2): the config's H1 plus seeded symmetric Gaussians
+        if order != 1:
+            raise SystemExit("--fields needs a first-order config")
+        from workloads.hamiltonians import symmetric_gaussian
+        h1s = [h1] + [torch.from_numpy(symmetric_gaussian(np.random.default_rng(wl.meta["seed"] + 100 * f), n, 0.01)
+                                       .astype(np.float32)).to(dev) for f in range(1, nf)]
+        solver = Dmpt(n, order=1, device=dev, num_fields=nf)
+        solver.set_hamiltonian_fields(h0, h1s, wl.n_occ)
+    else:
+        solver = Dmpt(n, order=order, device=dev)
+        solver.set_hamiltonian(h0, h1, wl.n_occ)
     d0 = torch.empty((n, n), dtype=torch.float32, device=dev)
     d1 = torch.empty((n, n), dtype=torch.float32, device=dev)
     d0_host = torch.empty((n, n), dtype=torch.float32).pin_memory()
@@ -227,8 +239,24 @@ def run_ours(args):
     def sum_over_ranks(x):
         return replicas.sum_over_ranks(x, dev)
 
+    def one_run():
+        """(result, paper-convention FMA, tensor FMA needed) of one step."""
+        if nf == 1:
+            r = solver.run(out=outs)
+            return (r, flops_paper(n, r.layers, r.layers_d0, order, r.layers_d1),
+                    fma_executed(solver_n_pad(n), r.layers, r.layers_d0, order, r.layers_d1))
+        r = solver.run_fields()
+        stops = [r.layers_d1, r.layers_d2, r.layers_d3][:nf]
+        # paper convention: every field as a run of its own (S0^2 counted per field, PAPER.md:558)
+        fl = sum(flops_paper(n, st, r.layers_d0) for st in stops)
+        fx = sum(fma_executed(solver_n_pad(n), st, r.layers_d0) for st in stops)
+        la = r.layers_d0 if r.layers_d0 > 0 else r.layers
+        nb = solver_n_pad(n) // 128
+        fx -= (nf - 1) * (nb * (nb + 1) // 2) * 128.0 * 128.0 * solver_n_pad(n) * 3.0 * la     # S0^2 is formed once
+        return r, fl, fx
+
     for _ in range(args.warmup):
-        res = solver.run(out=outs)
+        res = one_run()[0]
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
@@ -239,9 +267,9 @@ def run_ours(args):
     flops = fma = ms_loop = 0.0
     launches = layers_total = 0
     for _ in range(args.steps):
-        res = solver.run(out=outs)
-        flops += flops_paper(n, res.layers, res.layers_d0, order, res.layers_d1)
-        fma += fma_executed(solver_n_pad(n), res.layers, res.layers_d0, order, res.layers_d1)
+        res, fl, fx = one_run()
+        flops += fl
+        fma += fx
         ms_loop += res.ms_loop
         launches += res.launches
         layers_total += res.layers
@@ -253,18 +281,21 @@ def run_ours(args):
     value = total_flops / (ms * 1e-3) / 1e12
 
     # ---- end-to-end arm: host buffers through dmpt_run_host, copies inside the timed region
-    for _ in range(1):
-        solver.run_host(h0_host, h1_host, wl.n_occ, out=outs_host)
-    barrier()
-    ev0.record()
-    e2e_flops = 0.0
-    for _ in range(args.steps):
-        r2 = solver.run_host(h0_host, h1_host, wl.n_occ, out=outs_host)
-        e2e_flops += flops_paper(n, r2.layers, r2.layers_d0, order, r2.layers_d1)
-    ev1.record()
-    barrier()
-    ms_e2e = max_over_ranks(ev0.elapsed_time(ev1))
-    e2e_value = sum_over_ranks(e2e_flops) / (ms_e2e * 1e-3) / 1e12
+    # (the multi-field entry points take device matrices only: no end-to-end number with --fields > 1)
+    ms_e2e = e2e_value = None
+    if nf == 1:
+        for _ in range(1):
+            solver.run_host(h0_host, h1_host, wl.n_occ, out=outs_host)
+        barrier()
+        ev0.record()
+        e2e_flops = 0.0
+        for _ in range(args.steps):
+            r2 = solver.run_host(h0_host, h1_host, wl.n_occ, out=outs_host)
+            e2e_flops += flops_paper(n, r2.layers, r2.layers_d0, order, r2.layers_d1)
+        ev1.record()
+        barrier()
+        ms_e2e = max_over_ranks(ev0.elapsed_time(ev1))
+        e2e_value = sum_over_ranks(e2e_flops) / (ms_e2e * 1e-3) / 1e12
 
     if rank == 0:
         peaks, peaks_kind = load_peaks()
@@ -277,7 +308,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f16 x f16 -> f32 (dual-half), f64 scalars",
             "data": "synthetic", "gpu_launches": launches,
-            "config": {"workload": workload_name(args), "n": n, "n_occ": wl.n_occ, "order": order,
+            "config": {"workload": workload_name(args), "n": n, "n_occ": wl.n_occ, "order": order, "fields": nf,
                        "layers": res.layers, "layers_d0": res.layers_d0, "gap": wl.meta.get("gap"),
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": f"inputs larger than L2 ({n * n * 4 / 2**30:.2f} GiB per matrix); no flush needed",
@@ -286,8 +317,9 @@ def run_ours(args):
                        "frac_nominal_fp16_peak_fma1": value / NOMINAL_FP16_TFMA,
                        "paper_context": "~120 Tflops (FMA=1) on one A100, N=19008 (PAPER.md:546); another machine"},
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
-                    "h2d_bytes_per_step": 2 * n * n * 4, "d2h_bytes_per_step": n_out * n * n * 4},
+            "e2e": ({"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
+                     "h2d_bytes_per_step": 2 * n * n * 4, "d2h_bytes_per_step": n_out * n * n * 4}
+                    if nf == 1 else None),
             "roofline": {"bound": "tensor", "kernel": "dmpt_layer_kernel", "achieved": achieved_tf, "peak": peak_tf,
                          "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": args.traffic,
                          "peak_kind": f"bf16_tflops_sustained, {peaks_kind} (fp16 = bf16 rate), 2 flops per FMA",
@@ -323,12 +355,14 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override the matrix size (default: the config's)")
     ap.add_argument("--ref-n", type=int, default=4096, help="size of the oracle's bounded sample")
     ap.add_argument("--ref-layers", type=int, default=20)
+    ap.add_argument("--fields", type=int, default=1,
+                    help="perturbations sharing H0 in one run (1..3); value then counts every field as a run of its own")
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per layer launch from ncu (profiles/)")
     args = ap.parse_args()
     if args.n is None:
         from workloads import CONFIGS
         args.n = CONFIGS[args.config]["n"]
-    if args.traffic is None and args.config == 4:
+    if args.traffic is None and args.config == 4 and args.fields == 1:
         args.traffic = NCU_TRAFFIC_BYTES.get(args.n)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warmup raised to 3 (timing rules)", file=sys.stderr)
