@@ -132,7 +132,9 @@ int dmpt_set_hamiltonian_fields(dmpt_ctx *ctx, const float *d_h0, const float *c
 int dmpt_run_fields(dmpt_ctx *ctx, float *d_d0, float *const *d_d1, int ld, dmpt_result *res);
 
 /* The same call with HOST matrices (pinned memory recommended): copies H0, H1 to the device, runs,
- * and copies D0, D1 (D2) back, all on the context's stream.  ms_total then covers the copies too. */
+ * and copies D0, D1 (D2) back.  ms_total then covers the copies too.  D0 is final as soon as Algorithm 2
+ * fired, a few layers before the end: its read-back then starts on an internal copy stream and overlaps
+ * the remaining layers (h_d0 must not be touched until the call returns, as for every output). */
 int dmpt_run_host(dmpt_ctx *ctx, const float *h_h0, const float *h_h1, int ld_in, int n_occ,
                   float *h_d0, float *h_d1, float *h_d2, int ld_out, dmpt_result *res);
 

@@ -134,7 +134,10 @@ struct dmpt_ctx {
     LayerParams lp{};
     cudaEvent_t ev[kNumEvents]{};
     cudaEvent_t ev_t[6]{};       // 0 start, 1 loop start, 2 loop end, 3 end, 4 after bounds, 5 after transform
-    int* h_flags = nullptr;      // pinned
+    int* h_flags = nullptr;      // pinned: ctl.done after every chunk of launches
+    int* h_flags0 = nullptr;     // pinned: ctl.conv0 after every chunk (dmpt_run_host: early copy of D0)
+    cudaStream_t side = nullptr; // copy stream of dmpt_run_host's early D0 read-back
+    cudaEvent_t ev_side = nullptr;
     DmptCtl* h_ctl = nullptr;    // pinned
     char err[256] = {0};
 
@@ -249,7 +252,10 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
         for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
         for (auto& e : ctx->ev_t) if (e) cudaEventDestroy(e);
         if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
+        if (ctx->h_flags0) cudaFreeHost(ctx->h_flags0);
         if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
+        if (ctx->side) cudaStreamDestroy(ctx->side);
+        if (ctx->ev_side) cudaEventDestroy(ctx->ev_side);
         delete ctx;
         return code;
     };
@@ -273,6 +279,9 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     for (auto& e : ctx->ev) CKC(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     for (auto& e : ctx->ev_t) CKC(cudaEventCreate(&e));
     CKC(cudaHostAlloc(&ctx->h_flags, kFlagSlots * sizeof(int), cudaHostAllocDefault));
+    CKC(cudaHostAlloc(&ctx->h_flags0, kFlagSlots * sizeof(int), cudaHostAllocDefault));
+    CKC(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
+    CKC(cudaEventCreateWithFlags(&ctx->ev_side, cudaEventDisableTiming));
     CKC(cudaHostAlloc(&ctx->h_ctl, sizeof(DmptCtl), cudaHostAllocDefault));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<0>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<1>()));
@@ -348,7 +357,10 @@ extern "C" int dmpt_destroy(dmpt_ctx* ctx) {
     for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
     for (auto& e : ctx->ev_t) if (e) cudaEventDestroy(e);
     if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
+    if (ctx->h_flags0) cudaFreeHost(ctx->h_flags0);
     if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
+    if (ctx->side) cudaStreamDestroy(ctx->side);
+    if (ctx->ev_side) cudaEventDestroy(ctx->ev_side);
     delete ctx;
     return DMPT_OK;
 }
@@ -418,7 +430,11 @@ static int elementwise_grid(const dmpt_ctx* ctx, long long work_items, int threa
 }
 
 // Everything from the spectral bounds to the last layer; leaves the result in the workspace.
-static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld, int* launches) {
+// `h_d0_early` (dmpt_run_host only): S0 is final once Algorithm 2 fired, two to four layers before the run
+// ends, so its read-back to the host is started on a side stream as soon as the host sees ctl.conv0 and
+// overlaps the remaining layers.  *early_issued tells the caller whether that happened.
+static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld, int* launches,
+                    float* h_d0_early = nullptr, int ld_early = 0, bool* early_issued = nullptr) {
     const Layout& L = ctx->L;
     const int n = ctx->n, np = L.n_pad;
     cudaStream_t st = ctx->stream;
@@ -492,6 +508,8 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
             if (rc) return rc;
         }
         CK(cudaMemcpyAsync(&ctx->h_flags[chunks % kFlagSlots], &ctl->done, sizeof(int), cudaMemcpyDeviceToHost, st));
+        if (h_d0_early)
+            CK(cudaMemcpyAsync(&ctx->h_flags0[chunks % kFlagSlots], &ctl->conv0, sizeof(int), cudaMemcpyDeviceToHost, st));
         CK(cudaEventRecord(ctx->ev[chunks % kNumEvents], st));
         ++chunks;
         return DMPT_OK;
@@ -501,6 +519,13 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     if (launched < max_layers && (rc = launch_chunk())) return rc;
     for (int w = 0; w < chunks; ++w) {
         CK(cudaEventSynchronize(ctx->ev[w % kNumEvents]));
+        if (h_d0_early && !*early_issued && ctx->h_flags0[w % kFlagSlots] && !ctx->h_flags[w % kFlagSlots]) {
+            // the launch that set conv0 has completed: S0 will not change any more
+            CK(cudaMemcpy2DAsync(h_d0_early, (size_t)ld_early * 4, ctx->lp.s0, (size_t)np * 4, (size_t)n * 4, n,
+                                 cudaMemcpyDeviceToHost, ctx->side));
+            CK(cudaEventRecord(ctx->ev_side, ctx->side));
+            *early_issued = true;
+        }
         if (ctx->h_flags[w % kFlagSlots]) break;
         if (launched < max_layers && (rc = launch_chunk())) return rc;
     }
@@ -626,10 +651,14 @@ extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1
     CK(cudaMemcpy2DAsync(s_h0, n * 4, h_h0, (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, ctx->stream));
     if (ctx->opt.order >= 1)
         CK(cudaMemcpy2DAsync(s_h1, n * 4, h_h1, (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, ctx->stream));
-    int rc = run_core(ctx, s_h0, ctx->opt.order >= 1 ? s_h1 : nullptr, (int)n, &launches);
+    bool early = false;
+    int rc = run_core(ctx, s_h0, ctx->opt.order >= 1 ? s_h1 : nullptr, (int)n, &launches, h_d0, ld_out, &early);
     if (rc) return rc;
     if ((rc = fetch_ctl(ctx))) return rc;
-    CK(cudaMemcpy2DAsync(h_d0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToHost, ctx->stream));
+    if (early)
+        CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_side, 0));       // D0 went out while the last layers ran
+    else
+        CK(cudaMemcpy2DAsync(h_d0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToHost, ctx->stream));
     if (ctx->opt.order >= 1)
         CK(cudaMemcpy2DAsync(h_d1, (size_t)ld_out * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
                              cudaMemcpyDeviceToHost, ctx->stream));
