@@ -461,10 +461,10 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     CK(cudaEventRecord(ctx->ev_t[5], st));
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
     CK(cudaGetLastError());
     if (ctx->opt.order >= 1) {      // order 0 (ground state only) has no response operands
-        dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
+        dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
         CK(cudaGetLastError());
         ++*launches;
     }
@@ -490,7 +490,7 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
         CK(cudaGetLastError());
         dmpt_field_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, tgrid, f + 1);
         CK(cudaGetLastError());
-        dmpt_split_kernel<<<sgrid, 256, 0, st>>>(dst, c8, (int)np, ctx->lp.h[0][2 + 2 * f], ctx->lp.h[0][3 + 2 * f], ctl,
+        dmpt_split_kernel<<<sgrid, 256, 0, st>>>(dst, (int)np, ctx->lp.h[0][2 + 2 * f], ctx->lp.h[0][3 + 2 * f], ctl,
                                                  f + 1, ctx->s0_shift, 0);
         CK(cudaGetLastError());
         *launches += 3;
@@ -711,9 +711,9 @@ extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
     CK(cudaGetLastError());
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
     CK(cudaGetLastError());
     int rc = launch_pass<0>(ctx);
     if (rc) return rc;
@@ -744,11 +744,11 @@ extern "C" int dmpt_layer_products2(dmpt_ctx* ctx, const float* d_s0, const floa
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
     CK(cudaGetLastError());
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], c8, (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
     CK(cudaGetLastError());
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s2[0], c8, (int)np, ctx->lp.h[0][4], ctx->lp.h[0][5], ctl, 2, ctx->s0_shift, 0);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s2[0], (int)np, ctx->lp.h[0][4], ctx->lp.h[0][5], ctl, 2, ctx->s0_shift, 0);
     CK(cudaGetLastError());
     int rc = launch_pass<1>(ctx);
     if (rc) return rc;
@@ -825,7 +825,7 @@ extern "C" int dmpt_split(dmpt_ctx* ctx, const float* d_x, int ld, int shift, in
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, c8, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, shift,
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, shift,
                                              diag_half ? 1 : 0);
     CK(cudaGetLastError());
     CK(cudaMemcpy2DAsync(d_hi, (size_t)ld_out * 2, ctx->lp.h[0][0], np * 2, n * 2, n, cudaMemcpyDeviceToDevice, st));

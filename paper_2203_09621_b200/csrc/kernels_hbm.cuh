@@ -287,27 +287,29 @@ __device__ __forceinline__ void split_scaled(float x, float scale, __half& hi, _
     lo = __float2half_rn(t - __half2float(hi));
 }
 
-__global__ void __launch_bounds__(256) dmpt_split_kernel(const float* __restrict__ x, long long count8, int n_pad,
+__global__ void __launch_bounds__(256) dmpt_split_kernel(const float* __restrict__ x, int n_pad,
                                                          __half* __restrict__ hi, __half* __restrict__ lo,
                                                          const DmptCtl* __restrict__ ctl, int which, int s0_shift,
                                                          int diag_half) {
     const int e = which == 0 ? s0_shift : (which == 1 ? ctl->e1_in : (which == 2 ? ctl->e2_in : ctl->e3_in));
     const float scale = exp2f((float)e);
     const float diag_shift = diag_half ? 0.5f : 0.f;       // order 0: the operands hold M = S0 - I/2
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < count8;
-         i += (long long)gridDim.x * blockDim.x) {
-        const float4 v0 = ldg_stream4(x + i * 8);
-        const float4 v1 = ldg_stream4(x + i * 8 + 4);
-        float v[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
-        const long long e0 = i * 8;
-        const int row = (int)(e0 / n_pad), col = (int)(e0 - (long long)row * n_pad);
-        __align__(16) __half h[8];
-        __align__(16) __half l[8];
+    const int c8_per_row = n_pad >> 3;
+    // block per row (grid-stride), threads along the row: no 64-bit division per element
+    for (int row = blockIdx.x; row < n_pad; row += gridDim.x)
+        for (int c8 = threadIdx.x; c8 < c8_per_row; c8 += blockDim.x) {
+            const int col = c8 << 3;
+            const size_t i8 = (size_t)row * n_pad + col;
+            const float4 v0 = ldg_stream4(x + i8);
+            const float4 v1 = ldg_stream4(x + i8 + 4);
+            float v[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+            __align__(16) __half h[8];
+            __align__(16) __half l[8];
 #pragma unroll
-        for (int t = 0; t < 8; ++t) split_scaled(col + t == row ? v[t] - diag_shift : v[t], scale, h[t], l[t]);
-        *reinterpret_cast<uint4*>(hi + i * 8) = *reinterpret_cast<const uint4*>(h);
-        *reinterpret_cast<uint4*>(lo + i * 8) = *reinterpret_cast<const uint4*>(l);
-    }
+            for (int t = 0; t < 8; ++t) split_scaled(col + t == row ? v[t] - diag_shift : v[t], scale, h[t], l[t]);
+            *reinterpret_cast<uint4*>(hi + i8) = *reinterpret_cast<const uint4*>(h);
+            *reinterpret_cast<uint4*>(lo + i8) = *reinterpret_cast<const uint4*>(l);
+        }
 }
 
 }  // namespace dmpt
