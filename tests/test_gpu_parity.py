@@ -709,3 +709,32 @@ def test_fields_argument_checks(dev):
     assert r.status == p.binding.DMPT_EINVAL
     assert s.run_fields().status == 0
     s.close()
+
+
+# ------------------------------------------------------------------------------------------
+# bench.py contract (small configuration; the timed workload of record is config 4)
+# ------------------------------------------------------------------------------------------
+def test_bench_line_has_the_contract_keys(dev):
+    import json
+    import os
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--config", "1", "--steps", "2", "--warmup", "3",
+                        "--ref-n", "128", "--ref-layers", "3"], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert k in d, k
+    assert d["n_gpus"] == 1 and d["steps"] == 2 and d["warmup"] == 3 and d["value"] > 0 and d["vs_baseline"] is None
+    assert d["gpu_launches"] > 0 and d["data"] == "synthetic" and "workload" in d["config"]
+    rf = d["roofline"]
+    assert rf["bound"] == "tensor" and rf["unit"] == "TFLOP/s" and abs(rf["frac"] - rf["achieved"] / rf["peak"]) < 1e-9
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 2 * 256 * 256 * 4 and e["d2h_bytes_per_step"] == 2 * 256 * 256 * 4
+    cb = d["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] > 0 and "sample" in cb
