@@ -152,6 +152,14 @@ int dmpt_layer_products(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, int
 int dmpt_layer_products2(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, const float *d_s2, int ld,
                          float *d_x2, int ld_out);
 
+/* A general product in the dual half-precision representation, on its own (the
+ * congruence transforms either side of the hot path, H_orth = Z^T H Z and D = Z D_orth Z^T, PAPER.md:74-79,
+ * A18, are two of these each): C = A.B^T = A_hi.B_hi^T + A_hi.B_lo^T + A_lo.B_hi^T for ANY n x n device
+ * matrices A, B (fp32, leading dimension ld), fp32 accumulation promoted every 128 columns like the layer
+ * products; each operand is split after its own power-of-two scale (max|.| into [8, 16)).  Contexts of
+ * order >= 1.  C may not alias A or B. */
+int dmpt_product_nt(dmpt_ctx *ctx, const float *d_a, const float *d_b, int ld, float *d_c, int ld_out);
+
 /* The three HBM-bound steps on their own (tests and micro-benchmarks; dmpt_run does not call these
  * entry points but launches the same kernels).  All run on the context's stream and return after it
  * drained.  Matrices are n x n (n of dmpt_create), row-major, leading dimensions in elements.

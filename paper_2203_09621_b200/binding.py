@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = (
     "dmpt_default_options", "dmpt_workspace_bytes", "dmpt_create", "dmpt_set_hamiltonian",
     "dmpt_run", "dmpt_run_host", "dmpt_layer_products", "dmpt_destroy", "dmpt_strerror",
     "dmpt_last_cuda_error", "dmpt_spectral_bounds", "dmpt_initial_transform", "dmpt_split",
-    "dmpt_layer_products2", "dmpt_workspace_bytes_fields", "dmpt_set_hamiltonian_fields", "dmpt_run_fields",
+    "dmpt_layer_products2", "dmpt_product_nt", "dmpt_workspace_bytes_fields", "dmpt_set_hamiltonian_fields", "dmpt_run_fields",
 )
 
 DMPT_OK, DMPT_EINVAL, DMPT_ESTATE, DMPT_ECUDA = 0, -1, -2, -3
@@ -92,6 +92,8 @@ def lib():
         L.dmpt_layer_products2.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
                                            C.c_int]
         L.dmpt_layer_products2.restype = C.c_int
+        L.dmpt_product_nt.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int]
+        L.dmpt_product_nt.restype = C.c_int
         L.dmpt_spectral_bounds.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double),
                                            C.POINTER(C.c_double)]
         L.dmpt_spectral_bounds.restype = C.c_int
@@ -179,6 +181,10 @@ def dmpt_layer_products(ctx, s0_ptr, s1_ptr, ld, x0_ptr, x1_ptr, ld_out) -> int:
 def dmpt_layer_products2(ctx, s0_ptr, s1_ptr, s2_ptr, ld, x2_ptr, ld_out) -> int:
     return int(lib().dmpt_layer_products2(ctx, C.c_void_p(s0_ptr), C.c_void_p(s1_ptr), C.c_void_p(s2_ptr), int(ld),
                                           C.c_void_p(x2_ptr), int(ld_out)))
+
+
+def dmpt_product_nt(ctx, a_ptr, b_ptr, ld, c_ptr, ld_out) -> int:
+    return int(lib().dmpt_product_nt(ctx, C.c_void_p(a_ptr), C.c_void_p(b_ptr), int(ld), C.c_void_p(c_ptr), int(ld_out)))
 
 
 def dmpt_spectral_bounds(ctx, h0_ptr, ld):
@@ -387,6 +393,22 @@ class Dmpt:
         if rc != DMPT_OK:
             raise DmptError(rc, "dmpt_layer_products2", dmpt_last_cuda_error(self.ctx))
         return x2
+
+    def product_nt(self, a, b):
+        """C = a @ b.T in the dual half-precision representation (general matrices)."""
+        t = self.torch
+        c = t.empty((self.n, self.n), dtype=t.float32, device=self.device)
+        if a.stride(0) != b.stride(0):
+            raise DmptError(DMPT_EINVAL, "product_nt", "a and b need the same leading dimension")
+        rc = dmpt_product_nt(self.ctx, a.data_ptr(), b.data_ptr(), a.stride(0), c.data_ptr(), self.n)
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_product_nt", dmpt_last_cuda_error(self.ctx))
+        return c
+
+    def congruence(self, z, h):
+        """Z^T H Z for symmetric h: T = Z^T H = (Z^T).(H)^T, then T.Z = T.(Z^T)^T."""
+        zt = z.t().contiguous()
+        return self.product_nt(self.product_nt(zt, h), zt)
 
     def spectral_bounds(self, h0):
         rc, lo, hi = dmpt_spectral_bounds(self.ctx, h0.data_ptr(), h0.stride(0))

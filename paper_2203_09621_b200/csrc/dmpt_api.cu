@@ -37,7 +37,7 @@ struct Carve {
 
 struct Layout {
     int n, n_pad, order, nfields, num_tiles;
-    size_t ctl, bounds, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, fro3, partials, partials2, tiles;
+    size_t ctl, bounds, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, fro3, partials, partials2, tiles, tiles_full;
     size_t s0, s1[2], s2[2], s3[2];
     size_t h[2][8];          // [buffer][S0hi, S0lo, S1hi, S1lo, slot-2 hi, lo, slot-3 hi, lo]
     size_t stage_h0, stage_h1;
@@ -77,6 +77,7 @@ Layout make_layout(int n, int order, int nfields) {
     L.partials = c.take(kPartialDoubles * sizeof(double));
     L.partials2 = c.take(kPartialDoubles * sizeof(double));
     L.tiles = c.take((size_t)L.num_tiles * sizeof(uint32_t));
+    L.tiles_full = c.take((size_t)(nb / 2) * nb * sizeof(uint32_t));
     L.s0 = c.take(np2 * 4);
     L.s1[0] = c.take(np2 * 4);
     L.s1[1] = c.take(np2 * 4);
@@ -108,6 +109,19 @@ std::vector<uint32_t> make_tile_order(int nb, int band) {
         const int b1 = b0 + band < nbp ? b0 + band : nbp;
         for (int j = 2 * b0; j < nb; ++j)
             for (int ip = b0; ip < b1 && 2 * ip <= j; ++ip) t.push_back((uint32_t)ip | ((uint32_t)j << 16));
+    }
+    return t;
+}
+
+// Every pair tile (IP, J), same band order: the general product C = A.B^T has no symmetry to exploit.
+std::vector<uint32_t> make_tile_order_full(int nb, int band) {
+    std::vector<uint32_t> t;
+    const int nbp = nb / 2;
+    t.reserve((size_t)nbp * nb);
+    for (int b0 = 0; b0 < nbp; b0 += band) {
+        const int b1 = b0 + band < nbp ? b0 + band : nbp;
+        for (int j = 0; j < nb; ++j)
+            for (int ip = b0; ip < b1; ++ip) t.push_back((uint32_t)ip | ((uint32_t)j << 16));
     }
     return t;
 }
@@ -286,6 +300,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<0>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<1>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<2>()));
+    CKC(cudaFuncSetAttribute(dmpt_layer_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<3>()));
 
     const Layout& L = ctx->L;
     const int nb = L.n_pad / kTile;
@@ -294,6 +309,9 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     band = band / 2 > 0 ? band / 2 : 1;                          // ... in pair rows
     std::vector<uint32_t> tiles = make_tile_order(nb, band);
     CKC(cudaMemcpyAsync(ctx->at<void>(L.tiles), tiles.data(), tiles.size() * sizeof(uint32_t),
+                        cudaMemcpyHostToDevice, ctx->stream));
+    std::vector<uint32_t> tiles_full = make_tile_order_full(nb, band);
+    CKC(cudaMemcpyAsync(ctx->at<void>(L.tiles_full), tiles_full.data(), tiles_full.size() * sizeof(uint32_t),
                         cudaMemcpyHostToDevice, ctx->stream));
     CKC(cudaStreamSynchronize(ctx->stream));
     // one CTA pair (cluster of 2, one TPC) per pair tile in flight
@@ -325,6 +343,8 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     }
     lp.tiles = ctx->at<uint32_t>(L.tiles);
     lp.num_tiles = L.num_tiles;
+    lp.tiles_full = ctx->at<uint32_t>(L.tiles_full);
+    lp.num_tiles_full = (nb / 2) * nb;
     lp.n_pad = L.n_pad;
     lp.wave_sync = (o.wave_sync && L.num_tiles > ctx->grid_layer / 2) ? 1 : 0;
     lp.ctl = ctx->at<DmptCtl>(L.ctl);
@@ -753,6 +773,40 @@ extern "C" int dmpt_layer_products2(dmpt_ctx* ctx, const float* d_s0, const floa
     int rc = launch_pass<1>(ctx);
     if (rc) return rc;
     CK(cudaMemcpy2DAsync(d_x2, (size_t)ld_out * 4, ctx->lp.s2[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    return DMPT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// dmpt_product_nt: C = A.B^T for general n x n matrices in the dual half-precision representation
+// (the congruence transforms either side of the hot path are two of these)
+// ---------------------------------------------------------------------------------------------
+extern "C" int dmpt_product_nt(dmpt_ctx* ctx, const float* d_a, const float* d_b, int ld, float* d_c, int ld_out) {
+    if (!ctx || !d_a || !d_b || !d_c) return DMPT_EINVAL;
+    if (ld < ctx->n || ld_out < ctx->n || ctx->opt.order < 1) return DMPT_EINVAL;      // needs the S1 buffers
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    double* partials = ctx->at<double>(L.partials);
+    double* partials2 = ctx->at<double>(L.partials2);
+    const int grid = elementwise_grid(ctx, (long long)np * np, 256);
+    // A -> the S0 buffers (operand pair 0, scale 2^e2), B -> the S1 buffers (operand pair 1, scale 2^e1)
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_a, (int)n, ld, (int)np, ctx->lp.s0, partials2);
+    CK(cudaGetLastError());
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_b, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
+    CK(cudaGetLastError());
+    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, partials2, grid);
+    CK(cudaGetLastError());
+    const long long c8 = (long long)np * np / 8;
+    const int sgrid = elementwise_grid(ctx, c8, 256);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 2, ctx->s0_shift, 0);
+    CK(cudaGetLastError());
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
+    CK(cudaGetLastError());
+    int rc = launch_pass<3>(ctx);
+    if (rc) return rc;
+    CK(cudaMemcpy2DAsync(d_c, (size_t)ld_out * 4, ctx->lp.s1[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaStreamSynchronize(st));
     return DMPT_OK;
 }

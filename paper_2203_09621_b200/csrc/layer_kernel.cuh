@@ -62,6 +62,9 @@ template <int PASS> struct PassCfg;
 template <> struct PassCfg<0> { static constexpr int kOps = 4, kStages = 4; };
 template <> struct PassCfg<1> { static constexpr int kOps = 6, kStages = 3; };
 template <> struct PassCfg<2> { static constexpr int kOps = 6, kStages = 3; };
+// PASS 3: a general product C = A.B^T on its own (A, B any n x n matrices; the congruence
+// transforms Z^T H Z, Z D Z^T are two of these): the A side stages A hi/lo only, the B side B hi/lo only
+template <> struct PassCfg<3> { static constexpr int kOps = 4, kStages = 4; };
 constexpr int kChunkK = 128;               // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
@@ -92,6 +95,8 @@ struct LayerParams {
     __half* h[2][8];            // fp16 operand matrices the epilogue writes, same order as maps
     const uint32_t* tiles;      // pair tiles (IP | J << 16): block rows 2 IP, 2 IP + 1 x block column J >= 2 IP
     int num_tiles;
+    const uint32_t* tiles_full; // PASS 3: every (IP, J), the output is not symmetric
+    int num_tiles_full;
     int n_pad;
     int wave_sync;              // 1: producers of all CTAs re-align at every tile boundary (L2 reuse)
     DmptCtl* ctl;
@@ -253,12 +258,15 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     const int pair = blockIdx.x >> 1;
     const int num_pairs = gridDim.x >> 1;
     const int num_chunks = p.n_pad / kChunkK;
-    const int num_tiles = idle ? 0 : p.num_tiles;
+    const int num_tiles = PASS == 3 ? p.num_tiles_full : (idle ? 0 : p.num_tiles);
+    const uint32_t* tile_list = PASS == 3 ? p.tiles_full : p.tiles;
     // accumulator 0 / 1 in use.  PASS 0: P0 until S0 froze / P1 unless order 0 (ground state only).
     // PASS 2: one accumulator per extra field, until that field's stopping test fired.
-    const bool with_p0 = PASS == 0 ? c.mode0 != MODE_FROZEN : (PASS == 1 || c.conv2 == 0);
-    const bool with_p1 = PASS == 0 ? p.pb.order >= 1 : (PASS == 1 || (p.pb.nfields >= 3 && c.conv3 == 0));
-    const int nops = with_p1 ? kOps : kOps - 2;                   // the last operand pair only feeds accumulator 1
+    // PASS 3: accumulator 0 only, fed by A hi/lo (positions 0, 1, A side) and B hi/lo (positions 2, 3, B side).
+    const bool with_p0 = PASS == 3 ? true : (PASS == 0 ? c.mode0 != MODE_FROZEN : (PASS == 1 || c.conv2 == 0));
+    const bool with_p1 = PASS == 3 ? false
+                                   : (PASS == 0 ? p.pb.order >= 1 : (PASS == 1 || (p.pb.nfields >= 3 && c.conv3 == 0)));
+    const int nops = (with_p1 || PASS == 3) ? kOps : kOps - 2;    // the last operand pair only feeds accumulator 1
     unsigned int* wave_ctr = PASS == 0 ? &p.ctl->wave : &p.ctl->wave2;
 
     if (warp == 0 && lane == 0) {
@@ -318,7 +326,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                     }
                     __syncwarp();
                 }
-                const uint32_t tl = p.tiles[t];
+                const uint32_t tl = tile_list[t];
                 const int row_a = (2 * (int)(tl & 0xFFFF) + (int)rank) * kTile;
                 const int row_b = (int)(tl >> 16) * kTile + (int)rank * kBRows;
                 for (int kb = 0; kb < num_kb; ++kb) {
@@ -326,15 +334,17 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                     const uint32_t fb = full_bar(stage);      // completion is counted on the LEADER's barrier
                     const uint32_t base = smem_base + stage * kStageBytes;
                     if (elect_one()) {
-                        if (rank == 0) mbar_arrive_expect_tx(fb, 2 * nops * (kABytes + kBBytes));
+                        if (rank == 0)
+                            mbar_arrive_expect_tx(fb, PASS == 3 ? 2 * 2 * (kABytes + kBBytes) : 2 * nops * (kABytes + kBBytes));
                         const int k0 = kb * kBK;
 #pragma unroll
                         for (int o = 0; o < kOps; ++o) {
-                            if (o < nops) {
+                            if (o < nops && !(PASS == 3 && o >= 2)) {        // A side (PASS 3: A hi/lo only)
                                 tma_load_2d_2sm(base + o * kABytes, maps[o], fb, k0, row_a);
                                 tma_load_2d_2sm(base + o * kABytes + kBBytes, maps[o], fb, k0, row_a + kBRows);
-                                tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[o], fb, k0, row_b);
                             }
+                            if (o < nops && !(PASS == 3 && o < 2))           // B side (PASS 3: B hi/lo only)
+                                tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[o], fb, k0, row_b);
                         }
                     }
                     __syncwarp();
@@ -391,6 +401,10 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                                 if (PASS == 0) {            // P0 = M.M, P1 = M.S1 + S1.M
                                     if (with_p0) square(d0, PM_H, PM_L);
                                     if (with_p1) cross(d1, PY_H, PY_L);
+                                } else if (PASS == 3) {     // C = A.B^T: Ahi.Bhi + Ahi.Blo + Alo.Bhi
+                                    umma_f16<2>(d0, a[PM_H] + adv, b[PY_H] + adv, idesc, accum);
+                                    umma_f16<2>(d0, a[PM_H] + adv, b[PY_L] + adv, idesc, 1);
+                                    umma_f16<2>(d0, a[PM_L] + adv, b[PY_H] + adv, idesc, 1);
                                 } else if (PASS == 1) {     // Q = S1.S1, P2 = M.S2 + S2.M
                                     square(d0, PY_H, PY_L);
                                     cross(d1, PZ_H, PZ_L);
@@ -424,6 +438,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         const float unscale2 = exp2f(-(float)(p.pb.s0_shift + c.e2_in));          // M.S2 + S2.M sums
         const float scale2 = exp2f((float)c.e2_out);
         const float unscale3 = exp2f(-(float)(p.pb.s0_shift + c.e3_in));          // PASS 2: M.Z + Z.M sums
+        const float unscale_ab = exp2f(-(float)(c.e2_in + c.e1_in));              // PASS 3: A scaled by 2^e2, B by 2^e1
         const float scale3 = exp2f((float)c.e3_out);
         const bool upd0 = c.mode0 == MODE_ACTIVE;
         const bool conv0 = c.conv0 != 0;                // FroErr1 wanted (stop layer or frozen)
@@ -449,13 +464,13 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         int acc = 0;
         uint32_t acc_phase = 0;
         for (int t = pair; t < num_tiles; t += num_pairs) {
-            const uint32_t tl = p.tiles[t];
+            const uint32_t tl = tile_list[t];
             const int ti = 2 * (int)(tl & 0xFFFF) + (int)rank, tj = (int)(tl >> 16);
             const int gr = ti * kTile + q * 32 + lane;  // global row of this thread's TMEM lane
             const int gc_base = tj * kTile + half * kHalfCols;
             // the pair tile (IP, J = 2 IP) holds block (2 IP + 1, 2 IP) below the diagonal: its mirror is
             // computed by the pair tile (IP, 2 IP + 1), so the peer CTA only drains it
-            const bool live = ti <= tj;
+            const bool live = PASS == 3 || ti <= tj;
             float a0[kHalfCols], a1[kHalfCols];
 #pragma unroll
             for (int j = 0; j < kHalfCols; ++j) { a0[j] = 0.f; a1[j] = 0.f; }
@@ -500,6 +515,13 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 if (with_p1)
                     final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale1, scale1, conv0, r_dummy,
                                       r_dummy, r_f1, r_mx1);
+            } else if (PASS == 3) {
+                // C = 2^-(eA+eB) (A.B^T sums): plain fp32 output, no update, no split, no mirror
+                float* d = p.s1[1] + (size_t)gr * ld + gc_base;
+#pragma unroll
+                for (int j = 0; j < kHalfCols; j += 4)
+                    *reinterpret_cast<float4*>(d + j) = make_float4(unscale_ab * a0[j], unscale_ab * a0[j + 1],
+                                                                    unscale_ab * a0[j + 2], unscale_ab * a0[j + 3]);
             } else if (PASS == 2) {
                 // two more first-order fields, each exactly as P1 of pass 0
                 if (with_p0)

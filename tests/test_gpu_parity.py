@@ -738,3 +738,44 @@ def test_bench_line_has_the_contract_keys(dev):
     assert e["value"] > 0 and e["h2d_bytes_per_step"] == 2 * 256 * 256 * 4 and e["d2h_bytes_per_step"] == 2 * 256 * 256 * 4
     cb = d["cpu_baseline"]
     assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] > 0 and "sample" in cb
+
+
+# ------------------------------------------------------------------------------------------
+# general dual-half product and the congruence transforms (first half)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [40, 256, 333, 1100])
+def test_product_nt_matches_fp64(dev, n):
+    """C = A.B^T for general (non-symmetric) matrices: the dual-half product of PAPER.md:309-323 (Eqs. 44-46)."""
+    rng = np.random.default_rng(17 * n)
+    a = (rng.standard_normal((n, n)) * np.exp(rng.uniform(-3, 0, size=(n, 1)))).astype(np.float32)
+    b = (rng.uniform(-1, 1, size=(n, n)) * 37.0).astype(np.float32)
+    s = _solver(n, dev)
+    c = s.product_nt(torch.from_numpy(a).to(dev), torch.from_numpy(b).to(dev)).double().cpu().numpy()
+    s.close()
+    ad, bd = a.astype(np.float64), b.astype(np.float64)
+    ref = ad @ bd.T
+    bound = C_PROD * (np.abs(ad) @ np.abs(bd).T) + 3e-7 * np.abs(ref) + 1e-7 * np.abs(ad).max() * np.abs(bd).max()
+    assert np.all(np.abs(c - ref) <= bound), f"worst ratio {np.max(np.abs(c - ref) / bound):.2f}"
+
+
+def test_congruence_transform_with_the_inverse_factor(dev):
+    """PAPER.md:74-79, A17-A18: with Z = S^(-1/2) (Loewdin; computed in fp64 here, the factorisation itself is
+    not part of this build) Z^T S Z = I and H_orth = Z^T H Z, both through two dual-half products."""
+    n = 384
+    rng = np.random.default_rng(3)
+    g = rng.standard_normal((n, n)) / np.sqrt(n)
+    ovl = np.eye(n) + 0.3 * (g + g.T)                         # a well-conditioned overlap matrix
+    w, v = np.linalg.eigh(ovl)
+    assert w.min() > 0.05
+    z = (v / np.sqrt(w)) @ v.T
+    hb = rng.standard_normal((n, n))
+    h = (hb + hb.T) / 2
+    s = _solver(n, dev)
+    zt = torch.from_numpy(z.astype(np.float32)).to(dev)
+    i_gpu = s.congruence(zt, torch.from_numpy(ovl.astype(np.float32)).to(dev)).double().cpu().numpy()
+    h_gpu = s.congruence(zt, torch.from_numpy(h.astype(np.float32)).to(dev)).double().cpu().numpy()
+    s.close()
+    z32 = z.astype(np.float32).astype(np.float64)
+    assert np.abs(i_gpu - np.eye(n)).max() <= 5e-6
+    ref = z32.T @ h.astype(np.float32).astype(np.float64) @ z32
+    assert np.abs(h_gpu - ref).max() <= 1e-5 * np.abs(ref).max()
