@@ -160,6 +160,17 @@ int dmpt_layer_products2(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, co
  * order >= 1.  C may not alias A or B. */
 int dmpt_product_nt(dmpt_ctx *ctx, const float *d_a, const float *d_b, int ld, float *d_c, int ld_out);
 
+/* Inverse factor of a symmetric positive definite overlap matrix S (device, fp32, leading dimension ld):
+ * Z with Z^T S Z = I by the third-order recursion of PAPER.md:693-703 (A19-A21),
+ *     X_n = Z_n^T S Z_n,   Z_{n+1} = Z_n (1.875 I - 1.25 X_n + 0.375 X_n^2),   Z_0 = I / sqrt(eps_max(S)),
+ * every product through dmpt_product_nt's kernel (four per iteration).  eps_max is the Gershgorin bound, which
+ * the paper leaves open; all Z_n are then symmetric and the limit is S^(-1/2).  Stops when ||X_n - I||_F <= tol
+ * or when it no longer decreases (the noise floor of the arithmetic, ~1e-5 sqrt(n)); DMPT_ENOCONV after max_iter
+ * (<= 0: 30).  Writes Z to d_z (leading dimension ld_z), the iteration count and the last error (host).
+ * Contexts of order >= 1; uses the workspace's staging buffers (not concurrently with dmpt_run_host). */
+int dmpt_inverse_factor(dmpt_ctx *ctx, const float *d_s, int ld, float *d_z, int ld_z, int max_iter, double tol,
+                        int *h_iters, double *h_err);
+
 /* The three HBM-bound steps on their own (tests and micro-benchmarks; dmpt_run does not call these
  * entry points but launches the same kernels).  All run on the context's stream and return after it
  * drained.  Matrices are n x n (n of dmpt_create), row-major, leading dimensions in elements.

@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = (
     "dmpt_default_options", "dmpt_workspace_bytes", "dmpt_create", "dmpt_set_hamiltonian",
     "dmpt_run", "dmpt_run_host", "dmpt_layer_products", "dmpt_destroy", "dmpt_strerror",
     "dmpt_last_cuda_error", "dmpt_spectral_bounds", "dmpt_initial_transform", "dmpt_split",
-    "dmpt_layer_products2", "dmpt_product_nt", "dmpt_workspace_bytes_fields", "dmpt_set_hamiltonian_fields", "dmpt_run_fields",
+    "dmpt_layer_products2", "dmpt_product_nt", "dmpt_inverse_factor", "dmpt_workspace_bytes_fields", "dmpt_set_hamiltonian_fields", "dmpt_run_fields",
 )
 
 DMPT_OK, DMPT_EINVAL, DMPT_ESTATE, DMPT_ECUDA = 0, -1, -2, -3
@@ -94,6 +94,9 @@ def lib():
         L.dmpt_layer_products2.restype = C.c_int
         L.dmpt_product_nt.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int]
         L.dmpt_product_nt.restype = C.c_int
+        L.dmpt_inverse_factor.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_double,
+                                          C.POINTER(C.c_int), C.POINTER(C.c_double)]
+        L.dmpt_inverse_factor.restype = C.c_int
         L.dmpt_spectral_bounds.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double),
                                            C.POINTER(C.c_double)]
         L.dmpt_spectral_bounds.restype = C.c_int
@@ -185,6 +188,13 @@ def dmpt_layer_products2(ctx, s0_ptr, s1_ptr, s2_ptr, ld, x2_ptr, ld_out) -> int
 
 def dmpt_product_nt(ctx, a_ptr, b_ptr, ld, c_ptr, ld_out) -> int:
     return int(lib().dmpt_product_nt(ctx, C.c_void_p(a_ptr), C.c_void_p(b_ptr), int(ld), C.c_void_p(c_ptr), int(ld_out)))
+
+
+def dmpt_inverse_factor(ctx, s_ptr, ld, z_ptr, ld_z, max_iter, tol):
+    it, err = C.c_int(), C.c_double()
+    rc = int(lib().dmpt_inverse_factor(ctx, C.c_void_p(s_ptr), int(ld), C.c_void_p(z_ptr), int(ld_z), int(max_iter),
+                                       float(tol), C.byref(it), C.byref(err)))
+    return rc, it.value, err.value
 
 
 def dmpt_spectral_bounds(ctx, h0_ptr, ld):
@@ -404,6 +414,15 @@ class Dmpt:
         if rc != DMPT_OK:
             raise DmptError(rc, "dmpt_product_nt", dmpt_last_cuda_error(self.ctx))
         return c
+
+    def inverse_factor(self, s, max_iter=30, tol=0.0):
+        """(Z, iterations, ||Z^T S Z - I||_F) for a symmetric positive definite overlap matrix s."""
+        t = self.torch
+        z = t.empty((self.n, self.n), dtype=t.float32, device=self.device)
+        rc, it, err = dmpt_inverse_factor(self.ctx, s.data_ptr(), s.stride(0), z.data_ptr(), self.n, max_iter, tol)
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_inverse_factor", dmpt_last_cuda_error(self.ctx))
+        return z, it, err
 
     def congruence(self, z, h):
         """Z^T H Z for symmetric h: T = Z^T H = (Z^T).(H)^T, then T.Z = T.(Z^T)^T."""

@@ -781,9 +781,18 @@ extern "C" int dmpt_layer_products2(dmpt_ctx* ctx, const float* d_s0, const floa
 // dmpt_product_nt: C = A.B^T for general n x n matrices in the dual half-precision representation
 // (the congruence transforms either side of the hot path are two of these)
 // ---------------------------------------------------------------------------------------------
+static int product_nt_impl(dmpt_ctx* ctx, const float* d_a, int lda, const float* d_b, int ldb, float* d_c, int ld_out,
+                           bool sync);
+
 extern "C" int dmpt_product_nt(dmpt_ctx* ctx, const float* d_a, const float* d_b, int ld, float* d_c, int ld_out) {
     if (!ctx || !d_a || !d_b || !d_c) return DMPT_EINVAL;
     if (ld < ctx->n || ld_out < ctx->n || ctx->opt.order < 1) return DMPT_EINVAL;      // needs the S1 buffers
+    return product_nt_impl(ctx, d_a, ld, d_b, ld, d_c, ld_out, true);
+}
+
+// C may alias A or B here: both are copied into the workspace before the product and C is written afterwards.
+static int product_nt_impl(dmpt_ctx* ctx, const float* d_a, int lda, const float* d_b, int ldb, float* d_c, int ld_out,
+                           bool sync) {
     const Layout& L = ctx->L;
     const size_t n = ctx->n, np = L.n_pad;
     cudaStream_t st = ctx->stream;
@@ -792,9 +801,9 @@ extern "C" int dmpt_product_nt(dmpt_ctx* ctx, const float* d_a, const float* d_b
     double* partials2 = ctx->at<double>(L.partials2);
     const int grid = elementwise_grid(ctx, (long long)np * np, 256);
     // A -> the S0 buffers (operand pair 0, scale 2^e2), B -> the S1 buffers (operand pair 1, scale 2^e1)
-    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_a, (int)n, ld, (int)np, ctx->lp.s0, partials2);
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_a, (int)n, lda, (int)np, ctx->lp.s0, partials2);
     CK(cudaGetLastError());
-    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_b, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_b, (int)n, ldb, (int)np, ctx->lp.s1[0], partials);
     CK(cudaGetLastError());
     single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, partials2, grid);
     CK(cudaGetLastError());
@@ -807,8 +816,64 @@ extern "C" int dmpt_product_nt(dmpt_ctx* ctx, const float* d_a, const float* d_b
     int rc = launch_pass<3>(ctx);
     if (rc) return rc;
     CK(cudaMemcpy2DAsync(d_c, (size_t)ld_out * 4, ctx->lp.s1[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
-    CK(cudaStreamSynchronize(st));
+    if (sync) CK(cudaStreamSynchronize(st));
     return DMPT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// dmpt_inverse_factor: Z with Z^T S Z = I by the third-order recursion of PAPER.md:693-703 (A19-A21)
+// ---------------------------------------------------------------------------------------------
+extern "C" int dmpt_inverse_factor(dmpt_ctx* ctx, const float* d_s, int ld, float* d_z, int ld_z, int max_iter,
+                                   double tol, int* h_iters, double* h_err) {
+    if (!ctx || !d_s || !d_z || ld < ctx->n || ld_z < ctx->n || ctx->opt.order < 1) return DMPT_EINVAL;
+    if (max_iter <= 0) max_iter = 30;
+    const Layout& L = ctx->L;
+    const int n = ctx->n;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    long long* bounds = ctx->at<long long>(L.bounds);
+    double* partials = ctx->at<double>(L.partials);
+    float* x = ctx->at<float>(L.stage_h0);       // n x n scratch (the staging buffers of dmpt_run_host)
+    float* t = ctx->at<float>(L.stage_h1);
+    // Z_0 = I / sqrt(eps_max): S is positive definite, so X_0 = S / eps_max has its spectrum in (0, 1]
+    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    CK(cudaGetLastError());
+    dmpt_gershgorin_kernel<<<elementwise_grid(ctx, (long long)n * 32, 256), 256, 0, st>>>(d_s, n, ld, bounds);
+    CK(cudaGetLastError());
+    long long hb[2];
+    CK(cudaMemcpyAsync(hb, bounds, sizeof hb, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    const double emax = ordered_to_dbl(hb[1]);
+    if (!(emax > 0.0) || !isfinite(emax)) return DMPT_EDEGENERATE;
+    const int egrid = elementwise_grid(ctx, (long long)n * n, 256);
+    dmpt_scaled_identity_kernel<<<egrid, 256, 0, st>>>(d_z, n, ld_z, bounds);
+    CK(cudaGetLastError());
+    std::vector<double> hp(egrid);
+    double err = INFINITY, prev = INFINITY;
+    int it = 0, rc = DMPT_OK;
+    for (; it < max_iter; ++it) {
+        // X_n = Z_n^T S Z_n (A19); every Z_n is a polynomial in S, hence symmetric: Z^T = Z
+        if ((rc = product_nt_impl(ctx, d_z, ld_z, d_s, ld, t, n, false))) return rc;      // T = Z S
+        if ((rc = product_nt_impl(ctx, t, n, d_z, ld_z, x, n, false))) return rc;         // X = T Z
+        if ((rc = product_nt_impl(ctx, x, n, x, n, t, n, false))) return rc;              // X^2
+        dmpt_zpoly_kernel<<<egrid, 256, 0, st>>>(x, t, n, partials);                       // W = sum a_k X^k, ||X - I||_F^2
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(hp.data(), partials, egrid * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        prev = err;
+        err = 0.0;
+        for (int b = 0; b < egrid; ++b) err += hp[b];
+        err = sqrt(err);
+        if (!isfinite(err)) { rc = DMPT_ENUMERIC; break; }
+        // stop at the requested error, or at the noise floor of the arithmetic (no further decrease)
+        if (err <= tol || (it > 0 && err >= 0.5 * prev && err < 1e-2)) break;
+        if ((rc = product_nt_impl(ctx, d_z, ld_z, t, n, d_z, ld_z, false))) return rc;    // Z_{n+1} = Z_n W (A20)
+    }
+    CK(cudaStreamSynchronize(st));
+    if (h_iters) *h_iters = it;
+    if (h_err) *h_err = err;
+    if (rc == DMPT_OK && it >= max_iter) rc = DMPT_ENOCONV;
+    return rc;
 }
 
 // ---------------------------------------------------------------------------------------------

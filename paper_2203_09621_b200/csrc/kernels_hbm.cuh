@@ -275,6 +275,44 @@ __global__ void dmpt_field_init_kernel(DmptCtl* ctl, DmptProblem pb, const doubl
 }
 
 // ---------------------------------------------------------------------------------------------
+// Inverse factorisation (A19-A21): the two elementwise steps around the products.
+//   Z_0 = I / sqrt(eps_max(S)) with the Gershgorin bound of S, so that the spectrum of X_0 = Z_0 S Z_0 lies in (0, 1]
+//   W   = a_0 I + a_1 X + a_2 X^2,  a = {1.875, -1.25, 0.375} (A20, A21), and ||X - I||_F^2 per block
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dmpt_scaled_identity_kernel(float* __restrict__ z, int n, int ld,
+                                                                   const long long* __restrict__ bounds) {
+    const float d = (float)(1.0 / sqrt(ordered_to_dbl(bounds[1])));
+    const long long total = (long long)n * n;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int row = (int)(i / n), col = (int)(i - (long long)row * n);
+        z[(size_t)row * ld + col] = row == col ? d : 0.f;
+    }
+}
+
+__global__ void __launch_bounds__(256) dmpt_zpoly_kernel(const float* __restrict__ x, float* __restrict__ x2_to_w, int n,
+                                                         double* __restrict__ partials /* [grid] */) {
+    const long long total = (long long)n * n;
+    double err = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int row = (int)(i / n), col = (int)(i - (long long)row * n);
+        const float dg = row == col ? 1.f : 0.f;
+        const float xv = x[i];
+        const float d = xv - dg;
+        err += (double)d * (double)d;
+        x2_to_w[i] = fmaf(0.375f, x2_to_w[i], fmaf(-1.25f, xv, 1.875f * dg));
+    }
+    __shared__ double sh[8];
+    err = warp_sum(err);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = err;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += sh[w];
+        partials[blockIdx.x] = t;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // a3  Split (Eq. 13, 302-307 Eqs. 42-43) after an exact power-of-two scale 2^e
 //     (readings R12/R17): hi = fp16(2^e x), lo = fp16(2^e x - hi), round-to-nearest-even.
 //     8 elements per thread: two 128-bit loads, one 128-bit store per output.

@@ -779,3 +779,56 @@ def test_congruence_transform_with_the_inverse_factor(dev):
     assert np.abs(i_gpu - np.eye(n)).max() <= 5e-6
     ref = z32.T @ h.astype(np.float32).astype(np.float64) @ z32
     assert np.abs(h_gpu - ref).max() <= 1e-5 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("n", [96, 384, 1000])
+def test_inverse_factor_matches_oracle(dev, n):
+    """PAPER.md:693-703 (A19-A21) on the device against oracle/inverse_factor.py (fp64), then the full
+    non-orthogonal round trip of PAPER.md:74-79: H_orth = Z^T H Z -> D_orth -> D = Z D_orth Z^T."""
+    from oracle.inverse_factor import inverse_factor
+
+    rng = np.random.default_rng(5 * n)
+    g = rng.standard_normal((n, n)) / np.sqrt(n)
+    ovl = (np.eye(n) + 0.3 * (g + g.T)).astype(np.float32)
+    ovl = ((ovl + ovl.T) / 2).astype(np.float32)
+    z_ref, errs = inverse_factor(ovl)
+    s = _solver(n, dev)
+    z, it, err = s.inverse_factor(torch.from_numpy(ovl).to(dev))
+    zd = z.double().cpu().numpy()
+    assert abs(it - (len(errs) - 1)) <= 3, (it, len(errs))          # fp64 runs on to 1e-12, the device to its noise floor
+    assert err <= 2e-5 * np.sqrt(n)
+    assert np.abs(zd - z_ref).max() <= 2e-5 * np.abs(z_ref).max()
+    od = ovl.astype(np.float64)
+    assert np.abs(zd.T @ od @ zd - np.eye(n)).max() <= 2e-5
+    s.close()
+
+
+def test_non_orthogonal_round_trip(dev, config1):
+    """PAPER.md:74-79 and A9-A18: for a non-orthogonal basis with overlap S, D = Z D_orth Z^T with
+    D_orth = theta(mu I - Z^T H Z).  The whole chain on the device (inverse factor, congruence, the layer
+    recursion, back-transformation) against the generalised eigenproblem H c = eps S c solved in fp64."""
+    import scipy.linalg
+
+    wl = config1
+    n = wl.n
+    rng = np.random.default_rng(8)
+    g = rng.standard_normal((n, n)) / np.sqrt(n)
+    ovl = np.eye(n) + 0.25 * (g + g.T)
+    w, v = np.linalg.eigh(ovl)
+    s_half = (v * np.sqrt(w)) @ v.T
+    h = s_half @ wl.h0.astype(np.float64) @ s_half                 # so that the orthogonalised H is config 1's H0
+    h32 = ((h + h.T) / 2).astype(np.float32)
+    s32 = ((ovl + ovl.T) / 2).astype(np.float32)
+    eps, c = scipy.linalg.eigh(h32.astype(np.float64), s32.astype(np.float64))
+    d_ref = c[:, :wl.n_occ] @ c[:, :wl.n_occ].T                    # A11 in the non-orthogonal basis
+    sol = _solver(n, dev, order=1)
+    z, _, _ = sol.inverse_factor(torch.from_numpy(s32).to(dev))
+    h_orth = sol.congruence(z, torch.from_numpy(h32).to(dev))       # Z^T H Z
+    h_orth = ((h_orth + h_orth.T) / 2).contiguous()                 # exact symmetry is a precondition of dmpt_run
+    sol.set_hamiltonian(h_orth, torch.zeros_like(h_orth), wl.n_occ)
+    res = sol.run()
+    assert res.status == 0
+    d = sol.product_nt(sol.product_nt(z, res.d0), z)                # (Z D_orth^T) Z^T = Z D_orth Z^T (A18)
+    sol.close()
+    assert np.abs(d.double().cpu().numpy() - d_ref).max() <= 2e-4
+    assert abs(np.trace(d.double().cpu().numpy() @ s32.astype(np.float64)) - wl.n_occ) <= 2e-3      # Tr[D S] = N_occ

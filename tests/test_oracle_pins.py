@@ -358,3 +358,27 @@ def test_ground_state_sp2_matches_the_definition():
         assert np.abs(d0 - ref0).max() < 1e-10
         assert abs(np.trace(d0) - wl.n_occ) < 1e-9
         assert layers == O2.dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ).layers_d0
+
+
+def test_inverse_factor_recursion():
+    """PAPER.md:686-703 (A17-A21): Z^T S Z = I, the limit from Z_0 ~ I is the Loewdin factor S^(-1/2), the
+    error decays cubically, and the polynomial is the third-order expansion of x^(-1/2) around 1."""
+    from oracle.inverse_factor import A_K, inverse_factor
+
+    rng = np.random.default_rng(11)
+    n = 60
+    g = rng.standard_normal((n, n)) / np.sqrt(n)
+    s = np.eye(n) + 0.35 * (g + g.T)
+    w, v = np.linalg.eigh(s)
+    assert w.min() > 0.05
+    z, err = inverse_factor(s)
+    assert np.abs(z.T @ s @ z - np.eye(n)).max() < 1e-12                     # A17
+    assert np.abs(z - (v / np.sqrt(w)) @ v.T).max() < 1e-11                   # Loewdin factor (PAPER.md:688)
+    # cubic decay once inside the convergence region: e_{n+1} <= C e_n^3 with a modest C
+    tail = [e for e in err if e < 0.3]
+    assert len(tail) >= 2 and all(b <= 2.0 * a ** 3 + 1e-13 for a, b in zip(tail, tail[1:]))
+    # A21: (1 + d)^(-1/2) = 1 - d/2 + 3 d^2/8 + O(d^3), rewritten in x = 1 + d
+    d = 1e-3
+    x = 1.0 + d
+    assert abs((A_K[0] + A_K[1] * x + A_K[2] * x * x) - x ** -0.5) < 1.0 * d ** 3
+    assert abs(sum(A_K) - 1.0) < 1e-15
