@@ -113,14 +113,14 @@ std::vector<uint32_t> make_tile_order(int nb, int band) {
     return t;
 }
 
-// Every pair tile (IP, J), same band order: the general product C = A.B^T has no symmetry to exploit.
+// Every 256 x 256 tile (IP, J even), same band order: the general product C = A.B^T has no symmetry to exploit.
 std::vector<uint32_t> make_tile_order_full(int nb, int band) {
     std::vector<uint32_t> t;
     const int nbp = nb / 2;
-    t.reserve((size_t)nbp * nb);
+    t.reserve((size_t)nbp * nbp);
     for (int b0 = 0; b0 < nbp; b0 += band) {
         const int b1 = b0 + band < nbp ? b0 + band : nbp;
-        for (int j = 0; j < nb; ++j)
+        for (int j = 0; j < nb; j += 2)                      // block columns j, j + 1 together
             for (int ip = b0; ip < b1; ++ip) t.push_back((uint32_t)ip | ((uint32_t)j << 16));
     }
     return t;
@@ -344,7 +344,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.tiles = ctx->at<uint32_t>(L.tiles);
     lp.num_tiles = L.num_tiles;
     lp.tiles_full = ctx->at<uint32_t>(L.tiles_full);
-    lp.num_tiles_full = (nb / 2) * nb;
+    lp.num_tiles_full = (nb / 2) * (nb / 2);
     lp.n_pad = L.n_pad;
     lp.wave_sync = (o.wave_sync && L.num_tiles > ctx->grid_layer / 2) ? 1 : 0;
     lp.ctl = ctx->at<DmptCtl>(L.ctl);

@@ -63,8 +63,10 @@ template <> struct PassCfg<0> { static constexpr int kOps = 4, kStages = 4; };
 template <> struct PassCfg<1> { static constexpr int kOps = 6, kStages = 3; };
 template <> struct PassCfg<2> { static constexpr int kOps = 6, kStages = 3; };
 // PASS 3: a general product C = A.B^T on its own (A, B any n x n matrices; the congruence
-// transforms Z^T H Z, Z D Z^T are two of these): the A side stages A hi/lo only, the B side B hi/lo only
-template <> struct PassCfg<3> { static constexpr int kOps = 4, kStages = 4; };
+// transforms Z^T H Z, Z D Z^T are two of these).  A tile is 256 rows x 256 columns: the A side stages A hi/lo
+// (positions 0, 1), the B side B hi/lo of column block 2 JP (positions 2, 3) and of 2 JP + 1 (positions 4, 5);
+// one accumulator per column block, six MMAs per 32 KiB staged.
+template <> struct PassCfg<3> { static constexpr int kOps = 6, kStages = 3; };
 constexpr int kChunkK = 128;               // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
@@ -95,7 +97,8 @@ struct LayerParams {
     __half* h[2][8];            // fp16 operand matrices the epilogue writes, same order as maps
     const uint32_t* tiles;      // pair tiles (IP | J << 16): block rows 2 IP, 2 IP + 1 x block column J >= 2 IP
     int num_tiles;
-    const uint32_t* tiles_full; // PASS 3: every (IP, J), the output is not symmetric
+    const uint32_t* tiles_full; // PASS 3: every (IP | J << 16) with J even: block rows 2 IP, 2 IP + 1 x block
+                                // columns J, J + 1 (256 x 256); the output is not symmetric
     int num_tiles_full;
     int n_pad;
     int wave_sync;              // 1: producers of all CTAs re-align at every tile boundary (L2 reuse)
@@ -264,7 +267,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     // PASS 2: one accumulator per extra field, until that field's stopping test fired.
     // PASS 3: accumulator 0 only, fed by A hi/lo (positions 0, 1, A side) and B hi/lo (positions 2, 3, B side).
     const bool with_p0 = PASS == 3 ? true : (PASS == 0 ? c.mode0 != MODE_FROZEN : (PASS == 1 || c.conv2 == 0));
-    const bool with_p1 = PASS == 3 ? false
+    const bool with_p1 = PASS == 3 ? true
                                    : (PASS == 0 ? p.pb.order >= 1 : (PASS == 1 || (p.pb.nfields >= 3 && c.conv3 == 0)));
     const int nops = (with_p1 || PASS == 3) ? kOps : kOps - 2;    // the last operand pair only feeds accumulator 1
     unsigned int* wave_ctr = PASS == 0 ? &p.ctl->wave : &p.ctl->wave2;
@@ -335,7 +338,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                     const uint32_t base = smem_base + stage * kStageBytes;
                     if (elect_one()) {
                         if (rank == 0)
-                            mbar_arrive_expect_tx(fb, PASS == 3 ? 2 * 2 * (kABytes + kBBytes) : 2 * nops * (kABytes + kBBytes));
+                            mbar_arrive_expect_tx(fb, PASS == 3 ? 2 * (2 * kABytes + 4 * kBBytes) : 2 * nops * (kABytes + kBBytes));
                         const int k0 = kb * kBK;
 #pragma unroll
                         for (int o = 0; o < kOps; ++o) {
@@ -343,8 +346,9 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                                 tma_load_2d_2sm(base + o * kABytes, maps[o], fb, k0, row_a);
                                 tma_load_2d_2sm(base + o * kABytes + kBBytes, maps[o], fb, k0, row_a + kBRows);
                             }
-                            if (o < nops && !(PASS == 3 && o < 2))           // B side (PASS 3: B hi/lo only)
-                                tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[o], fb, k0, row_b);
+                            if (o < nops && !(PASS == 3 && o < 2))           // B side (PASS 3: B hi/lo of two column blocks)
+                                tma_load_2d_2sm(base + kBOff + o * kBBytes, maps[PASS == 3 && o >= 4 ? o - 2 : o], fb, k0,
+                                                PASS == 3 && o >= 4 ? row_b + kTile : row_b);
                         }
                     }
                     __syncwarp();
@@ -401,10 +405,13 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                                 if (PASS == 0) {            // P0 = M.M, P1 = M.S1 + S1.M
                                     if (with_p0) square(d0, PM_H, PM_L);
                                     if (with_p1) cross(d1, PY_H, PY_L);
-                                } else if (PASS == 3) {     // C = A.B^T: Ahi.Bhi + Ahi.Blo + Alo.Bhi
+                                } else if (PASS == 3) {     // C = A.B^T: Ahi.Bhi + Ahi.Blo + Alo.Bhi, two column blocks
                                     umma_f16<2>(d0, a[PM_H] + adv, b[PY_H] + adv, idesc, accum);
                                     umma_f16<2>(d0, a[PM_H] + adv, b[PY_L] + adv, idesc, 1);
                                     umma_f16<2>(d0, a[PM_L] + adv, b[PY_H] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[PM_H] + adv, b[PZ_H] + adv, idesc, accum);
+                                    umma_f16<2>(d1, a[PM_H] + adv, b[PZ_L] + adv, idesc, 1);
+                                    umma_f16<2>(d1, a[PM_L] + adv, b[PZ_H] + adv, idesc, 1);
                                 } else if (PASS == 1) {     // Q = S1.S1, P2 = M.S2 + S2.M
                                     square(d0, PY_H, PY_L);
                                     cross(d1, PZ_H, PZ_L);
@@ -519,9 +526,12 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 // C = 2^-(eA+eB) (A.B^T sums): plain fp32 output, no update, no split, no mirror
                 float* d = p.s1[1] + (size_t)gr * ld + gc_base;
 #pragma unroll
-                for (int j = 0; j < kHalfCols; j += 4)
+                for (int j = 0; j < kHalfCols; j += 4) {
                     *reinterpret_cast<float4*>(d + j) = make_float4(unscale_ab * a0[j], unscale_ab * a0[j + 1],
                                                                     unscale_ab * a0[j + 2], unscale_ab * a0[j + 3]);
+                    *reinterpret_cast<float4*>(d + kTile + j) = make_float4(unscale_ab * a1[j], unscale_ab * a1[j + 1],
+                                                                            unscale_ab * a1[j + 2], unscale_ab * a1[j + 3]);
+                }
             } else if (PASS == 2) {
                 // two more first-order fields, each exactly as P1 of pass 0
                 if (with_p0)
