@@ -127,38 +127,80 @@ def fma_executed(n_pad, layers, layers_d0, order=1, layers_d1=0):
 # ---------------------------------------------------------------------------------------------
 # CPU oracle legs (cpu_baseline and --impl reference): the only places that touch oracle/
 # ---------------------------------------------------------------------------------------------
-def oracle_sample(config, n_sample, layers):
+ORACLE_FP64_TFLOPS_GUESS = 0.4      # dgemm rate of the host BLAS on 16 threads (round 1: 0.5 Tflops FMA=1 ... /1.25), sizing only
+
+
+def oracle_sample(config, n_sample, layers, wl=None):
     """Time oracle.dnn_sp2_pt (fp64, numpy/host BLAS, as it stands) for `layers` layers of the
-    bench workload's generator at size n_sample.  Returns (Tflops FMA=1, seconds, threads)."""
+    bench workload's generator at size n_sample (the bench workload itself when `wl` is given).
+    Returns (Tflops FMA=1, seconds, threads, layers run)."""
     from oracle.dnn_sp2_pt import dnn_sp2_pt
     from workloads import make_config
 
-    wl = make_config(config, n=n_sample)
+    if wl is None or wl.n != n_sample:
+        import torch
+        wl = make_config(config, n=n_sample, device="cuda" if (n_sample >= 8192 and torch.cuda.is_available()) else None)
     t0 = time.perf_counter()
     res = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, order=wl.order, max_layers=layers)
     dt = time.perf_counter() - t0
     fl = flops_paper(n_sample, res.layers, res.layers_d0, wl.order, res.layers_d1)
-    return fl / dt / 1e12, dt, len(os.sched_getaffinity(0))
+    return fl / dt / 1e12, dt, len(os.sched_getaffinity(0)), res.layers
+
+
+def oracle_o3_d0(wl):
+    """Layer at which Algorithm 2 fires in fp64, from O3 (oracle/spectral.py) on the spectrum the generator
+    constructed and the oracle's own Gershgorin bounds of the rounded H0: O(N) per layer."""
+    from oracle.dnn_sp2_pt import gershgorin
+    from oracle.spectral import spectral_recursion
+
+    if "eps" not in wl.meta:
+        return None
+    lo, hi = gershgorin(wl.h0)
+    return int(spectral_recursion(wl.meta["eps"], wl.n_occ, lo, hi)["layers_d0"])
+
+
+def reference_sample_size(n, order, steps, budget_s=300.0):
+    """Bounded sample of the reference arm: the bench workload's own N with 3 layers per step when K steps of it
+    fit `budget_s`, else the generator at N/2, N/4, ... with as many layers (<= 20) as fit.  Cost model: 2 (order
+    2: 4) dgemm of 2 n^3 flop per layer at ORACLE_FP64_TFLOPS_GUESS, + 30 % for the elementwise passes."""
+    per_step = budget_s / max(1, steps)
+    dgemms = 4 if order == 2 else 2
+    n_s = n
+    while True:
+        per_layer = 1.3 * dgemms * 2.0 * float(n_s) ** 3 / (ORACLE_FP64_TFLOPS_GUESS * 1e12)
+        if 3 * per_layer <= per_step or n_s <= 512:
+            return n_s, (3 if (n_s == n and n > 4096) else int(max(3, min(20, per_step // per_layer))))
+        n_s //= 2
 
 
 def run_reference(args):
     from paper_2203_09621_b200 import replicas
+    from workloads import CONFIGS
 
     if replicas.env_ranks()[0] != 0:          # under torchrun rank 0 alone runs and prints the oracle's line
         return 0
-    n_s, layers = args.ref_n, args.ref_layers
+    order = CONFIGS[args.config]["order"]
+    n_s, layers = reference_sample_size(args.n, order, args.steps)
+    if args.ref_n is not None:
+        n_s = args.ref_n
+    if args.ref_layers is not None:
+        layers = args.ref_layers
     for _ in range(args.warmup and 1):          # one untimed pass pages numpy/BLAS in
         oracle_sample(args.config, min(n_s, 512), 1)
+    from workloads import make_config
+    import torch
+    wl = make_config(args.config, n=n_s, device="cuda" if (n_s >= 8192 and torch.cuda.is_available()) else None)
     vals, secs = [], []
     cores = len(os.sched_getaffinity(0))
     for _ in range(args.steps):
-        v, dt, cores = oracle_sample(args.config, n_s, layers)
+        v, dt, cores, _ = oracle_sample(args.config, n_s, layers, wl)
         vals.append(v)
         secs.append(dt)
     value = sum(vals) / len(vals)
-    sample = f"oracle.dnn_sp2_pt (fp64) on the config-{args.config} generator at n={n_s}, first {layers} layers, per step"
+    sample = (f"oracle.dnn_sp2_pt (fp64) on the config-{args.config} generator at n={n_s}, first {layers} layers, per step"
+              + ("" if n_s == args.n else f" (the workload's N={args.n} does not fit {args.steps} steps in a few minutes)"))
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": replicas.env_ranks()[2],
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(secs) / len(secs),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "gpu_launches": 0,
@@ -298,18 +340,32 @@ def run_ours(args):
         e2e_value = sum_over_ranks(e2e_flops) / (ms_e2e * 1e-3) / 1e12
 
     if rank == 0:
+        traffic, traffic_src = ncu_traffic(n, order, nf, args.traffic)
         peaks, peaks_kind = load_peaks()
         peak_tf = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
         layer_ms = ms_loop / max(1, layers_total)
         achieved_tf = 2.0 * fma / (ms_loop * 1e-3) / 1e12
-        cpu_v, cpu_dt, cores = oracle_sample(args.config, args.ref_n, args.ref_layers)
+        # the oracle as it stands on THIS workload: 3 layers at the bench N when that is about
+        # 1-3 min of host time, the whole run when it is shorter; per-layer seconds and the time-to-D1 extrapolated
+        # with O3's layer count.  A second, smaller sample (n = 4096 generator, 20 layers) keeps round 1's key.
+        ref_n = args.ref_n if args.ref_n is not None else n
+        ref_layers = args.ref_layers if args.ref_layers is not None else (3 if n > 4096 else 200)
+        cpu_v, cpu_dt, cores, cpu_layers = oracle_sample(args.config, ref_n, ref_layers, wl)
+        o3_d0 = oracle_o3_d0(wl) if ref_n == n else None
+        cpu_extra = {}
+        if ref_n == n and n > 4096 and args.ref_n is None:
+            v2, dt2, _, l2 = oracle_sample(args.config, 4096, 20)
+            cpu_extra = {"secondary": {"value": v2, "seconds": dt2, "sample": f"config-{args.config} generator at n=4096, first {l2} layers"}}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f16 x f16 -> f32 (dual-half), f64 scalars",
             "data": "synthetic", "gpu_launches": launches,
             "config": {"workload": workload_name(args), "n": n, "n_occ": wl.n_occ, "order": order, "fields": nf,
-                       "layers": res.layers, "layers_d0": res.layers_d0, "gap": wl.meta.get("gap"),
+                       "layers": res.layers, "layers_d0": res.layers_d0, "layers_d0_oracle_o3": o3_d0,
+                       "layers_note": "O3 = the fp64 recursion on the constructed spectrum; it runs 1-5 layers past "
+                                      "any dual-half run (stop at the noise floor, R14)",
+                       "gap": wl.meta.get("gap"),
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": f"inputs larger than L2 ({n * n * 4 / 2**30:.2f} GiB per matrix); no flush needed",
                        "time_to_d1_ms": ms / args.steps, "loop_ms": ms_loop / args.steps,
@@ -321,13 +377,19 @@ def run_ours(args):
                      "h2d_bytes_per_step": 2 * n * n * 4, "d2h_bytes_per_step": n_out * n * n * 4}
                     if nf == 1 else None),
             "roofline": {"bound": "tensor", "kernel": "dmpt_layer_kernel", "achieved": achieved_tf, "peak": peak_tf,
-                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": args.traffic,
+                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": traffic,
+                         "traffic_source": traffic_src,
                          "peak_kind": f"bf16_tflops_sustained, {peaks_kind} (fp16 = bf16 rate), 2 flops per FMA",
                          "avg_launch_ms": layer_ms, "executed_tfma_per_s": achieved_tf / 2.0,
                          "frac_nominal_1125_tfma": achieved_tf / 2.0 / NOMINAL_FP16_TFMA},
-            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": cpu_dt,
-                             "sample": f"oracle.dnn_sp2_pt (fp64) on the config-{args.config} generator at "
-                                       f"n={args.ref_n}, first {args.ref_layers} layers"},
+            "cpu_baseline": dict({"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": cpu_dt,
+                                  "sample": f"oracle.dnn_sp2_pt (fp64) on the bench workload itself (config {args.config}, "
+                                            f"n={ref_n}), first {cpu_layers} layers incl. bounds and transform",
+                                  "seconds_per_layer": cpu_dt / max(1, cpu_layers),
+                                  "time_to_d1_s_extrapolated": (cpu_dt / max(1, cpu_layers) * (o3_d0 + 3)
+                                                                if o3_d0 and cpu_layers < o3_d0 else None),
+                                  "extrapolation": "seconds_per_layer x (O3 fp64 D0 stop layer + 3 further layers, "
+                                                   "PAPER.md:483); extrapolated, not run"}, **cpu_extra),
         }
         print(json.dumps(line), flush=True)
     solver.close()
@@ -340,9 +402,43 @@ def solver_n_pad(n):
     return (n + 255) // 256 * 256      # CTA-pair tiles: 256 rows
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE dmpt_layer_kernel launch, from the `ncu --set full`
-# capture of this command committed under profiles/ (the file named there); only for the default workload
-NCU_TRAFFIC_BYTES = {16384: 30.65e9}      # profiles/r01_layer_kernel_v3.md: 26.18 GB read + 4.47 GB written
+def kernel_source_sha():
+    """sha256 (first 16 hex digits) of the layer kernel's sources: an ncu capture is only quoted for the code it saw."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("layer_kernel.cuh", "ptx.cuh"):
+        with open(os.path.join(ROOT, "paper_2203_09621_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(n, order, nf, override):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE dmpt_layer_kernel launch from the `ncu --set full` capture
+    recorded in profiles/layer_kernel_traffic.json (written from the capture named there); null when that capture
+    saw other kernel sources than the ones being timed, or another workload."""
+    if override is not None:
+        return override, "--traffic"
+    p = os.path.join(ROOT, "profiles", "layer_kernel_traffic.json")
+    if not os.path.exists(p):
+        return None, "no capture recorded"
+    with open(p) as f:
+        rec = json.load(f)
+    if rec.get("n") != n or rec.get("order") != order or nf != 1:
+        return None, "capture is of another workload"
+    if rec.get("kernel_source_sha") != kernel_source_sha():
+        return None, f"stale: {rec.get('capture')} saw kernel sources {rec.get('kernel_source_sha')}"
+    return rec["dram_bytes_per_launch"], rec.get("capture")
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` with N > 1 outside torchrun: launch the N ranks ourselves (one per GPU)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -353,8 +449,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--n", type=int, default=None, help="override the matrix size (default: the config's)")
-    ap.add_argument("--ref-n", type=int, default=4096, help="size of the oracle's bounded sample")
-    ap.add_argument("--ref-layers", type=int, default=20)
+    ap.add_argument("--ref-n", type=int, default=None, help="size of the oracle's bounded sample (default: the workload's)")
+    ap.add_argument("--ref-layers", type=int, default=None)
     ap.add_argument("--fields", type=int, default=1,
                     help="perturbations sharing H0 in one run (1..3); value then counts every field as a run of its own")
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per layer launch from ncu (profiles/)")
@@ -362,8 +458,11 @@ def main():
     if args.n is None:
         from workloads import CONFIGS
         args.n = CONFIGS[args.config]["n"]
-    if args.traffic is None and args.config == 4 and args.fields == 1:
-        args.traffic = NCU_TRAFFIC_BYTES.get(args.n)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus != world:
+        if world == 1 and args.gpus > 1:
+            return respawn_under_torchrun(args)
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warmup raised to 3 (timing rules)", file=sys.stderr)
         args.warmup = 3

@@ -81,9 +81,9 @@ typedef struct dmpt_result {
     double fro_err0;           /* FroErr0 = ||S0 - S0^2||_F at the D0 stop layer; NaN at order 0 */
     double ms_total;           /* CUDA-event time of the whole run (bounds + transform + split + loop) */
     double ms_loop;            /* CUDA-event time of the layer loop alone ("time for main loop", Eq. 82)*/
-    double ms_bounds;          /* a1: Gershgorin kernel (+ scalar set-up)                                */
-    double ms_transform;       /* a2: initial transform kernel (+ first decision)                        */
-    double ms_split;           /* a3: the two initial split kernels                                      */
+    double ms_bounds;          /* a1: Gershgorin kernel, which also takes max|H1| (+ scalar set-up)      */
+    double ms_transform;       /* a2 + a3 fused: S0, S1 and their first operand split (+ first decision) */
+    double ms_split;           /* what follows it before the loop (order 2: S2_0 = 0 and its first scale) */
     double reserved_d[1];
     /* Per-layer records, entry n-1 for layer n.  Caller-allocated HOST arrays of max_layers
      * entries each, or NULL to skip.  Entries the run did not reach are left untouched. */
@@ -157,7 +157,7 @@ int dmpt_layer_products2(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, co
  * A18, are two of these each): C = A.B^T = A_hi.B_hi^T + A_hi.B_lo^T + A_lo.B_hi^T for ANY n x n device
  * matrices A, B (fp32, leading dimension ld), fp32 accumulation promoted every 128 columns like the layer
  * products; each operand is split after its own power-of-two scale (max|.| into [8, 16)).  Contexts of
- * order >= 1.  C may not alias A or B. */
+ * order >= 1.  C may alias A or B (both are copied into the workspace before C is written). */
 int dmpt_product_nt(dmpt_ctx *ctx, const float *d_a, const float *d_b, int ld, float *d_c, int ld_out);
 
 /* Inverse factor of a symmetric positive definite overlap matrix S (device, fp32, leading dimension ld):
@@ -176,7 +176,8 @@ int dmpt_inverse_factor(dmpt_ctx *ctx, const float *d_s, int ld, float *d_z, int
  * drained.  Matrices are n x n (n of dmpt_create), row-major, leading dimensions in elements.
  *   a1  Gershgorin discs of d_h0 -> *h_eps_min, *h_eps_max (host).
  *   a2  S0 = (eps_max I - H0)/W, S1 = -H1/W, W = eps_max - eps_min (Eq. 34, 493), each
- *       element formed in fp64 and rounded once to fp32; *h_tr_s0 (host, may be NULL) = Tr S0.
+ *       element formed in fp64 and rounded once to fp32; *h_tr_s0 (host, may be NULL) = Tr S0.  (The kernel
+ *       is the fused a2 + a3 kernel of dmpt_run: it also leaves the first operand split in the workspace.)
  *   a3  hi = fp16(2^shift x), lo = fp16(2^shift x - hi), round-to-nearest-even (Eq. 13);
  *       d_hi, d_lo are device fp16 (uint16_t bit patterns), leading dimension ld_out.  diag_half != 0
  *       splits x - I/2 instead (the form the order-0 operands take). */

@@ -274,6 +274,10 @@ class Dmpt:
         if bounds is not None:
             opt.bounds = 1
             opt.eps_min, opt.eps_max = float(bounds[0]), float(bounds[1])
+        # size the per-layer record buffers as the library does (dmpt_create: <= 0 -> 200, capped at 1024)
+        if opt.max_layers <= 0:
+            opt.max_layers = 200
+        opt.max_layers = min(opt.max_layers, 1024)
         self.max_layers = opt.max_layers
         nbytes = (dmpt_workspace_bytes_fields(self.n, self.num_fields) if self.num_fields > 1
                   else dmpt_workspace_bytes(self.n, self.order))
@@ -292,6 +296,8 @@ class Dmpt:
                 continue                # ground-state mode takes no perturbation
             if m is None or not (m.is_cuda and m.dtype == t.float32 and m.dim() == 2 and m.stride(1) == 1):
                 raise DmptError(DMPT_EINVAL, "set_hamiltonian", "need row-major fp32 CUDA matrices")
+        if h1 is not None and h1.stride(0) != h0.stride(0):
+            raise DmptError(DMPT_EINVAL, "set_hamiltonian", "h0 and h1 need the same leading dimension")
         self._h = (h0, h1)          # keep the storage alive
         dmpt_set_hamiltonian(self.ctx, h0.data_ptr(), h1.data_ptr() if h1 is not None else 0, h0.stride(0), n_occ)
 
@@ -321,6 +327,15 @@ class Dmpt:
                           fro_err3=list(bufs["fro_err3"][:nl]) if self.num_fields > 2 else [],
                           layers_d2=r.layers_d2, layers_d3=r.layers_d3, d0=d0, d1=d1, d2=d2)
 
+    def _check_outputs(self, where, cuda, *mats):
+        """The C ABI takes ONE leading dimension for all outputs: refuse views that disagree."""
+        t = self.torch
+        ms = [m for m in mats if m is not None]
+        for m in ms:
+            if not (m.is_cuda == cuda and m.dtype == t.float32 and m.dim() == 2 and m.stride(1) == 1
+                    and m.stride(0) == ms[0].stride(0) and m.shape[0] >= self.n and m.shape[1] >= self.n):
+                raise DmptError(DMPT_EINVAL, where, "outputs must be row-major fp32 matrices with one leading dimension")
+
     def run(self, out=None, check=True) -> DmptResult:
         t = self.torch
         n = self.n
@@ -335,6 +350,7 @@ class Dmpt:
             d2 = out[2]
         else:
             d2 = t.empty((n, n), dtype=t.float32, device=self.device)
+        self._check_outputs("run", True, d0, d1, d2)
         r, bufs = self._new_result()
         rc = dmpt_run(self.ctx, d0.data_ptr(), d1.data_ptr() if d1 is not None else 0,
                       d2.data_ptr() if d2 is not None else 0, d0.stride(0), r)
@@ -378,6 +394,9 @@ class Dmpt:
             d2 = out[2]
         else:
             d2 = t.empty((n, n), dtype=t.float32, pin_memory=True)
+        if h1 is not None and h1.stride(0) != h0.stride(0):
+            raise DmptError(DMPT_EINVAL, "run_host", "h0 and h1 need the same leading dimension")
+        self._check_outputs("run_host", False, d0, d1, d2)
         r, bufs = self._new_result()
         rc = dmpt_run_host(self.ctx, h0.data_ptr(), h1.data_ptr() if h1 is not None else 0, h0.stride(0), n_occ,
                            d0.data_ptr(), d1.data_ptr() if d1 is not None else 0,

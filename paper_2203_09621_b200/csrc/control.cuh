@@ -52,6 +52,8 @@ struct DmptCtl {
     int e1_out;     // scale for the split of S1_n
     int e2_in, e2_out;
     int e3_in, e3_out;
+    int p1, p2, p3; // prescale exponents: slot k holds 2^pk times the true response iterate (0 unless |H1|/W is
+                    // outside [2^-30, 2^30]; at order 2 slot 2 then holds 2^(2 p1) S2)
     // ---- state of Algorithms 1-3
     int conv0, conv1, conv2, conv3;
     int n_c, n_c1, n_c2, n_c3;
@@ -87,7 +89,10 @@ __device__ __forceinline__ int scale_exponent(double m) {
     if (!(m > 0.0) || !isfinite(m)) return 0;
     int e;
     frexp(m, &e);          // m = f * 2^e, f in [0.5, 1)  ->  m in [2^(e-1), 2^e)
-    return 4 - e;          // m * 2^(4-e) in [8, 16)
+    e = 4 - e;             // m * 2^(4-e) in [8, 16)
+    // every factor 2^(+-e), 2^(+-2e) of the layer epilogue must stay a normal fp32 number; the prescale of
+    // dmpt_bounds_to_ctl_kernel keeps |e| far inside this range on every input
+    return e < -48 ? -48 : (e > 48 ? 48 : e);
 }
 
 // Decide layer n = ctl.layer from N_S, N_X (PAPER.md:499-505 and Algorithm 2).

@@ -37,7 +37,7 @@ struct Carve {
 
 struct Layout {
     int n, n_pad, order, nfields, num_tiles;
-    size_t ctl, bounds, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, fro3, partials, partials2, tiles, tiles_full;
+    size_t ctl, bounds, h1max, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, fro3, partials, partials2, tiles, tiles_full;
     size_t s0, s1[2], s2[2], s3[2];
     size_t h[2][8];          // [buffer][S0hi, S0lo, S1hi, S1lo, slot-2 hi, lo, slot-3 hi, lo]
     size_t stage_h0, stage_h1;
@@ -66,6 +66,7 @@ Layout make_layout(int n, int order, int nfields) {
     Carve c;
     L.ctl = c.take(sizeof(DmptCtl));
     L.bounds = c.take(2 * sizeof(long long));
+    L.h1max = c.take(4 * sizeof(unsigned int));
     L.s2_est = c.take(sizeof(unsigned long long));
     L.sigma = c.take(kMaxLayersCap * sizeof(int));
     L.tr_s = c.take(kMaxLayersCap * sizeof(double));
@@ -449,6 +450,41 @@ static int elementwise_grid(const dmpt_ctx* ctx, long long work_items, int threa
     return (int)blocks;
 }
 
+// a2 + a3 fused (dmpt_transform_split_kernel): S0, S1_f and their first operand splits in one pass over H0, H1_f.
+static int launch_transform_split(dmpt_ctx* ctx, const float* d_h0, const H1Ptrs& h1p, int ld, int nf, int* grid_out) {
+    const Layout& L = ctx->L;
+    const int np = L.n_pad;
+    TransformArgs ta{};
+    ta.h0 = d_h0;
+    ta.n = ctx->n;
+    ta.ld = ld;
+    ta.n_pad = np;
+    ta.s0_shift = ctx->s0_shift;
+    ta.s0 = ctx->lp.s0;
+    ta.mh = ctx->lp.h[0][0];
+    ta.ml = ctx->lp.h[0][1];
+    float* s1dst[3] = {ctx->lp.s1[0], ctx->lp.s2[0], ctx->lp.s3[0]};
+    for (int f = 0; f < nf; ++f) {
+        ta.h1[f] = h1p.p[f];
+        ta.s1[f] = s1dst[f];
+        ta.yh[f] = ctx->lp.h[0][2 + 2 * f];
+        ta.yl[f] = ctx->lp.h[0][3 + 2 * f];
+    }
+    ta.ctl = ctx->at<DmptCtl>(L.ctl);
+    ta.partials = ctx->at<double>(L.partials);
+    const int grid = elementwise_grid(ctx, (long long)np * 256, 256);       // block per row, 8 blocks per SM at most
+    *grid_out = grid;
+    cudaStream_t st = ctx->stream;
+    switch (nf) {
+        case 0: dmpt_transform_split_kernel<0><<<grid, 256, 0, st>>>(ta); break;
+        case 1: dmpt_transform_split_kernel<1><<<grid, 256, 0, st>>>(ta); break;
+        case 2: dmpt_transform_split_kernel<2><<<grid, 256, 0, st>>>(ta); break;
+        default: dmpt_transform_split_kernel<3><<<grid, 256, 0, st>>>(ta); break;
+    }
+    CK(cudaGetLastError());
+    return DMPT_OK;
+}
+
 // Everything from the spectral bounds to the last layer; leaves the result in the workspace.
 // `h_d0_early` (dmpt_run_host only): S0 is final once Algorithm 2 fired, two to four layers before the run
 // ends, so its read-back to the host is started on a side stream as soon as the host sees ctl.conv0 and
@@ -462,33 +498,31 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     long long* bounds = ctx->at<long long>(L.bounds);
     double* partials = ctx->at<double>(L.partials);
 
-    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    unsigned int* h1max = ctx->at<unsigned int>(L.h1max);
+    const int nf = ctx->opt.order == 0 ? 0 : ctx->opt.num_fields;
+    H1Ptrs h1p{{nf >= 1 ? d_h1 : nullptr, nf >= 2 ? ctx->d_h1x[0] : nullptr, nf >= 3 ? ctx->d_h1x[1] : nullptr}};
+
+    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds, h1max);
     CK(cudaGetLastError());
-    if (!ctx->opt.bounds) {
+    if (!ctx->opt.bounds || nf > 0) {
+        // a1: Gershgorin discs of H0 and, in the same pass, max|H1_f| (the scale of the first split of S1_0)
         const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
-        dmpt_gershgorin_kernel<<<grid, 256, 0, st>>>(d_h0, n, ld, bounds);
+        dmpt_gershgorin_kernel<<<grid, 256, 0, st>>>(ctx->opt.bounds ? nullptr : d_h0, h1p, n, ld, bounds, h1max);
         CK(cudaGetLastError());
         ++*launches;
     }
-    dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, ctl, ctx->opt.bounds, ctx->opt.eps_min, ctx->opt.eps_max);
+    dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, h1max, ctl, ctx->lp.pb, ctx->opt.bounds, ctx->opt.eps_min,
+                                                ctx->opt.eps_max);
     CK(cudaGetLastError());
     CK(cudaEventRecord(ctx->ev_t[4], st));
-    const int tgrid = elementwise_grid(ctx, (long long)np * (np / 4), 256);
-    dmpt_transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, d_h1, n, ld, np, ctx->lp.s0, ctx->lp.s1[0], ctl, partials);
-    CK(cudaGetLastError());
+    // a2 + a3: one pass writes S0, S1_f (fp32) and their first operand splits
+    int tgrid = 0;
+    int rc0 = launch_transform_split(ctx, d_h0, h1p, ld, nf, &tgrid);
+    if (rc0) return rc0;
     dmpt_control_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.logs, ctx->lp.pb, partials, tgrid);
     CK(cudaGetLastError());
     CK(cudaEventRecord(ctx->ev_t[5], st));
-    const long long c8 = (long long)np * np / 8;
-    const int sgrid = elementwise_grid(ctx, c8, 256);
-    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
-    CK(cudaGetLastError());
-    if (ctx->opt.order >= 1) {      // order 0 (ground state only) has no response operands
-        dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
-        CK(cudaGetLastError());
-        ++*launches;
-    }
-    *launches += 5;
+    *launches += 4;
     if (ctx->opt.order == 2) {      // S2_0 = 0 (H2 = 0): fp32 iterate and its operands
         const size_t np2 = (size_t)np * np;
         CK(cudaMemsetAsync(ctx->lp.s2[0], 0, np2 * 4, st));
@@ -501,19 +535,6 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
         dmpt_s2_scale_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, est);
         CK(cudaGetLastError());
         *launches += 2;
-    }
-    for (int f = 1; f < ctx->opt.num_fields; ++f) {
-        // fields 2, 3 share H0: the transform kernel is run again for (H0, H1_f) - it rewrites S0 with the
-        // same values and leaves S1 of the field in response slot f + 1 - then the slot's first scale and split
-        float* dst = f == 1 ? ctx->lp.s2[0] : ctx->lp.s3[0];
-        dmpt_transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, ctx->d_h1x[f - 1], n, ld, np, ctx->lp.s0, dst, ctl, partials);
-        CK(cudaGetLastError());
-        dmpt_field_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, tgrid, f + 1);
-        CK(cudaGetLastError());
-        dmpt_split_kernel<<<sgrid, 256, 0, st>>>(dst, (int)np, ctx->lp.h[0][2 + 2 * f], ctx->lp.h[0][3 + 2 * f], ctl,
-                                                 f + 1, ctx->s0_shift, 0);
-        CK(cudaGetLastError());
-        *launches += 3;
     }
     CK(cudaEventRecord(ctx->ev_t[1], st));
 
@@ -598,6 +619,12 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
                 CK(cudaMemcpy(res->fro_err2, ctx->at<double>(L.fro2), nl * sizeof(double), cudaMemcpyDeviceToHost));
             if (res->fro_err3 && ctx->opt.num_fields > 2)
                 CK(cudaMemcpy(res->fro_err3, ctx->at<double>(L.fro3), nl * sizeof(double), cudaMemcpyDeviceToHost));
+            // the norms were taken on the prescaled iterates (DmptCtl::p1..p3; 0 in all but extreme cases)
+            const int pw[3] = {c.p1, ctx->opt.order == 2 ? 2 * c.p1 : c.p2, c.p3};
+            double* logs[3] = {res->fro_err1, res->fro_err2, res->fro_err3};
+            for (int k = 0; k < 3; ++k)
+                if (logs[k] && pw[k] != 0 && (k == 0 || ctx->opt.order == 2 || ctx->opt.num_fields > k))
+                    for (int i = 0; i < nl; ++i) logs[k][i] = ldexp(logs[k][i], -pw[k]);
         }
     }
     return status;
@@ -607,6 +634,25 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
 static int fetch_ctl(dmpt_ctx* ctx) {
     CK(cudaMemcpyAsync(ctx->h_ctl, ctx->at<DmptCtl>(ctx->L.ctl), sizeof(DmptCtl), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
+    return DMPT_OK;
+}
+
+// Undo the prescale of the response iterates (DmptCtl::p1..p3, nonzero only for a perturbation far outside
+// fp16's reach) on the accepted buffers, before they are copied out.  Needs ctx->h_ctl (fetch_ctl).
+static int unscale_outputs(dmpt_ctx* ctx, int* launches) {
+    const DmptCtl& c = *ctx->h_ctl;
+    const int np = ctx->L.n_pad;
+    const int order = ctx->opt.order, nf = ctx->opt.num_fields;
+    float* buf[3] = {order >= 1 ? ctx->lp.s1[c.s1_buf & 1] : nullptr,
+                     (order == 2 || nf >= 2) ? ctx->lp.s2[c.s2_buf & 1] : nullptr,
+                     nf >= 3 ? ctx->lp.s3[c.s3_buf & 1] : nullptr};
+    const int pw[3] = {c.p1, order == 2 ? 2 * c.p1 : c.p2, c.p3};
+    for (int k = 0; k < 3; ++k)
+        if (buf[k] && pw[k] != 0) {
+            dmpt_unscale_kernel<<<elementwise_grid(ctx, (long long)np * np, 256), 256, 0, ctx->stream>>>(buf[k], np, -pw[k]);
+            CK(cudaGetLastError());
+            ++*launches;
+        }
     return DMPT_OK;
 }
 
@@ -621,6 +667,7 @@ extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, in
     int rc = run_core(ctx, ctx->d_h0, ctx->d_h1, ctx->ld_in, &launches);
     if (rc) return rc;
     if ((rc = fetch_ctl(ctx))) return rc;
+    if ((rc = unscale_outputs(ctx, &launches))) return rc;
     CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
     if (ctx->opt.order >= 1)
         CK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
@@ -645,6 +692,7 @@ extern "C" int dmpt_run_fields(dmpt_ctx* ctx, float* d_d0, float* const* d_d1, i
     int rc = run_core(ctx, ctx->d_h0, ctx->d_h1, ctx->ld_in, &launches);
     if (rc) return rc;
     if ((rc = fetch_ctl(ctx))) return rc;
+    if ((rc = unscale_outputs(ctx, &launches))) return rc;
     const DmptCtl& c = *ctx->h_ctl;
     const float* src[3] = {ctx->lp.s1[c.s1_buf & 1], nf > 1 ? ctx->lp.s2[c.s2_buf & 1] : nullptr,
                            nf > 2 ? ctx->lp.s3[c.s3_buf & 1] : nullptr};
@@ -675,6 +723,7 @@ extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1
     int rc = run_core(ctx, s_h0, ctx->opt.order >= 1 ? s_h1 : nullptr, (int)n, &launches, h_d0, ld_out, &early);
     if (rc) return rc;
     if ((rc = fetch_ctl(ctx))) return rc;
+    if ((rc = unscale_outputs(ctx, &launches))) return rc;
     if (early)
         CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_side, 0));       // D0 went out while the last layers ran
     else
@@ -716,7 +765,7 @@ __global__ void single_shot_init_kernel(DmptCtl* ctl, DmptProblem pb, const doub
 extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float* d_s1, int ld,
                                    float* d_x0, float* d_x1, int ld_out) {
     if (!ctx || !d_s0 || !d_s1 || !d_x0 || !d_x1) return DMPT_EINVAL;
-    if (ld < ctx->n || ld_out < ctx->n) return DMPT_EINVAL;
+    if (ld < ctx->n || ld_out < ctx->n || ctx->opt.order < 1) return DMPT_EINVAL;      // order 0 forms no X1
     const Layout& L = ctx->L;
     const size_t n = ctx->n, np = L.n_pad;
     cudaStream_t st = ctx->stream;
@@ -836,9 +885,10 @@ extern "C" int dmpt_inverse_factor(dmpt_ctx* ctx, const float* d_s, int ld, floa
     float* x = ctx->at<float>(L.stage_h0);       // n x n scratch (the staging buffers of dmpt_run_host)
     float* t = ctx->at<float>(L.stage_h1);
     // Z_0 = I / sqrt(eps_max): S is positive definite, so X_0 = S / eps_max has its spectrum in (0, 1]
-    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds, ctx->at<unsigned int>(L.h1max));
     CK(cudaGetLastError());
-    dmpt_gershgorin_kernel<<<elementwise_grid(ctx, (long long)n * 32, 256), 256, 0, st>>>(d_s, n, ld, bounds);
+    dmpt_gershgorin_kernel<<<elementwise_grid(ctx, (long long)n * 32, 256), 256, 0, st>>>(
+        d_s, H1Ptrs{{nullptr, nullptr, nullptr}}, n, ld, bounds, ctx->at<unsigned int>(L.h1max));
     CK(cudaGetLastError());
     long long hb[2];
     CK(cudaMemcpyAsync(hb, bounds, sizeof hb, cudaMemcpyDeviceToHost, st));
@@ -886,10 +936,11 @@ extern "C" int dmpt_spectral_bounds(dmpt_ctx* ctx, const float* d_h0, int ld, do
     cudaStream_t st = ctx->stream;
     DmptCtl* ctl = ctx->at<DmptCtl>(ctx->L.ctl);
     long long* bounds = ctx->at<long long>(ctx->L.bounds);
-    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    unsigned int* h1max = ctx->at<unsigned int>(ctx->L.h1max);
+    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds, h1max);
     CK(cudaGetLastError());
     const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
-    dmpt_gershgorin_kernel<<<grid, 256, 0, st>>>(d_h0, n, ld, bounds);
+    dmpt_gershgorin_kernel<<<grid, 256, 0, st>>>(d_h0, H1Ptrs{{nullptr, nullptr, nullptr}}, n, ld, bounds, h1max);
     CK(cudaGetLastError());
     long long hb[2];
     CK(cudaMemcpyAsync(hb, bounds, sizeof hb, cudaMemcpyDeviceToHost, st));
@@ -911,13 +962,28 @@ extern "C" int dmpt_initial_transform(dmpt_ctx* ctx, const float* d_h0, const fl
     DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
     long long* bounds = ctx->at<long long>(L.bounds);
     double* partials = ctx->at<double>(L.partials);
-    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds);
+    // the same two launches dmpt_run makes: max|H1| (scale of the first split), then the fused a2 + a3 kernel
+    unsigned int* h1max = ctx->at<unsigned int>(L.h1max);
+    const H1Ptrs h1p{{d_h1, nullptr, nullptr}};
+    dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds, h1max);
     CK(cudaGetLastError());
-    dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, ctl, 1, eps_min, eps_max);
+    dmpt_gershgorin_kernel<<<elementwise_grid(ctx, (long long)n * 32, 256), 256, 0, st>>>(nullptr, h1p, (int)n, ld, bounds,
+                                                                                         h1max);
     CK(cudaGetLastError());
-    const int tgrid = elementwise_grid(ctx, (long long)np * (np / 4), 256);
-    dmpt_transform_kernel<<<tgrid, 256, 0, st>>>(d_h0, d_h1, (int)n, ld, (int)np, ctx->lp.s0, ctx->lp.s1[0], ctl, partials);
+    DmptProblem pb1 = ctx->lp.pb;
+    pb1.order = 1;
+    pb1.nfields = 1;
+    dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, h1max, ctl, pb1, 1, eps_min, eps_max);
     CK(cudaGetLastError());
+    int tgrid = 0;
+    int rc = launch_transform_split(ctx, d_h0, h1p, ld, 1, &tgrid);
+    if (rc) return rc;
+    if ((rc = fetch_ctl(ctx))) return rc;
+    if (ctx->h_ctl->p1 != 0) {       // hand back S1 itself, not the prescaled iterate
+        dmpt_unscale_kernel<<<elementwise_grid(ctx, (long long)np * np, 256), 256, 0, st>>>(ctx->lp.s1[0], (int)np,
+                                                                                           -ctx->h_ctl->p1);
+        CK(cudaGetLastError());
+    }
     CK(cudaMemcpy2DAsync(d_s0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpy2DAsync(d_s1, (size_t)ld_out * 4, ctx->lp.s1[0], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     std::vector<double> hp((size_t)tgrid * 3);

@@ -46,36 +46,77 @@ __device__ __forceinline__ T warp_max(T v) {
     return v;
 }
 
+// hi = fp16(2^e x), lo = fp16(2^e x - hi), round-to-nearest-even (Eq. 13 after an exact
+// power-of-two scale, readings R12/R17)
+__device__ __forceinline__ void split_scaled(float x, float scale, __half& hi, __half& lo) {
+    const float t = x * scale;              // exact: scale is a power of two (barring overflow)
+    hi = __float2half_rn(t);
+    lo = __float2half_rn(t - __half2float(hi));
+}
+
 // ---------------------------------------------------------------------------------------------
 // a1  Gershgorin discs: one warp per row, shuffle reduction of sum_j |H0_ij|,
 //     eps_min = min_i (H0_ii - r_i), eps_max = max_i (H0_ii + r_i), r_i = sum_{j != i} |H0_ij|.
-//     bounds[0], bounds[1]: ordered-int encodings, initialised to +inf / -inf by the host.
+//     bounds[0], bounds[1]: ordered-int encodings, initialised to +inf / -inf by dmpt_reset_state_kernel.
+//     The same pass streams the perturbation(s) and leaves max|H1_f| in h1max[f] (bit pattern of a
+//     non-negative float, ordered like an unsigned integer): the power-of-two scale of the first split of
+//     S1_0 = -H1/W is then known BEFORE the fused transform + split kernel runs (reading R12).
+//     h0 == nullptr (caller-supplied bounds) skips the discs; h1[f] == nullptr skips that field.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) dmpt_gershgorin_kernel(const float* __restrict__ h0, int n, int ld,
-                                                         long long* __restrict__ bounds) {
+struct H1Ptrs {
+    const float* p[3];
+};
+
+__device__ __forceinline__ float absmax4(float m, const float4& v) {
+    return fmaxf(fmaxf(m, fmaxf(fabsf(v.x), fabsf(v.y))), fmaxf(fabsf(v.z), fabsf(v.w)));
+}
+
+__global__ void __launch_bounds__(256) dmpt_gershgorin_kernel(const float* __restrict__ h0, H1Ptrs h1, int n, int ld,
+                                                              long long* __restrict__ bounds,
+                                                              unsigned int* __restrict__ h1max) {
     const int warps_per_block = blockDim.x >> 5;
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     double lo = INFINITY, hi = -INFINITY;
-    const bool vec = ((ld & 3) == 0) && ((reinterpret_cast<uintptr_t>(h0) & 15) == 0);
+    float m1[3] = {0.f, 0.f, 0.f};
+    bool vec = (ld & 3) == 0 && (reinterpret_cast<uintptr_t>(h0) & 15) == 0;
+#pragma unroll
+    for (int f = 0; f < 3; ++f) vec = vec && (reinterpret_cast<uintptr_t>(h1.p[f]) & 15) == 0;
     for (int row = blockIdx.x * warps_per_block + warp; row < n; row += gridDim.x * warps_per_block) {
-        const float* p = h0 + (size_t)row * ld;
+        const size_t off = (size_t)row * ld;
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
         int j = 0;
         if (vec) {
             const int n4 = n & ~3;
             for (j = lane * 4; j < n4; j += 128) {
-                float4 v = ldg_stream4(p + j);
-                a0 += fabsf(v.x); a1 += fabsf(v.y); a2 += fabsf(v.z); a3 += fabsf(v.w);
+                if (h0) {
+                    const float4 v = ldg_stream4(h0 + off + j);
+                    a0 += fabsf(v.x); a1 += fabsf(v.y); a2 += fabsf(v.z); a3 += fabsf(v.w);
+                }
+#pragma unroll
+                for (int f = 0; f < 3; ++f)
+                    if (h1.p[f]) m1[f] = absmax4(m1[f], ldg_stream4(h1.p[f] + off + j));
             }
             j = n4;
         }
-        for (j += lane; j < n; j += 32) a0 += fabsf(p[j]);
-        double s = warp_sum((double)a0 + (double)a1 + (double)a2 + (double)a3);
-        const double d = (double)p[row];
-        const double r = s - fabs(d);
-        lo = fmin(lo, d - r);
-        hi = fmax(hi, d + r);
+        for (j += lane; j < n; j += 32) {
+            if (h0) a0 += fabsf(h0[off + j]);
+#pragma unroll
+            for (int f = 0; f < 3; ++f)
+                if (h1.p[f]) m1[f] = fmaxf(m1[f], fabsf(h1.p[f][off + j]));
+        }
+        if (h0) {
+            double s = warp_sum((double)a0 + (double)a1 + (double)a2 + (double)a3);
+            const double d = (double)h0[off + row];
+            const double r = s - fabs(d);
+            lo = fmin(lo, d - r);
+            hi = fmax(hi, d + r);
+        }
+    }
+#pragma unroll
+    for (int f = 0; f < 3; ++f) {
+        const float m = warp_max(m1[f]);
+        if (lane == 0 && m > 0.f) atomicMax(&h1max[f], __float_as_uint(m));     // +inf orders above every finite value
     }
     if (lane == 0 && lo <= hi) {
         atomicMin(&bounds[0], dbl_to_ordered(lo));
@@ -84,76 +125,140 @@ __global__ void __launch_bounds__(256) dmpt_gershgorin_kernel(const float* __res
 }
 
 // ---------------------------------------------------------------------------------------------
-// a2  Initial normalisation layer (Eq. 34, 493):
-//        S0 = (eps_max I - H0)/W,  S1 = -H1/W,  W = eps_max - eps_min,
-//     written to n_pad x n_pad fp32 workspace matrices (zero outside n x n), together with the
-//     first reductions: Tr S0, ||S0||_F^2, max|S1| as per-block partials (summed in a fixed order
-//     by dmpt_control_init_kernel).  Each element is formed in fp64 and rounded once to fp32.
+// a2 + a3 fused.  Initial normalisation layer (Eq. 34, 493):
+//        S0 = (eps_max I - H0)/W,  S1_f = -H1_f/W,  W = eps_max - eps_min,
+//     each element formed in fp64 and rounded once to fp32, written to the n_pad x n_pad fp32 workspace
+//     matrices (zero outside n x n) TOGETHER WITH the first operand split (Eq. 13, 302-307):
+//        (Mhi, Mlo) = split(2^a (S0 - I/2)),   (S1hi, S1lo)_f = split(2^e_f S1_f)
+//     (residual form and power-of-two scales: DESIGN.md R12, R17).  Algorithmic bytes per element:
+//     4 (1 + NF) read + (4 + 4)(1 + NF) written = 24 at one field, against 32 for transform + two splits.
+//     Partials per block: Tr S0, ||S0||_F^2 (summed in a fixed order by dmpt_control_init_kernel).
+//     NF = 0: ground-state mode (no perturbation).  The scales e_f and the optional prescale 2^p_f of a
+//     perturbation outside [2^-30, 2^30] come from DmptCtl (dmpt_bounds_to_ctl_kernel).
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) dmpt_transform_kernel(const float* __restrict__ h0,
-                                                        const float* __restrict__ h1, int n, int ld,
-                                                        int n_pad, float* __restrict__ s0,
-                                                        float* __restrict__ s1,
-                                                        const DmptCtl* __restrict__ ctl,
-                                                        double* __restrict__ partials /* [grid][3] */) {
-    const double emax = ctl->eps_max;
-    const double inv_w = 1.0 / (ctl->eps_max - ctl->eps_min);
-    const int q_per_row = n_pad >> 2;
-    const bool with_h1 = h1 != nullptr;        // order 0 (ground state only): S1 = 0
-    const bool vec = ((ld & 3) == 0) && ((reinterpret_cast<uintptr_t>(h0) & 15) == 0) &&
-                     ((reinterpret_cast<uintptr_t>(h1) & 15) == 0);
-    double tr = 0.0, fro = 0.0;
-    float mx = 0.f;
-    // block per row (grid-stride), threads along the row: no 64-bit division per element
-    for (int row = blockIdx.x; row < n_pad; row += gridDim.x)
-    for (int qc = threadIdx.x; qc < q_per_row; qc += blockDim.x) {
-        const int col = qc << 2;
-        float a[4] = {0.f, 0.f, 0.f, 0.f}, b[4] = {0.f, 0.f, 0.f, 0.f};
-        if (row < n) {
-            if (vec && col + 3 < n) {
-                float4 va = ldg_stream4(h0 + (size_t)row * ld + col);
-                float4 vb = with_h1 ? ldg_stream4(h1 + (size_t)row * ld + col) : make_float4(0.f, 0.f, 0.f, 0.f);
-                a[0] = va.x; a[1] = va.y; a[2] = va.z; a[3] = va.w;
-                b[0] = vb.x; b[1] = vb.y; b[2] = vb.z; b[3] = vb.w;
-            } else {
+struct TransformArgs {
+    const float* h0;
+    const float* h1[3];
+    int n, ld, n_pad, s0_shift;
+    float* s0;
+    float* s1[3];
+    __half* mh;
+    __half* ml;
+    __half* yh[3];
+    __half* yl[3];
+    const DmptCtl* ctl;
+    double* partials;      // [grid][3]: Tr S0, ||S0||_F^2, unused
+};
+
+template <int NF>
+__global__ void __launch_bounds__(256) dmpt_transform_split_kernel(const TransformArgs a) {
+    const DmptCtl c = *a.ctl;
+    const double emax = c.eps_max;
+    const double inv_w = 1.0 / (c.eps_max - c.eps_min);
+    double inv_wf[3];
+    float scale1[3];
+    const int e_in[3] = {c.e1_in, c.e2_in, c.e3_in};
+    const int pre[3] = {c.p1, c.p2, c.p3};
 #pragma unroll
-                for (int t = 0; t < 4; ++t)
-                    if (col + t < n) {
-                        a[t] = h0[(size_t)row * ld + col + t];
-                        b[t] = with_h1 ? h1[(size_t)row * ld + col + t] : 0.f;
+    for (int f = 0; f < 3; ++f) {
+        inv_wf[f] = ldexp(inv_w, pre[f]);          // exact; pre = 0 unless |H1|/W is far outside fp16's reach
+        scale1[f] = exp2f((float)e_in[f]);
+    }
+    const float scale0 = exp2f((float)a.s0_shift);
+    const int n = a.n, ld = a.ld, n_pad = a.n_pad;
+    const int c8_per_row = n_pad >> 3;
+    bool vec = (ld & 3) == 0 && (reinterpret_cast<uintptr_t>(a.h0) & 15) == 0;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) vec = vec && (reinterpret_cast<uintptr_t>(a.h1[f]) & 15) == 0;
+    double tr = 0.0, fro = 0.0;
+    // block per row (grid-stride), 8 consecutive columns per thread: 128-bit loads and stores throughout
+    for (int row = blockIdx.x; row < n_pad; row += gridDim.x)
+        for (int c8 = threadIdx.x; c8 < c8_per_row; c8 += blockDim.x) {
+            const int col = c8 << 3;
+            float x0[8], x1[NF > 0 ? NF : 1][8];
+#pragma unroll
+            for (int t = 0; t < 8; ++t) {
+                x0[t] = 0.f;
+#pragma unroll
+                for (int f = 0; f < NF; ++f) x1[f][t] = 0.f;
+            }
+            if (row < n && col < n) {
+                const size_t off = (size_t)row * ld + col;
+                if (vec && col + 7 < n) {
+                    const float4 u0 = ldg_stream4(a.h0 + off), u1 = ldg_stream4(a.h0 + off + 4);
+                    x0[0] = u0.x; x0[1] = u0.y; x0[2] = u0.z; x0[3] = u0.w;
+                    x0[4] = u1.x; x0[5] = u1.y; x0[6] = u1.z; x0[7] = u1.w;
+#pragma unroll
+                    for (int f = 0; f < NF; ++f) {
+                        const float4 w0 = ldg_stream4(a.h1[f] + off), w1 = ldg_stream4(a.h1[f] + off + 4);
+                        x1[f][0] = w0.x; x1[f][1] = w0.y; x1[f][2] = w0.z; x1[f][3] = w0.w;
+                        x1[f][4] = w1.x; x1[f][5] = w1.y; x1[f][6] = w1.z; x1[f][7] = w1.w;
                     }
+                } else {
+#pragma unroll
+                    for (int t = 0; t < 8; ++t)
+                        if (col + t < n) {
+                            x0[t] = a.h0[off + t];
+#pragma unroll
+                            for (int f = 0; f < NF; ++f) x1[f][t] = a.h1[f][off + t];
+                        }
+                }
+            }
+            float o0[8];
+            __align__(16) __half hh[8];
+            __align__(16) __half ll[8];
+            float fsum[2] = {0.f, 0.f};        // fp32 per four elements, fp64 beyond
+#pragma unroll
+            for (int t = 0; t < 8; ++t) {
+                const bool inside = row < n && col + t < n;
+                const bool dg = col + t == row;
+                o0[t] = inside ? (float)(((dg ? emax : 0.0) - (double)x0[t]) * inv_w) : 0.f;
+                if (inside && dg) tr += (double)o0[t];
+                fsum[t >> 2] = fmaf(o0[t], o0[t], fsum[t >> 2]);
+                split_scaled(dg ? o0[t] - 0.5f : o0[t], scale0, hh[t], ll[t]);     // operands hold M = S0 - I/2
+            }
+            fro += (double)fsum[0] + (double)fsum[1];
+            const size_t i8 = (size_t)row * n_pad + col;
+            *reinterpret_cast<float4*>(a.s0 + i8) = make_float4(o0[0], o0[1], o0[2], o0[3]);
+            *reinterpret_cast<float4*>(a.s0 + i8 + 4) = make_float4(o0[4], o0[5], o0[6], o0[7]);
+            *reinterpret_cast<uint4*>(a.mh + i8) = *reinterpret_cast<const uint4*>(hh);
+            *reinterpret_cast<uint4*>(a.ml + i8) = *reinterpret_cast<const uint4*>(ll);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+                float o1[8];
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    const bool inside = row < n && col + t < n;
+                    o1[t] = inside ? (float)(-(double)x1[f][t] * inv_wf[f]) : 0.f;
+                    split_scaled(o1[t], scale1[f], hh[t], ll[t]);
+                }
+                *reinterpret_cast<float4*>(a.s1[f] + i8) = make_float4(o1[0], o1[1], o1[2], o1[3]);
+                *reinterpret_cast<float4*>(a.s1[f] + i8 + 4) = make_float4(o1[4], o1[5], o1[6], o1[7]);
+                *reinterpret_cast<uint4*>(a.yh[f] + i8) = *reinterpret_cast<const uint4*>(hh);
+                *reinterpret_cast<uint4*>(a.yl[f] + i8) = *reinterpret_cast<const uint4*>(ll);
             }
         }
-        float o0[4], o1[4];
-        float fsum = 0.f;
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-            const bool inside = row < n && col + t < n;
-            const double diag = (inside && col + t == row) ? emax : 0.0;
-            o0[t] = inside ? (float)((diag - (double)a[t]) * inv_w) : 0.f;
-            o1[t] = inside ? (float)(-(double)b[t] * inv_w) : 0.f;
-            if (inside && col + t == row) tr += (double)o0[t];
-            fsum = fmaf(o0[t], o0[t], fsum);
-            mx = fmaxf(mx, fabsf(o1[t]));
-        }
-        fro += (double)fsum;
-        *reinterpret_cast<float4*>(s0 + (size_t)row * n_pad + col) = make_float4(o0[0], o0[1], o0[2], o0[3]);
-        *reinterpret_cast<float4*>(s1 + (size_t)row * n_pad + col) = make_float4(o1[0], o1[1], o1[2], o1[3]);
-    }
-    __shared__ double sh[3][8];
+    __shared__ double sh[2][8];
     tr = warp_sum(tr);
     fro = warp_sum(fro);
-    double dmx = warp_max((double)mx);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (lane == 0) { sh[0][warp] = tr; sh[1][warp] = fro; sh[2][warp] = dmx; }
+    if (lane == 0) { sh[0][warp] = tr; sh[1][warp] = fro; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double t = 0.0, f = 0.0, m = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { t += sh[0][w]; f += sh[1][w]; m = fmax(m, sh[2][w]); }
-        partials[blockIdx.x * 3 + 0] = t;
-        partials[blockIdx.x * 3 + 1] = f;
-        partials[blockIdx.x * 3 + 2] = m;
+        double t = 0.0, f = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { t += sh[0][w]; f += sh[1][w]; }
+        a.partials[blockIdx.x * 3 + 0] = t;
+        a.partials[blockIdx.x * 3 + 1] = f;
+        a.partials[blockIdx.x * 3 + 2] = 0.0;
     }
+}
+
+// Undo the prescale 2^p of a response iterate in place (only launched when p != 0: a perturbation whose
+// size is far outside fp16's reach, see dmpt_bounds_to_ctl_kernel).  Exact unless the true value is subnormal.
+__global__ void __launch_bounds__(256) dmpt_unscale_kernel(float* __restrict__ x, int n_pad, int minus_p) {
+    const long long total = (long long)n_pad * n_pad;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x)
+        x[i] = ldexpf(x[i], minus_p);
 }
 
 // zero-padded copy of a caller matrix into an n_pad x n_pad workspace matrix (dmpt_layer_products)
@@ -184,47 +289,78 @@ __global__ void __launch_bounds__(256) dmpt_pad_copy_kernel(const float* __restr
 // Scalar set-up between the transform and the first layer: spectral bounds -> ctl (before the
 // transform), then first reductions -> ctl and the decision for layer 1 (after it).
 // ---------------------------------------------------------------------------------------------
-__global__ void dmpt_reset_state_kernel(DmptCtl* ctl, long long* bounds) {
+__global__ void dmpt_reset_state_kernel(DmptCtl* ctl, long long* bounds, unsigned int* h1max) {
     if (threadIdx.x | blockIdx.x) return;
     DmptCtl c;
     memset(&c, 0, sizeof c);
     *ctl = c;
     bounds[0] = dbl_to_ordered(INFINITY);
     bounds[1] = dbl_to_ordered(-INFINITY);
+    h1max[0] = h1max[1] = h1max[2] = 0u;
 }
 
-__global__ void dmpt_bounds_to_ctl_kernel(const long long* __restrict__ bounds, DmptCtl* ctl, int use_given,
-                                     double eps_min, double eps_max) {
-    if (threadIdx.x | blockIdx.x) return;
-    const double lo = use_given ? eps_min : ordered_to_dbl(bounds[0]);
-    const double hi = use_given ? eps_max : ordered_to_dbl(bounds[1]);
-    ctl->eps_min = lo;
-    ctl->eps_max = hi;
-    const double w = hi - lo;
-    if (!(w > 0.0) || !isfinite(w)) {
-        ctl->done = 1;
-        ctl->status = -4;  // DMPT_EDEGENERATE
-        // keep the transform finite
-        ctl->eps_min = 0.0;
-        ctl->eps_max = 1.0;
-    }
-}
-
-__global__ void dmpt_control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProblem pb,
-                                    const double* __restrict__ partials, int nblocks) {
+// Spectral bounds -> ctl, and for every perturbation the size of S1_0 = -H1/W and the exponent of its first
+// split (reading R12): max|S1_0| = fl32(max|H1| / W) because the rounding is monotone.  A perturbation whose
+// S1_0 lies outside [2^-30, 2^30] is carried with an exact prescale 2^p (max|2^p S1_0| in [1, 2)) so that every
+// power-of-two factor of the layer epilogue stays a normal fp32 number; the run undoes it on the outputs.
+__global__ void dmpt_bounds_to_ctl_kernel(const long long* __restrict__ bounds, const unsigned int* __restrict__ h1max,
+                                          DmptCtl* ctl, DmptProblem pb, int use_given, double eps_min, double eps_max) {
     if (threadIdx.x | blockIdx.x) return;
     DmptCtl c = *ctl;
-    double t = 0.0, f = 0.0, m = 0.0;
-    for (int b = 0; b < nblocks; ++b) {
+    const double lo = use_given ? eps_min : ordered_to_dbl(bounds[0]);
+    const double hi = use_given ? eps_max : ordered_to_dbl(bounds[1]);
+    c.eps_min = lo;
+    c.eps_max = hi;
+    const double w = hi - lo;
+    if (!(w > 0.0) || !isfinite(w)) {
+        c.done = 1;
+        c.status = -4;  // DMPT_EDEGENERATE
+        // keep the transform finite
+        c.eps_min = 0.0;
+        c.eps_max = 1.0;
+    }
+    const double inv_w = 1.0 / (c.eps_max - c.eps_min);
+    const int nslots = pb.order == 0 ? 0 : pb.nfields;
+    int pre[3] = {0, 0, 0}, e[3] = {0, 0, 0};
+    double mx[3] = {0.0, 0.0, 0.0};
+    for (int f = 0; f < nslots; ++f) {
+        const double m = (double)__uint_as_float(h1max[f]) * inv_w;
+        if (!isfinite(m)) {
+            c.done = 1;
+            c.status = -6;  // DMPT_ENUMERIC
+            continue;
+        }
+        if (m > 0.0 && (m < 0x1p-30 || m > 0x1p30)) {
+            int ex;
+            frexp(m, &ex);              // m in [2^(ex-1), 2^ex)
+            pre[f] = 1 - ex;
+        }
+        mx[f] = (double)(float)ldexp(m, pre[f]);
+        e[f] = pb.s1_autoscale ? scale_exponent(mx[f]) : 0;
+    }
+    c.p1 = pre[0]; c.p2 = pre[1]; c.p3 = pre[2];
+    c.s1_max = mx[0]; c.s2_max = mx[1]; c.s3_max = mx[2];
+    c.e1_in = c.e1_out = e[0];
+    c.e2_in = c.e2_out = e[1];
+    c.e3_in = c.e3_out = e[2];
+    *ctl = c;
+}
+
+// First reductions -> ctl and the decision for layer 1.  One warp, fixed summation order.
+__global__ void dmpt_control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProblem pb,
+                                         const double* __restrict__ partials, int nblocks) {
+    if (blockIdx.x || threadIdx.x >= 32) return;
+    double t = 0.0, f = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += 32) {
         t += partials[b * 3 + 0];
         f += partials[b * 3 + 1];
-        m = fmax(m, partials[b * 3 + 2]);
     }
+    t = warp_sum(t);
+    f = warp_sum(f);
+    if (threadIdx.x) return;
+    DmptCtl c = *ctl;
     c.n_s = t;
     c.n_x = f;
-    c.s1_max = m;
-    c.e1_in = c.e1_out = pb.s1_autoscale ? scale_exponent(m) : 0;
-    c.e2_in = c.e2_out = 0;
     c.layer = 1;
     if (!c.done) control_decide(c, logs, pb);
     *ctl = c;
@@ -260,18 +396,6 @@ __global__ void dmpt_s2_scale_init_kernel(DmptCtl* ctl, DmptProblem pb, const un
     ctl->s2_max = m;
     ctl->e2_in = 0;
     ctl->e2_out = pb.s1_autoscale ? scale_exponent(m) : 0;
-}
-
-// Multi-field runs: first scale of response slot 2 or 3 from max|S1_0| of that field (the third of the
-// per-block partials the transform kernel wrote for it).
-__global__ void dmpt_field_init_kernel(DmptCtl* ctl, DmptProblem pb, const double* __restrict__ partials, int nblocks,
-                                       int slot) {
-    if (threadIdx.x | blockIdx.x) return;
-    double m = 0.0;
-    for (int b = 0; b < nblocks; ++b) m = fmax(m, partials[b * 3 + 2]);
-    const int e = pb.s1_autoscale ? scale_exponent(m) : 0;
-    if (slot == 2) { ctl->s2_max = m; ctl->e2_in = ctl->e2_out = e; }
-    else { ctl->s3_max = m; ctl->e3_in = ctl->e3_out = e; }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -319,12 +443,6 @@ __global__ void __launch_bounds__(256) dmpt_zpoly_kernel(const float* __restrict
 //     `which` selects the exponent on the device: 0 -> s0_shift, 1, 2, 3 -> ctl->e1_in, e2_in, e3_in.
 //     With diag_half the matrix split is M = S0 - I/2 (residual form, layer_kernel.cuh).
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void split_scaled(float x, float scale, __half& hi, __half& lo) {
-    const float t = x * scale;              // exact: scale is a power of two (barring overflow)
-    hi = __float2half_rn(t);
-    lo = __float2half_rn(t - __half2float(hi));
-}
-
 __global__ void __launch_bounds__(256) dmpt_split_kernel(const float* __restrict__ x, int n_pad,
                                                          __half* __restrict__ hi, __half* __restrict__ lo,
                                                          const DmptCtl* __restrict__ ctl, int which, int s0_shift,

@@ -276,8 +276,8 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         for (int m = 0; m < 2; ++m) {
             prefetch_tensormap(&p.maps[c.s0_buf][m]);
             prefetch_tensormap(&p.maps[c.s1_buf][2 + m]);
-            if (PASS >= 1) prefetch_tensormap(&p.maps[c.s2_buf][S2H + m]);
-            if (PASS == 2) prefetch_tensormap(&p.maps[c.s3_buf][S3H + m]);
+            if (PASS == 1 || PASS == 2) prefetch_tensormap(&p.maps[c.s2_buf][S2H + m]);       // only maps that were encoded
+            if (PASS == 2 && p.pb.nfields >= 3) prefetch_tensormap(&p.maps[c.s3_buf][S3H + m]);
         }
         for (int s = 0; s < kStages; ++s) {
             mbar_init(full_bar(s), 1);                       // leader's: its producer's arrive + both CTAs' bytes

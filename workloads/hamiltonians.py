@@ -238,6 +238,7 @@ def make_config(index: int, n: int | None = None, device=None, seed: int | None 
         meta["gap"] = float(eps[n_occ] - eps[n_occ - 1])
         meta["mu"] = float(0.5 * (eps[n_occ] + eps[n_occ - 1]))
         meta["spectrum"] = (float(eps[0]), float(eps[-1]))
+        meta["eps"] = np.asarray(eps, dtype=np.float64)      # the constructed spectrum (before the fp32 rounding of H0)
         pos = atom = None
     else:
         if n % 4:
@@ -260,6 +261,7 @@ def make_config(index: int, n: int | None = None, device=None, seed: int | None 
             meta["gap"] = float(eps[n_occ] - eps[n_occ - 1])
             meta["mu"] = float(0.5 * (eps[n_occ] + eps[n_occ - 1]))
             meta["spectrum"] = (float(eps[0]), float(eps[-1]))
+            meta["eps"] = np.asarray(eps, dtype=np.float64)  # spectrum after the scissor shift (before fp32 rounding)
         else:
             meta["gap"] = None
 
