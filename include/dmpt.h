@@ -64,7 +64,11 @@ typedef struct dmpt_options {
     int num_fields;    /* 1 (default; 0 reads as 1) .. 3 perturbations H1_a sharing H0, first order only:      */
                        /* D1_a for each in one run - S0^2 once per layer, S0.S1_a per field (the x, y, z       */
                        /* fields of the polarizability, Eq. 79).  Use the *_fields entry points.  */
-    int reserved[6];   /* must be 0                                                                   */
+    int epilogue_direct; /* 0 (default): the layer kernel's final epilogue goes through shared memory and TMA (old      */
+                       /* iterate in, new iterate and its split out, direct and mirrored, as full lines); 1: every  */
+                       /* thread reads and writes its own row of the tile directly (round 1's path, kept for A/B     */
+                       /* measurements; same arithmetic, bit-identical results)                                      */
+    int reserved[5];   /* must be 0                                                                   */
 } dmpt_options;
 
 typedef struct dmpt_result {

@@ -28,7 +28,7 @@ class DmptOptions(C.Structure):
         ("max_layers", C.c_int), ("order", C.c_int), ("s0_shift", C.c_int),
         ("s1_autoscale", C.c_int), ("bounds", C.c_int),
         ("eps_min", C.c_double), ("eps_max", C.c_double),
-        ("wave_sync", C.c_int), ("num_fields", C.c_int), ("reserved", C.c_int * 6),
+        ("wave_sync", C.c_int), ("num_fields", C.c_int), ("epilogue_direct", C.c_int), ("reserved", C.c_int * 5),
     ]
 
 
@@ -254,7 +254,7 @@ class Dmpt:
     """Owns a dmpt_ctx plus the torch-allocated workspace.  Marshalling only."""
 
     def __init__(self, n, order=1, max_layers=200, s0_shift=-1, s1_autoscale=True, bounds=None,
-                 device="cuda:0", stream=None, wave_sync=True, num_fields=1):
+                 device="cuda:0", stream=None, wave_sync=True, num_fields=1, epilogue_direct=False):
         import torch
 
         self.torch = torch
@@ -270,6 +270,7 @@ class Dmpt:
         opt.s1_autoscale = 1 if s1_autoscale else 0
         opt.wave_sync = 1 if wave_sync else 0
         opt.num_fields = int(num_fields)
+        opt.epilogue_direct = 1 if epilogue_direct else 0
         self.num_fields = int(num_fields)
         if bounds is not None:
             opt.bounds = 1

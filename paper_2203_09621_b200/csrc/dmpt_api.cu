@@ -102,15 +102,21 @@ Layout make_layout(int n, int order, int nfields) {
 
 // Launch order of the upper-triangular pair tiles: bands of `band` pair rows, column by column inside
 // a band, so that the ~#SM/2 pair tiles in flight share few row panels (L2 reuse of the operand panels).
+// The pair tiles that hold a diagonal block ((IP, 2 IP) and (IP, 2 IP + 1)) come last, together: their final
+// epilogue is the element-wise one (the mirror of a diagonal block lies inside the block), several times slower
+// than the TMA epilogue of the other tiles, and with wave-aligned producers every CTA of a wave waits for the
+// slowest tile in it - spread over the bands, one such tile per wave held all 74 pairs back on every wave.
 std::vector<uint32_t> make_tile_order(int nb, int band) {
-    std::vector<uint32_t> t;
+    std::vector<uint32_t> t, diag;
     t.reserve(num_tiles_for(nb));
     const int nbp = nb / 2;
     for (int b0 = 0; b0 < nbp; b0 += band) {
         const int b1 = b0 + band < nbp ? b0 + band : nbp;
         for (int j = 2 * b0; j < nb; ++j)
-            for (int ip = b0; ip < b1 && 2 * ip <= j; ++ip) t.push_back((uint32_t)ip | ((uint32_t)j << 16));
+            for (int ip = b0; ip < b1 && 2 * ip <= j; ++ip)
+                (j <= 2 * ip + 1 ? diag : t).push_back((uint32_t)ip | ((uint32_t)j << 16));
     }
+    t.insert(t.end(), diag.begin(), diag.end());
     return t;
 }
 
@@ -235,6 +241,32 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
                 return DMPT_ECUDA;
             }
         }
+    // epilogue maps of the layer kernel's TMA path (layer_kernel.cuh, final_epilogue_tma): per matrix a direct
+    // 16 x 32 box (swizzled so that one thread per row reads and writes it without bank conflicts) and a
+    // mirrored 32 x 16 box (written transposed, one row per instruction)
+    auto encode_epi = [&](CUtensorMap* m, void* base, bool fp16, bool mirrored) -> int {
+        const cuuint64_t est1[1] = {(cuuint64_t)L.n_pad * (fp16 ? 2 : 4)};
+        const cuuint32_t ebox[2] = {(cuuint32_t)(mirrored ? 32 : kSub), (cuuint32_t)(mirrored ? kSub : 32)};
+        const CUtensorMapSwizzle sw = mirrored ? CU_TENSOR_MAP_SWIZZLE_NONE
+                                               : (fp16 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_64B);
+        CUresult r = encode(m, fp16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims,
+                            est1, ebox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+                            fp16 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            snprintf(ctx->err, sizeof ctx->err, "cuTensorMapEncodeTiled (epilogue map) failed with CUresult %d", (int)r);
+            return DMPT_ECUDA;
+        }
+        return DMPT_OK;
+    };
+    void* f32[3] = {ctx->at<void>(L.s0), ctx->at<void>(L.s1[0]), ctx->at<void>(L.s1[1])};
+    for (int i = 0; i < 3; ++i)
+        for (int t = 0; t < 2; ++t)
+            if (encode_epi(&ctx->lp.emap32[i][t], f32[i], false, t == 1)) return DMPT_ECUDA;
+    for (int b = 0; b < 2; ++b)
+        for (int m = 0; m < 4; ++m)
+            for (int t = 0; t < 2; ++t)
+                if (encode_epi(&ctx->lp.emap16[b][m][t], ctx->at<void>(L.h[b][m]), true, t == 1)) return DMPT_ECUDA;
     return DMPT_OK;
 }
 
@@ -348,6 +380,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.num_tiles_full = (nb / 2) * (nb / 2);
     lp.n_pad = L.n_pad;
     lp.wave_sync = (o.wave_sync && L.num_tiles > ctx->grid_layer / 2) ? 1 : 0;
+    lp.epilogue_direct = o.epilogue_direct ? 1 : 0;
     lp.ctl = ctx->at<DmptCtl>(L.ctl);
     lp.logs.sigma = ctx->at<int>(L.sigma);
     lp.logs.tr_s = ctx->at<double>(L.tr_s);

@@ -33,9 +33,9 @@
 // CTA pairs: a cluster of two CTAs (one TPC) shares a 256 x 128 pair tile through
 // tcgen05.mma.cta_group::2 (see the comment on the kernel).
 //
-// Warp roles (per CTA): warp 0 TMA producer, warp 1 MMA issuer (leader CTA, one elected lane) and
-// TMEM owner, warps 2-9 epilogue: warp w owns TMEM lane quadrant w % 4 and column half (w - 2) / 4
-// of both accumulators (64 + 64 fp32 registers per thread).  TMEM holds two accumulator stages
+// Warp roles (per CTA, three warpgroups): warp 0 TMA producer, warp 1 MMA issuer (leader CTA, one elected lane) and
+// TMEM owner, warps 2-3 idle (they only hand their registers over), warps 4-11 epilogue: warp w owns TMEM lane
+// quadrant w % 4 and column half (w - 4) / 4 of both accumulators (64 + 64 fp32 registers per thread).  TMEM holds two accumulator stages
 // (2 x [P0 | P1] x 128 columns): the drain of chunk c overlaps the MMAs of chunk c + 1.
 //
 // Orders: PASS 0 of the kernel does orders 0 and 1 (order 0 alone when the context was created
@@ -56,10 +56,10 @@ constexpr int kPair = 2 * kTile;           // rows of a CTA-pair tile (UMMA M = 
 constexpr int kBRows = kTile / 2;          // rows of the J panel each CTA of the pair stages (half of UMMA N)
 constexpr int kABytes = kTile * kRowBytes;           // 8 KiB per A-side operand tile (this CTA's 128 rows of panel I)
 constexpr int kBBytes = kBRows * kRowBytes;          // 4 KiB per B-side operand tile (this CTA's 64 rows of panel J)
-// Per CTA and k-block: PASS 0 (orders 0 and 1) stages 4 A + 4 B tiles (48 KiB), 4 stages;
+// Per CTA and k-block: PASS 0 (orders 0 and 1) stages 4 A + 4 B tiles (48 KiB), 3 stages + 80 KiB of epilogue staging;
 //                      PASS 1 (order 2) stages 6 A + 6 B tiles (72 KiB), 3 stages.
 template <int PASS> struct PassCfg;
-template <> struct PassCfg<0> { static constexpr int kOps = 4, kStages = 4; };
+template <> struct PassCfg<0> { static constexpr int kOps = 4, kStages = 3; };
 template <> struct PassCfg<1> { static constexpr int kOps = 6, kStages = 3; };
 template <> struct PassCfg<2> { static constexpr int kOps = 6, kStages = 3; };
 // PASS 3: a general product C = A.B^T on its own (A, B any n x n matrices; the congruence
@@ -71,15 +71,25 @@ constexpr int kChunkK = 128;               // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;
-constexpr int kEpiWarp0 = 2;
+constexpr int kEpiWarp0 = 4;               // warpgroup 0: TMA producer, MMA issuer, two idle warps; warpgroups 1, 2: epilogue
 constexpr int kNumEpiWarps = 8;
-constexpr int kNumThreads = 32 * (kEpiWarp0 + kNumEpiWarps);   // 320
+constexpr int kNumThreads = 32 * (kEpiWarp0 + kNumEpiWarps);   // 384
+// Registers: 384 threads x 168 at launch; warpgroup 0 then gives its registers back (setmaxnreg.dec) and the two
+// epilogue warpgroups, which hold 2 x 64 fp32 accumulators per thread, grow to 176 (152 + 2 x 176 = 504 <= 512 registers per lane of a scheduler)
+constexpr int kRegsLight = 152, kRegsEpi = 176;
 constexpr int kHalfCols = kTile / 2;       // accumulator columns per epilogue thread and product
 constexpr int kSub = 16;                   // columns per step of the final epilogue
+// Final epilogue through shared memory and TMA (PASS 0, off-diagonal tiles).  Each epilogue warp owns 10 KiB:
+//   ring[2]  32 x 16 fp32 (SWIZZLE_64B): the old iterate arrives here by TMA, the new one is written in place
+//   t32      16 x 32 fp32: the same block transposed (mirrored copy)
+//   dhi, dlo 32 x 16 fp16 (SWIZZLE_32B);  thi, tlo 16 x 32 fp16: the operand split, direct and mirrored
+constexpr int kEpiWarpBytes = 10240;
+constexpr int kEpiRing = 2048, kEpiT32 = 4096, kEpiDhi = 6144, kEpiDlo = 7168, kEpiThi = 8192, kEpiTlo = 9216;
+template <int PASS> struct TmaEpilogue { static constexpr bool value = PASS == 0; };
 template <int PASS>
 constexpr int smem_bytes() {
-    return PassCfg<PASS>::kStages * PassCfg<PASS>::kOps * (kABytes + kBBytes) + 1024 /* alignment slack */ +
-           256 /* barriers */;
+    return PassCfg<PASS>::kStages * PassCfg<PASS>::kOps * (kABytes + kBBytes) +
+           (TmaEpilogue<PASS>::value ? kNumEpiWarps * kEpiWarpBytes : 0) + 1024 /* alignment slack */ + 256 /* barriers */;
 }
 
 // operand matrices, in the order of LayerParams::maps / ::h; a stage holds the A tiles of the first kOps of
@@ -90,6 +100,9 @@ enum Pos : int { PM_H = 0, PM_L = 1, PY_H = 2, PY_L = 3, PZ_H = 4, PZ_L = 5 };
 
 struct LayerParams {
     CUtensorMap maps[2][8];     // [buffer][Mhi, Mlo, S1hi, S1lo, S2hi, S2lo, S3hi, S3lo], box = kBK x kBRows, SWIZZLE_64B
+    // epilogue maps: [..][0] direct 16 x 32 box (fp32: SWIZZLE_64B, fp16: SWIZZLE_32B), [..][1] mirrored 32 x 16 box
+    CUtensorMap emap32[3][2];   // fp32 iterates S0, S1[0], S1[1]
+    CUtensorMap emap16[2][4][2];  // fp16 operand matrices [buffer][Mhi, Mlo, S1hi, S1lo]
     float* s0;                  // fp32 S0, updated in place, ld = n_pad
     float* s1[2];               // fp32 S1, ping-pong
     float* s2[2];               // fp32 response slot 2, ping-pong (order 2: S2; multi-field: S1 of field 2)
@@ -102,6 +115,7 @@ struct LayerParams {
     int num_tiles_full;
     int n_pad;
     int wave_sync;              // 1: producers of all CTAs re-align at every tile boundary (L2 reuse)
+    int epilogue_direct;        // 1: row-per-thread final epilogue on every tile (dmpt_options::epilogue_direct)
     DmptCtl* ctl;
     DmptLogs logs;
     DmptProblem pb;
@@ -121,6 +135,15 @@ struct EpiOut {
     const float* old;      // fp32 matrix holding the previous iterate
     __half* hi;
     __half* lo;
+    // TMA path: maps of the same four matrices (direct box; the mirrored box is the next map)
+    const CUtensorMap* m_old;
+    const CUtensorMap* m_dst;
+    const CUtensorMap* m_hi;
+    const CUtensorMap* m_lo;
+};
+
+struct EpiTma {            // shared-memory addresses of this warp's staging
+    uint32_t ring[2], t32, dhi, dlo, thi, tlo, bar[2];
 };
 
 template <int ORDER>
@@ -212,6 +235,104 @@ __device__ __forceinline__ void final_epilogue(float (&acc)[kHalfCols], const Ep
 }
 
 
+// Final epilogue of one product on an OFF-DIAGONAL tile, through shared memory and TMA: the same arithmetic as
+// final_epilogue with w = 2, dg = 0 (so delta = -+unscale acc exactly and S <- fmaf(+-unscale, acc, old)), but
+//   * the old iterate comes by TMA into this warp's ring (issued one step ahead),
+//   * the new iterate and its split are written to shared memory in the direct and the transposed layout and
+//     leave by six TMA stores per 32 x 16 block: full lines instead of row-per-thread accesses,
+//   * the split uses the packed conversions (cvt.rn.f16x2.f32).
+// step s (0 .. ns-1) of the tile handles product s / 4 (0: P0, 1: P1; when only one is live it is steps 0-3) and
+// columns (s & 3) * 16 of this thread's 64.
+template <int ORDER>
+__device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols], const EpiOut& o, const EpiTma& et,
+                                                   uint32_t& ring_phase, int s_base, int ns,
+                                                   const CUtensorMap* next_old /* old map of step s_base + 4 */,
+                                                   int gr0, int gcb, int lane, float su, float unscale, float scale,
+                                                   bool want_fro, double& r_fs, double& r_fro, float& r_max) {
+    const uint32_t row64 = (uint32_t)lane * 64u, sw64 = ((uint32_t)lane >> 1) & 3u;
+    const uint32_t row32 = (uint32_t)lane * 32u, sw32 = ((uint32_t)lane >> 2) & 1u;
+#pragma unroll
+    for (int sc = 0; sc < kHalfCols / kSub; ++sc) {
+        const int s = s_base + sc;
+        const int slot = s & 1;
+        const int gc0 = gcb + sc * kSub;
+        // the stores of the previous step must have read the staging before it is rewritten; the other ring slot
+        // is then free for the old iterate of the next step
+        if (lane == 0) {
+            bulk_wait_read<0>();
+            if (s >= 1 && s + 1 < ns) {
+                const CUtensorMap* m = sc + 1 < kHalfCols / kSub ? o.m_old : next_old;
+                const int gcn = sc + 1 < kHalfCols / kSub ? gc0 + kSub : gcb;
+                mbar_arrive_expect_tx(et.bar[slot ^ 1], kSub * 32 * 4);
+                tma_load_2d(et.ring[slot ^ 1], m, et.bar[slot ^ 1], gcn, gr0);
+            }
+        }
+        __syncwarp();
+        mbar_wait(et.bar[slot], (ring_phase >> slot) & 1u);
+        ring_phase ^= 1u << slot;
+        float f_fs = 0.f, f_fro = 0.f;
+#pragma unroll
+        for (int q2 = 0; q2 < 2; ++q2) {                  // eight columns: one 16-byte chunk of the fp16 rows
+            uint32_t ph[4], pl[4];
+#pragma unroll
+            for (int j4 = 2 * q2; j4 < 2 * q2 + 2; ++j4) {
+                const uint32_t a32 = et.ring[slot] + row64 + (((uint32_t)j4 ^ sw64) << 4);
+                const float4 x = lds128(a32);
+                float v[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                for (int t = 0; t < 4; t += 2) {
+                    const int j = 4 * j4 + t;
+                    const float a0 = acc[sc * kSub + j], a1 = acc[sc * kSub + j + 1];
+                    const float n0 = fmaf(su, a0, v[t]), n1 = fmaf(su, a1, v[t + 1]);
+                    if (want_fro) {
+                        const float d0 = unscale * a0, d1 = unscale * a1;
+                        f_fro = fmaf(d0, d0, f_fro);
+                        f_fro = fmaf(d1, d1, f_fro);
+                    }
+                    if (ORDER == 0) {
+                        f_fs = fmaf(n0, n0, f_fs);
+                        f_fs = fmaf(n1, n1, f_fs);
+                    } else {
+                        r_max = fmaxf(r_max, fmaxf(fabsf(n0), fabsf(n1)));
+                    }
+                    v[t] = n0; v[t + 1] = n1;
+                    const float t0 = n0 * scale, t1 = n1 * scale;
+                    const __half2 h2 = __floats2half2_rn(t0, t1);
+                    const float2 hf = __half22float2(h2);
+                    const __half2 l2 = __floats2half2_rn(t0 - hf.x, t1 - hf.y);
+                    const uint32_t hw = *reinterpret_cast<const uint32_t*>(&h2);
+                    const uint32_t lw = *reinterpret_cast<const uint32_t*>(&l2);
+                    ph[(j >> 1) & 3] = hw;
+                    pl[(j >> 1) & 3] = lw;
+                    // transposed: for a fixed column the 32 lanes write one row of the mirrored block
+                    sts32(et.t32 + (uint32_t)j * 128u + (uint32_t)lane * 4u, __float_as_uint(n0));
+                    sts32(et.t32 + (uint32_t)(j + 1) * 128u + (uint32_t)lane * 4u, __float_as_uint(n1));
+                    sts16(et.thi + (uint32_t)j * 64u + (uint32_t)lane * 2u, (uint16_t)(hw & 0xFFFF));
+                    sts16(et.thi + (uint32_t)(j + 1) * 64u + (uint32_t)lane * 2u, (uint16_t)(hw >> 16));
+                    sts16(et.tlo + (uint32_t)j * 64u + (uint32_t)lane * 2u, (uint16_t)(lw & 0xFFFF));
+                    sts16(et.tlo + (uint32_t)(j + 1) * 64u + (uint32_t)lane * 2u, (uint16_t)(lw >> 16));
+                }
+                sts128(a32, __float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3]));   // in place
+            }
+            sts128(et.dhi + row32 + (((uint32_t)q2 ^ sw32) << 4), ph[0], ph[1], ph[2], ph[3]);
+            sts128(et.dlo + row32 + (((uint32_t)q2 ^ sw32) << 4), pl[0], pl[1], pl[2], pl[3]);
+        }
+        r_fs += (double)(2.f * f_fs);           // off-diagonal elements count twice
+        r_fro += (double)(2.f * f_fro);
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+            tma_store_2d(o.m_dst, et.ring[slot], gc0, gr0);
+            tma_store_2d(o.m_dst + 1, et.t32, gr0, gc0);
+            tma_store_2d(o.m_hi, et.dhi, gc0, gr0);
+            tma_store_2d(o.m_hi + 1, et.thi, gr0, gc0);
+            tma_store_2d(o.m_lo, et.dlo, gc0, gr0);
+            tma_store_2d(o.m_lo + 1, et.tlo, gr0, gc0);
+            bulk_commit();
+        }
+    }
+}
+
 // One layer launch.  Clusters of two CTAs (one TPC) work on 256 x 128 pair tiles with
 // tcgen05.mma.cta_group::2: CTA r of the pair owns block row 2 IP + r (its 128 rows of every A-side
 // operand and its 128 TMEM lanes of both accumulators) and stages rows r*64 .. r*64+63 of the J panel
@@ -241,16 +362,21 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     const bool idle = PASS == 0 && c.conv1 != 0;
 
     extern __shared__ uint8_t smem_raw[];
+    constexpr bool kTmaEpi = TmaEpilogue<PASS>::value;
+    constexpr int kEpiBytes = kTmaEpi ? kNumEpiWarps * kEpiWarpBytes : 0;
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_base = smem_base + kStages * kStageBytes;
+    const uint32_t epi_base = smem_base + kStages * kStageBytes;          // 1024-byte aligned: stages are multiples of 1 KiB
+    const uint32_t bar_base = epi_base + kEpiBytes;
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
     auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * kStages + s); };
     auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kStages + kAccStages + s); };
-    const uint32_t tmem_slot = bar_base + 8u * (2 * kStages + 2 * kAccStages);
+    auto ring_bar = [&](int w, int s) { return bar_base + 8u * (2 * kStages + 2 * kAccStages + 2 * w + s); };
+    constexpr int kNumBars = 2 * kStages + 2 * kAccStages + 2 * kNumEpiWarps;
+    const uint32_t tmem_slot = bar_base + 8u * kNumBars;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
     volatile uint32_t* tmem_slot_ptr =
-        reinterpret_cast<volatile uint32_t*>(smem_gen + kStages * kStageBytes + 8 * (2 * kStages + 2 * kAccStages));
+        reinterpret_cast<volatile uint32_t*>(smem_gen + kStages * kStageBytes + kEpiBytes + 8 * kNumBars);
 
     // warp index through a shuffle: the compiler then knows it is warp-uniform, and the single-thread
     // sections below are entered through elect.sync, so TMA / MMA operands stay in uniform registers
@@ -287,6 +413,10 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             mbar_init(tfull_bar(s), 1);                      // MMA commit, multicast to both CTAs
             mbar_init(tempty_bar(s), 2 * kNumEpiWarps);      // leader's: epilogue warps of both CTAs
         }
+        for (int w = 0; w < kNumEpiWarps; ++w) {
+            mbar_init(ring_bar(w, 0), 1);                    // old-iterate ring of epilogue warp w (TMA epilogue)
+            mbar_init(ring_bar(w, 1), 1);
+        }
         fence_mbar_init();
     }
     if (warp == 1) {
@@ -297,6 +427,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     cluster_sync_all();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    if (warp < kEpiWarp0) setmaxnreg_dec<kRegsLight>(); else setmaxnreg_inc<kRegsEpi>();
 
     if (warp == 0) {
         // =========================== TMA producer (both CTAs) ===========================
@@ -431,7 +562,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 }
             }
         }
-    } else {
+    } else if (warp >= kEpiWarp0) {
         // =========================== epilogue (both CTAs) ===========================
         const int q = warp & 3;                         // TMEM lane quadrant this warp may read
         const int half = (warp - kEpiWarp0) >> 2;       // which 64 accumulator columns
@@ -455,6 +586,10 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             o0.hi = p.h[c.s0_buf ^ 1][MH]; o0.lo = p.h[c.s0_buf ^ 1][ML];
             o1.dst = p.s1[c.s1_buf ^ 1]; o1.old = p.s1[c.s1_buf];
             o1.hi = p.h[c.s1_buf ^ 1][S1H]; o1.lo = p.h[c.s1_buf ^ 1][S1L];
+            o0.m_old = o0.m_dst = &p.emap32[0][0];
+            o0.m_hi = &p.emap16[c.s0_buf ^ 1][MH][0]; o0.m_lo = &p.emap16[c.s0_buf ^ 1][ML][0];
+            o1.m_old = &p.emap32[1 + c.s1_buf][0]; o1.m_dst = &p.emap32[1 + (c.s1_buf ^ 1)][0];
+            o1.m_hi = &p.emap16[c.s1_buf ^ 1][S1H][0]; o1.m_lo = &p.emap16[c.s1_buf ^ 1][S1L][0];
         } else if (PASS == 1) {
             o0.dst = nullptr; o0.old = nullptr; o0.hi = nullptr; o0.lo = nullptr;
             o1.dst = p.s2[c.s2_buf ^ 1]; o1.old = p.s2[c.s2_buf];
@@ -470,6 +605,19 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         float r_mx1 = 0.f, r_mx0 = 0.f, r_mx_dummy = 0.f;
         int acc = 0;
         uint32_t acc_phase = 0;
+        // TMA epilogue (PASS 0): this warp's staging, and the steps of a tile: 4 per live product
+        EpiTma et;
+        uint32_t ring_phase = 0;
+        {
+            const uint32_t eb = epi_base + (uint32_t)(warp - kEpiWarp0) * kEpiWarpBytes;
+            et.ring[0] = eb; et.ring[1] = eb + kEpiRing; et.t32 = eb + kEpiT32;
+            et.dhi = eb + kEpiDhi; et.dlo = eb + kEpiDlo; et.thi = eb + kEpiThi; et.tlo = eb + kEpiTlo;
+            et.bar[0] = ring_bar(warp - kEpiWarp0, 0); et.bar[1] = ring_bar(warp - kEpiWarp0, 1);
+        }
+        const bool tma_on = kTmaEpi && !p.epilogue_direct;
+        const bool do0 = tma_on && with_p0 && upd0, do1 = tma_on && with_p1;
+        const int ns = 4 * (int)do0 + 4 * (int)do1;
+        const int pre_ch = num_chunks > 4 ? num_chunks - 4 : 0;       // where the first old blocks are requested
         for (int t = pair; t < num_tiles; t += num_pairs) {
             const uint32_t tl = tile_list[t];
             const int ti = 2 * (int)(tl & 0xFFFF) + (int)rank, tj = (int)(tl >> 16);
@@ -478,11 +626,28 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             // the pair tile (IP, J = 2 IP) holds block (2 IP + 1, 2 IP) below the diagonal: its mirror is
             // computed by the pair tile (IP, 2 IP + 1), so the peer CTA only drains it
             const bool live = PASS == 3 || ti <= tj;
+            const bool tma_tile = kTmaEpi && live && ti != tj && ns > 0;
+            const int gr0 = ti * kTile + q * 32;          // first row of this warp's 32 x 64 block
             float a0[kHalfCols], a1[kHalfCols];
 #pragma unroll
             for (int j = 0; j < kHalfCols; ++j) { a0[j] = 0.f; a1[j] = 0.f; }
             // ---- promoted accumulation: drain every chunk with round-to-nearest adds
             for (int ch = 0; ch < num_chunks; ++ch) {
+                if (kTmaEpi && tma_tile && ch == pre_ch && lane == 0) {
+                    // old iterate of steps 0 and 1 into the ring (the previous tile's stores have long been read),
+                    // the rest of this warp's block into L2
+                    bulk_wait_read<0>();
+                    for (int s = 0; s < ns; ++s) {
+                        const CUtensorMap* m = (do0 && s < 4) ? o0.m_old : o1.m_old;
+                        const int gc = gc_base + (s & 3) * kSub;
+                        if (s < 2) {
+                            mbar_arrive_expect_tx(et.bar[s], kSub * 32 * 4);
+                            tma_load_2d(et.ring[s], m, et.bar[s], gc, gr0);
+                        } else {
+                            tma_prefetch_l2_2d(m, gc, gr0);
+                        }
+                    }
+                }
                 mbar_wait(tfull_bar(acc), acc_phase);
                 tc_fence_after();
                 const uint32_t trow = tmem_base + ((uint32_t)(q * 32) << 16) + acc * 256 + half * kHalfCols;
@@ -516,12 +681,20 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             // ---- branch, update, re-split, reductions
             const bool diag = ti == tj;
             if (PASS == 0) {
-                if (with_p0)
+                if (with_p0 && !(tma_tile && upd0))       // diagonal tiles, and the measure-only D0 stop layer
                     final_epilogue<0>(a0, o0, ld, gr, gc_base, diag, upd0, sig, unscale0, scale0, !upd0, r_tr, r_fs0,
                                       r_f0, r_mx_dummy);
-                if (with_p1)
+                if (with_p1 && !tma_tile)
                     final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale1, scale1, conv0, r_dummy,
                                       r_dummy, r_f1, r_mx1);
+                if (kTmaEpi && tma_tile) {
+                    if (do0)
+                        final_epilogue_tma<0>(a0, o0, et, ring_phase, 0, ns, o1.m_old, gr0, gc_base, lane, sig * unscale0,
+                                              unscale0, scale0, false, r_fs0, r_dummy, r_mx_dummy);
+                    if (do1)
+                        final_epilogue_tma<1>(a1, o1, et, ring_phase, do0 ? 4 : 0, ns, nullptr, gr0, gc_base, lane,
+                                              sig * unscale1, unscale1, scale1, conv0, r_dummy, r_f1, r_mx1);
+                }
             } else if (PASS == 3) {
                 // C = 2^-(eA+eB) (A.B^T sums): plain fp32 output, no update, no split, no mirror
                 float* d = p.s1[1] + (size_t)gr * ld + gc_base;
@@ -548,6 +721,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                                   r_f1, r_mx1);
             }
         }
+        if (kTmaEpi && lane == 0) bulk_wait<0>();      // this warp's TMA stores have been performed
         // per-warp partials, fixed slot per (CTA, warp): the finalizer sums them in a fixed order
         r_tr = warp_sum(r_tr);
         r_fs0 = warp_sum(r_fs0);
