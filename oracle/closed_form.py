@@ -9,7 +9,9 @@ f = 1 (occupied) / 0 (virtual), and 0 inside the occ-occ and virt-virt blocks - 
 pattern of PAPER.md:384-393 (Eqs. 56-58) divided by the level spacing.
 
 D2 has no printed formula; it follows from the order-2 blocks of D^2 = D and HD - DH = 0
- with H^(2) = 0.
+ with H^(2) = 0.  `density_matrices_to_order` carries the same
+two block identities to any order k (the (m+1)N x (m+1)N upper-triangular block
+matrices of D and H are idempotent and commute, order by order).
 """
 from __future__ import annotations
 
@@ -59,6 +61,41 @@ def density_matrices(h0, h1, n_occ, order=1, eig=None):
     z[u, o] = z[o, u].T
     d2 = v @ z @ v.T
     return d0, d1, d2
+
+
+def density_matrices_to_order(h0, h1, n_occ, order, eig=None):
+    """[D0, D1, ..., D_order] with D_k = (1/k!) d^k theta(mu I - H0 - lambda H1)/d lambda^k at 0.
+
+    In the eigenbasis of H0 (Z_k = V^T D_k V, A = V^T H1 V, Z_0 = diag(f)) the order-k blocks of
+    D(lambda)^2 = D(lambda) and [H(lambda), D(lambda)] = 0 (PAPER.md:237-245), with H^(k) = 0 for k >= 2, read
+        sum_{j=0..k} Z_j Z_{k-j} = Z_k          and          [diag(eps), Z_k] + [A, Z_{k-1}] = 0,
+    which give, with C_k = sum_{0<j<k} Z_j Z_{k-j},
+        (Z_k)_oo = -(C_k)_oo,   (Z_k)_vv = (C_k)_vv,   (Z_k)_ia = (Z_{k-1} A - A Z_{k-1})_ia / (eps_i - eps_a).
+    Orders 1 and 2 reduce to `density_matrices`.
+    """
+    eps, v = eigensystem(h0) if eig is None else eig
+    a = v.T @ np.asarray(h1, dtype=np.float64) @ v
+    n = eps.shape[0]
+    if not 0 < n_occ < n:
+        raise ValueError("need 0 < n_occ < n")
+    o = slice(0, n_occ)
+    u = slice(n_occ, n)
+    de = eps[:, None] - eps[None, :]
+    f = np.zeros(n)
+    f[:n_occ] = 1.0
+    z = [np.diag(f)]
+    for k in range(1, order + 1):
+        c = np.zeros((n, n))
+        for j in range(1, k):
+            c += z[j] @ z[k - j]
+        zk = np.zeros((n, n))
+        zk[o, o] = -c[o, o]
+        zk[u, u] = c[u, u]
+        num = z[k - 1] @ a - a @ z[k - 1]
+        zk[o, u] = num[o, u] / de[o, u]
+        zk[u, o] = zk[o, u].T
+        z.append(zk)
+    return [v @ zk @ v.T for zk in z]
 
 
 def invariants(h0, h1, d0, d1, d2=None):

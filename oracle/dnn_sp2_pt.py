@@ -120,6 +120,9 @@ class Sp2PtResult:
     id_err: list = field(default_factory=list)     # IdErr_n (nan once S0 froze)
     fro_err1: list = field(default_factory=list)   # FroErr1_n (nan before D0 converged)
     fro_err2: list = field(default_factory=list)   # FroErr2_n (order 2; nan before D1 converged)
+    dk: list = field(default_factory=list)         # [D0, D1, ..., D_order]
+    layers_dk: list = field(default_factory=list)  # layer at which the test of each order fired
+    fro_errk: list = field(default_factory=list)   # fro_errk[k][n-1] = FroErr^(k)_n, k >= 1
 
 
 def _fro(x):
@@ -131,7 +134,8 @@ def _fro(x):
 # ----------------------------------------------------------------------------
 def dnn_sp2_pt(h0, h1, n_occ, order=1, max_layers=200, product=None, bounds=None,
                nx_mode="trace"):
-    """First- (or second-) order DNN-SP2-PT.
+    """DNN-SP2-PT to response order `order` >= 1 (Algorithms 1-3 are printed for order 1; orders >= 2 follow
+    Eq. 26, "a straightforward generalization", with the cascaded stop of reading R15).
 
     h0, h1: symmetric (n, n) (already orthogonalised); n_occ: occupied count.
     bounds: (eps_min, eps_max) or None for Gershgorin (R1, R18).
@@ -143,6 +147,9 @@ def dnn_sp2_pt(h0, h1, n_occ, order=1, max_layers=200, product=None, bounds=None
     h0 = np.asarray(h0, dtype=np.float64)
     h1 = np.asarray(h1, dtype=np.float64)
     n = h0.shape[0]
+    m = int(order)
+    if m < 1:
+        raise ValueError("order >= 1 (dnn_sp2 is the ground-state recursion)")
     eps_min, eps_max = gershgorin(h0) if bounds is None else bounds
     w = eps_max - eps_min
     if not (np.isfinite(w) and w > 0.0):
@@ -150,28 +157,33 @@ def dnn_sp2_pt(h0, h1, n_occ, order=1, max_layers=200, product=None, bounds=None
 
     # initial normalisation layer                        PAPER.md:209-215, 249 (Eq. 34), 493
     s0 = ((eps_max * np.eye(n) - h0) / w).astype(st)
-    s1 = (-h1 / w).astype(st)
-    s2 = np.zeros((n, n), dtype=st) if order == 2 else None      # H^(2) = 0
+    sk = [None, (-h1 / w).astype(st)] + [np.zeros((n, n), dtype=st) for _ in range(2, m + 1)]   # H^(k) = 0, k >= 2
     n_s = float(np.trace(s0.astype(np.float64)))                  # N_S = Tr[S0_0]
 
     res = Sp2PtResult(d0=None, d1=None, d2=None, layers=0, layers_d0=0, layers_d1=0,
                       status="noconv", eps_min=eps_min, eps_max=eps_max, fro_err0=float("nan"))
-    sig, id_err, fro1, fro2 = res.sigma, res.id_err, res.fro_err1, res.fro_err2
-    conv0 = conv1 = conv2 = False
-    n_c = n_c1 = 0
+    sig, id_err = res.sigma, res.id_err
+    fro = [None, res.fro_err1, res.fro_err2] + [[] for _ in range(3, m + 1)]     # fro[k][n-1] = FroErr^(k)_n
+    conv = [False] * (m + 1)          # conv[0]: Algorithm 2; conv[k]: Algorithm 3 for order k
+    n_cv = [0] * (m + 1)              # layer at which each fired
     fro0 = float("nan")
     nan = float("nan")
     nl = 1
-    while nl <= max_layers and not (conv2 if order == 2 else conv1):      # R2
-        # activation functions f^(1), f^(2)              PAPER.md:497, 195 (Eq. 25), 325-329
-        p1 = P.cross(s0, s1, 0, 1)
-        x1 = p1 + p1.T
-        if order == 2:
-            p2 = P.cross(s0, s2, 0, 1)
-            q2 = P.cross(s1, s1, 1, 1)
-            x2 = p2 + p2.T + q2
+    while nl <= max_layers and not conv[m]:                              # R2
+        # activation functions f^(k) = sum_j S^(j) S^(k-j)   PAPER.md:201 (Eq. 26), 285 (Eq. 40); the products
+        # with j > k/2 are the transposes of those with j < k/2
+        xk = [None] * (m + 1)
+        for k in range(1, m + 1):
+            acc = None
+            for j in range(0, (k + 1) // 2):
+                p = P.cross(s0 if j == 0 else sk[j], sk[k - j], j, k - j)
+                t = p + p.T
+                acc = t if acc is None else acc + t
+            if k % 2 == 0:
+                acc = acc + P.cross(sk[k // 2], sk[k // 2], k // 2, k // 2)
+            xk[k] = acc
         res.tr_s.append(n_s)
-        if not conv0:
+        if not conv[0]:
             x0 = P.square(s0)
             if nx_mode == "trace":
                 n_x = float(np.trace(x0.astype(np.float64)))
@@ -187,8 +199,8 @@ def dnn_sp2_pt(h0, h1, n_occ, order=1, max_layers=200, product=None, bounds=None
             if not stop and nl > 2 and sig[nl - 2] != sig[nl - 3]:
                 stop = not (ide <= C_D0 * id_err[nl - 3] ** 2)
             if stop:
-                conv0 = True
-                n_c = nl
+                conv[0] = True
+                n_cv[0] = nl
                 fro0 = _fro(s0.astype(np.float64) - x0.astype(np.float64))
             else:
                 s0 = (s * x0 + (1 - s) * s0).astype(st)                   # PAPER.md:182 (Eq. 23)
@@ -199,40 +211,34 @@ def dnn_sp2_pt(h0, h1, n_occ, order=1, max_layers=200, product=None, bounds=None
             sig.append(-sig[nl - 2])
         s = sig[nl - 1]
 
-        # Algorithm 3                                     PAPER.md:521-525 (R5, R6, R7)
-        if not conv1:
-            if conv0:
-                fro1.append(_fro(s1.astype(np.float64) - x1.astype(np.float64)))
-                if nl - 2 >= n_c and not (fro1[nl - 1] < C_PT * fro0 * fro1[nl - 3]):
-                    conv1 = True
-                    n_c1 = nl
+        # Algorithm 3 (R5, R6, R7) for order 1; the same test cascaded for every further order
+        # (reading R15): order k is measured once order k-1 has converged, first test two layers later
+        for k in range(1, m + 1):
+            if conv[k]:
+                fro[k].append(nan)
+                continue
+            if conv[k - 1]:
+                fro[k].append(_fro(sk[k].astype(np.float64) - xk[k].astype(np.float64)))
+                if nl - 2 >= n_cv[k - 1] and not (fro[k][nl - 1] < C_PT * fro0 * fro[k][nl - 3]):
+                    conv[k] = True
+                    n_cv[k] = nl
             else:
-                fro1.append(nan)
-            if not conv1:
-                s1 = (s * x1 + (1 - s) * s1).astype(st)                   # PAPER.md:193 (Eq. 25)
-        else:
-            fro1.append(nan)
-
-        # second order: the same test cascaded (reading R15)
-        if order == 2:
-            if conv1:
-                fro2.append(_fro(s2.astype(np.float64) - x2.astype(np.float64)))
-                if nl - 2 >= n_c1 and not (fro2[nl - 1] < C_PT * fro0 * fro2[nl - 3]):
-                    conv2 = True
-            else:
-                fro2.append(nan)
-            if not conv2:
-                s2 = (s * x2 + (1 - s) * s2).astype(st)                   # PAPER.md:195 (Eq. 25)
+                fro[k].append(nan)
+            if not conv[k]:
+                sk[k] = (s * xk[k] + (1 - s) * sk[k]).astype(st)          # PAPER.md:193-201 (Eqs. 25, 26)
         nl += 1
 
     res.layers = nl - 1
-    res.layers_d0 = n_c
-    res.layers_d1 = n_c1
+    res.layers_d0 = n_cv[0]
+    res.layers_d1 = n_cv[1]
+    res.layers_dk = list(n_cv)
     res.fro_err0 = fro0
-    res.status = "ok" if (conv2 if order == 2 else conv1) else "noconv"
+    res.fro_errk = fro
+    res.status = "ok" if conv[m] else "noconv"
     res.d0 = np.asarray(s0, dtype=np.float64)
-    res.d1 = np.asarray(s1, dtype=np.float64)
-    res.d2 = None if s2 is None else np.asarray(s2, dtype=np.float64)
+    res.d1 = np.asarray(sk[1], dtype=np.float64)
+    res.d2 = None if m < 2 else np.asarray(sk[2], dtype=np.float64)
+    res.dk = [res.d0] + [np.asarray(x, dtype=np.float64) for x in sk[1:]]
     return res
 
 

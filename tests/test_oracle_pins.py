@@ -83,6 +83,37 @@ def test_o1_d2_second_difference():
     assert np.abs(fd - d2).max() < 2e-4 * max(1.0, np.abs(d2).max())
 
 
+def test_o1_general_order_matches_finite_differences_and_block_identities():
+    """Orders 3 and 4 of the definition (closed_form.density_matrices_to_order): D_k = (1/k!) d^k theta / d lambda^k
+    (Eq. 20) against central difference stencils of eigh projectors, the order-k blocks of D^2 = D and
+    [H, D] = 0 through the (m+1)N x (m+1)N block upper-triangular matrices, and orders <= 2
+    against the separately written order-2 closed form."""
+    h0, h1, n_occ, _, _ = small_problem(n=40, n_occ=17, seed=3)
+    n = h0.shape[0]
+    d = O1.density_matrices_to_order(h0, h1, n_occ, 4)
+    for a, b in zip(d, O1.density_matrices(h0, h1, n_occ, order=2)):
+        assert np.abs(a - b).max() < 1e-14
+    T = lambda x: _theta(h0 + x * h1, n_occ)
+    h = 5e-3
+    fd3 = (T(2 * h) - 2 * T(h) + 2 * T(-h) - T(-2 * h)) / (2 * h ** 3) / 6.0
+    fd4 = (T(2 * h) - 4 * T(h) + 6 * T(0.0) - 4 * T(-h) + T(-2 * h)) / h ** 4 / 24.0
+    assert np.abs(fd3 - d[3]).max() < 3e-4 * np.abs(d[3]).max()
+    assert np.abs(fd4 - d[4]).max() < 3e-4 * np.abs(d[4]).max()
+    # halving h divides the stencil error by four: the mismatch is the stencil's, not the closed form's
+    h = 1e-2
+    fd3b = (T(2 * h) - 2 * T(h) + 2 * T(-h) - T(-2 * h)) / (2 * h ** 3) / 6.0
+    assert 3.0 < np.abs(fd3b - d[3]).max() / np.abs(fd3 - d[3]).max() < 5.0
+    z = np.zeros((n, n))
+    m = 4
+    bd = np.block([[d[c - r] if c >= r else z for c in range(m + 1)] for r in range(m + 1)])
+    hs = [h0, h1, z, z, z]
+    bh = np.block([[hs[c - r] if c >= r else z for c in range(m + 1)] for r in range(m + 1)])
+    assert np.abs(bd @ bd - bd).max() < 1e-11
+    assert np.abs(bh @ bd - bd @ bh).max() < 1e-11
+    for k in (3, 4):
+        assert abs(np.trace(d[k])) < 1e-10 and np.abs(d[k] - d[k].T).max() < 1e-12
+
+
 def test_o1_invariants_and_block_identities():
     """Blocks of D^2 = D and HD - DH = 0 up to order 2 (PAPER.md:245); Tr D0 = N_occ (PAPER.md:81);
     Idemp^(1) = 0 (PAPER.md:399)."""
@@ -166,6 +197,52 @@ def test_o2_second_order_matches_definition():
     assert np.abs(r.d1 - d1).max() < 1e-10 * max(1.0, np.abs(d1).max())
     assert np.abs(r.d2 - d2).max() < 1e-9 * max(1.0, np.abs(d2).max())
     assert r.layers_d0 < r.layers_d1 < r.layers
+
+
+def test_o2_general_order_matches_definition_and_block_matrix_squaring():
+    """Order m of the method (Eq. 26 with the symmetry saving of PAPER.md:325-329): limits against the
+    definition at every order; the iterates against squaring the (m+1)N upper-triangular block matrix
+    (Eqs. 35-37, 285 Eq. 40) with the logged sigma; the cascaded stops two layers apart (R15)."""
+    h0, h1, n_occ, _, _ = small_problem(n=48, n_occ=20, seed=21, gap=0.5, h1_scale=0.02)
+    n = h0.shape[0]
+    for m in (3, 4):
+        d = O1.density_matrices_to_order(h0, h1, n_occ, m)
+        r = O2.dnn_sp2_pt(h0, h1, n_occ, order=m)
+        assert r.status == "ok" and len(r.dk) == m + 1
+        for k in range(m + 1):
+            assert np.abs(r.dk[k] - d[k]).max() < 1e-9 * max(1.0, np.abs(d[k]).max()), (m, k)
+        assert all(b - a >= 2 for a, b in zip(r.layers_dk, r.layers_dk[1:])) and r.layers == r.layers_dk[m]
+        # block-matrix squaring while every order is still being updated (layers 1 .. n_c - 1)
+        z = np.zeros((n, n))
+        hs = [h0, h1] + [z] * (m - 1)
+        bh = np.block([[hs[c - q] if c >= q else z for c in range(m + 1)] for q in range(m + 1)])
+        bs = (r.eps_max * np.eye((m + 1) * n) - bh) / (r.eps_max - r.eps_min)
+        for k in range(r.layers_d0 - 1):
+            bs = r.sigma[k] * (bs @ bs) + (1 - r.sigma[k]) * bs
+        assert np.abs(bs[:n, :n] - r.d0).max() < 1e-12
+        # from there on S0 is frozen; carry the first block row forward by Eq. 26 with the logged sigma, freezing
+        # order k at the layer its test fired
+        sk = [bs[:n, k * n:(k + 1) * n].copy() for k in range(m + 1)]
+        for layer in range(r.layers_d0, r.layers + 1):
+            s = r.sigma[layer - 1]
+            xs = [None] + [sum(sk[j] @ sk[k - j] for j in range(k + 1)) for k in range(1, m + 1)]
+            for k in range(1, m + 1):
+                if layer < r.layers_dk[k]:
+                    sk[k] = s * xs[k] + (1 - s) * sk[k]
+        for k in range(1, m + 1):
+            assert np.abs(sk[k] - r.dk[k]).max() < 1e-10 * max(1.0, np.abs(r.dk[k]).max()), (m, k)
+
+
+def test_o2_dual_half_general_order_accuracy():
+    """O2-dh at order 3: every order within a few 1e-6 of the definition on a well-gapped problem (the same
+    floor as the paper's 5e-5 relative 2-norm figure at order 1)."""
+    h0, h1, n_occ, _, _ = small_problem(n=96, n_occ=40, seed=21, gap=0.5, h1_scale=0.02)
+    d = O1.density_matrices_to_order(h0, h1, n_occ, 3)
+    r = O2.dnn_sp2_pt(h0.astype(np.float32), h1.astype(np.float32), n_occ, order=3,
+                      product=O2.DualHalfProduct(shift0=14, shift1="auto"), nx_mode="fro")
+    assert r.status == "ok"
+    for k in range(4):
+        assert np.abs(r.dk[k] - d[k]).max() < 5e-5 * max(1.0, np.abs(d[k]).max()), k
 
 
 def test_o2_h1_equal_h0_gives_zero_response():
