@@ -9,6 +9,7 @@ than the 126 MB L2, so no explicit L2 flush is needed (stated in `config`).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--n 16384]
     python bench.py --impl reference      # the fp64 CPU oracle, bounded sample, same JSON line
+    python bench.py --fd [--config 2]     # finite-difference stencils vs the first-order recursion (Fig. 5)
 
 value      paper-convention Tflops (one FMA = one flop, Eq. 82):
            (5 N^3 L_active + 3 N^3 L_frozen) / time of the whole dmpt_run, inputs resident in HBM.
@@ -398,6 +399,81 @@ def run_ours(args):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------
+# --fd: the finite-difference comparison of PAPER.md:562-582 (Eqs. 83-84, Fig. 5) as a workload
+# ---------------------------------------------------------------------------------------------
+def run_fd(args):
+    """D1 by the 2- and 4-point stencils (dmpt_fd_response: 2 / 4 ground-state runs) over a sweep of step sizes h,
+    next to the first-order DNN-SP2-PT run on the same input.  Errors are relative to the definition (oracle O1,
+    evaluated and timed on the host: this mode's cpu_baseline) in the paper's measure - the relative 2-norm - and as
+    max|.|/max|ref|.  Cost per layer in the paper's count: 4 / 8 products against 5."""
+    import numpy as np
+    import torch
+
+    from paper_2203_09621_b200 import Dmpt
+    from workloads import make_config
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU path")
+    dev = torch.device("cuda", 0)
+    wl = make_config(args.config, n=args.n, device=str(dev) if args.n >= 8192 else None)
+    if wl.order != 1:
+        raise SystemExit("--fd needs a first-order config")
+    n = wl.n
+    h0, h1 = torch.from_numpy(wl.h0).to(dev), torch.from_numpy(wl.h1).to(dev)
+    # the definition (O1) on the host, timed: the reference of every error below
+    from oracle.closed_form import density_matrices
+    t0 = time.perf_counter()
+    _, d1_ref = density_matrices(wl.h0, wl.h1, wl.n_occ)
+    cpu_s = time.perf_counter() - t0
+    ref = torch.from_numpy(d1_ref).to(dev)
+    ref2 = float(torch.linalg.matrix_norm(ref, ord=2))
+    refmax = float(ref.abs().max())
+
+    def errors(d1):
+        e = d1.double() - ref
+        return {"rel_2norm": float(torch.linalg.matrix_norm(e, ord=2)) / ref2, "max_rel": float(e.abs().max()) / refmax}
+
+    pt = Dmpt(n, order=1, device=dev)
+    pt.set_hamiltonian(h0, h1, wl.n_occ)
+    for _ in range(2):
+        r = pt.run()
+    dmpt = dict(errors(r.d1), layers=r.layers, layers_d0=r.layers_d0, ms=r.ms_total, products_per_layer=5,
+                products=5 * r.layers_d0 + 3 * (r.layers - r.layers_d0))
+    pt.close()
+    h1_scale = float(h1.abs().max())
+    gs = Dmpt(n, order=0, device=dev)
+    sweep = []
+    launches = 0
+    for points in (2, 4):
+        for hs in args.fd_steps:
+            # h is quoted relative to the perturbation's size: h max|H1| is the largest change of a matrix element
+            h = hs / h1_scale
+            d1, layers, ms = gs.fd_response(h0, h1, wl.n_occ, h, points)
+            d1, layers, ms = gs.fd_response(h0, h1, wl.n_occ, h, points)          # second call: warm
+            sweep.append(dict(errors(d1), points=points, h=h, h_times_max_h1=hs, layers=layers, ms=ms,
+                              products_per_layer=2 * points, products=2 * sum(layers)))
+            launches += sum(layers)
+    gs.close()
+    best = {p: min((x for x in sweep if x["points"] == p), key=lambda x: x["rel_2norm"]) for p in (2, 4)}
+    line = {"mode": "fd", "metric": "d1_relative_2norm_error", "unit": "relative 2-norm error", "higher_is_better": False,
+            "value": dmpt["rel_2norm"], "n_gpus": 1, "data": "synthetic", "gpu_launches": launches,
+            "config": {"workload": workload_name(args) + "; finite-difference stencils of ground-state runs against "
+                                   "the first-order recursion (PAPER.md:562-582, Fig. 5)", "n": n, "n_occ": wl.n_occ,
+                       "gap": wl.meta.get("gap")},
+            "dmpt": dmpt, "fd_sweep": sweep,
+            "best": {"two_point": best[2], "four_point": best[4],
+                     "two_point_over_dmpt": best[2]["rel_2norm"] / dmpt["rel_2norm"],
+                     "four_point_over_dmpt": best[4]["rel_2norm"] / dmpt["rel_2norm"],
+                     "paper": "best 2-point: almost an order of magnitude less accurate than DNN-SP2-PT; best 4-point: "
+                              "a factor 2 less accurate, at 8 instead of 5 products per layer (PAPER.md:578-582)"},
+            "cpu_baseline": {"value": cpu_s, "unit": "s", "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
+                             "sample": f"oracle.closed_form.density_matrices (fp64 eigendecomposition) at n={n}: the "
+                                       "reference of every error in this line"}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def solver_n_pad(n):
     return (n + 255) // 256 * 256      # CTA-pair tiles: 256 rows
 
@@ -454,7 +530,13 @@ def main():
     ap.add_argument("--fields", type=int, default=1,
                     help="perturbations sharing H0 in one run (1..3); value then counts every field as a run of its own")
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per layer launch from ncu (profiles/)")
+    ap.add_argument("--fd", action="store_true",
+                    help="finite-difference stencils (Eqs. 83-84) against the first-order recursion; default config 2")
+    ap.add_argument("--fd-steps", type=float, nargs="+", default=[3e-4, 1e-3, 3e-3, 1e-2, 3e-2, 1e-1],
+                    help="step sizes h of the sweep, as h x max|H1|")
     args = ap.parse_args()
+    if args.fd and "--config" not in " ".join(sys.argv):
+        args.config = 2
     if args.n is None:
         from workloads import CONFIGS
         args.n = CONFIGS[args.config]["n"]
@@ -463,6 +545,8 @@ def main():
         if world == 1 and args.gpus > 1:
             return respawn_under_torchrun(args)
         raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    if args.fd:
+        return run_fd(args)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warmup raised to 3 (timing rules)", file=sys.stderr)
         args.warmup = 3

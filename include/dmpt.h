@@ -37,7 +37,7 @@ extern "C" {
 #endif
 
 #define DMPT_OK            0
-#define DMPT_EINVAL       -1   /* null pointer, n <= 0, n_occ outside (0, n), ld < n, order not 0|1|2 */
+#define DMPT_EINVAL       -1   /* null pointer, n <= 0, n_occ outside (0, n), ld < n, order not 0..3  */
 #define DMPT_ESTATE       -2   /* dmpt_run before dmpt_set_hamiltonian                                */
 #define DMPT_ECUDA        -3   /* CUDA error (text via dmpt_strerror / dmpt_last_cuda_error)          */
 #define DMPT_EDEGENERATE  -4   /* eps_max - eps_min not positive and finite                           */
@@ -49,7 +49,8 @@ typedef struct dmpt_ctx dmpt_ctx;
 
 typedef struct dmpt_options {
     int max_layers;    /* cap on the while loop of Algorithm 1 (the paper has none); default 200       */
-    int order;         /* 1: D0, D1.  2: also D2 (Eq. 25 third line).  0: D0 only - the       */
+    int order;         /* 1: D0, D1.  2: also D2 (Eq. 25 third line).  3: also D3 (Eq. 26 at  */
+                       /* k = 3; results through dmpt_run_orders).  0: D0 only - the        */
                        /* ground-state DNN-SP2 recursion with Algorithm 2 as its stop (PAPER.md:176-186,   */
                        /* 515-519); pass NULL for every H1 / D1 argument                                  */
     int s0_shift;      /* a >= 0: S0 is split as hi = fp16(2^a S0), lo = fp16(2^a S0 - hi) and 2^-2a   */
@@ -79,7 +80,8 @@ typedef struct dmpt_result {
     int layers_d1;     /* layer at which the D1 test fired (Algorithm 3); 0 if it never did           */
     int launches;      /* kernels this run launched (all of them this library's own)                  */
     int layers_d2;     /* order 2: layer at which the D2 test fired (R15); 0 otherwise            */
-    int layers_d3;     /* multi-field runs: stop layer of field 3 (layers_d2: field 2, layers_d1: field 1)   */
+    int layers_d3;     /* order 3: layer at which the D3 test fired.  Multi-field runs: stop layer of field 3     */
+                       /* (layers_d2: field 2, layers_d1: field 1)                                               */
     int reserved_i[1];
     double eps_min, eps_max;   /* spectral bounds used                                 */
     double fro_err0;           /* FroErr0 = ||S0 - S0^2||_F at the D0 stop layer; NaN at order 0 */
@@ -97,7 +99,7 @@ typedef struct dmpt_result {
     double *id_err;            /* IdErr_n = N_S - N_X; NaN once S0 froze                              */
     double *fro_err1;          /* FroErr1_n; NaN before D0 converged                   */
     double *fro_err2;          /* FroErr2_n (order 2); NaN before D1 converged.  Multi-field: FroErr1 of field 2 */
-    double *fro_err3;          /* multi-field: FroErr1 of field 3 (else untouched)                    */
+    double *fro_err3;          /* order 3: FroErr3_n, NaN before D2 converged.  Multi-field: FroErr1 of field 3 */
 } dmpt_result;
 
 /* Defaults: max_layers 200, order 1, s0_shift -1, s1_autoscale 1, bounds 0, wave_sync 1, num_fields 1. */
@@ -125,6 +127,15 @@ int dmpt_set_hamiltonian(dmpt_ctx *ctx, const float *d_h0, const float *d_h1, in
  * with leading dimension ld >= n.  `res` may be NULL.  On DMPT_ENOCONV the outputs hold the last
  * iterate.  Safe to call repeatedly. */
 int dmpt_run(dmpt_ctx *ctx, float *d_d0, float *d_d1, float *d_d2, int ld, dmpt_result *res);
+
+/* General response order (Eq. 26, 285 Eq. 40): the same run for a context of any
+ * supported order m = 0..3.  d_d is a HOST array of m + 1 DEVICE matrices D0 .. D_m (leading dimension ld).  Per
+ * layer the activation of order k is f^(k) = sum_j S^(j) S^(k-j); the terms with j > k/2 are the transposes of those
+ * with j < k/2, so order k costs ceil(k/2) cross products M.Y + Y.M plus, for even k, one
+ * square: order 3 adds  X3 = (S0 S3 + S3 S0) + (S1 S2 + S2 S1)  as one more launch per layer (twelve tensor-core
+ * products per tile into two accumulators).  Stops are cascaded (R15): order k is tested with the
+ * inequality of Algorithm 3 once order k-1 has converged.  H^(k) = 0 for k >= 2. */
+int dmpt_run_orders(dmpt_ctx *ctx, float *const *d_d, int ld, dmpt_result *res);
 
 /* Multi-field variants (contexts created with order == 1 and num_fields >= 1).
  * d_h1 / d_d1 are HOST arrays of num_fields DEVICE matrix pointers, all with leading dimension ld.
@@ -156,6 +167,12 @@ int dmpt_layer_products(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, int
 int dmpt_layer_products2(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, const float *d_s2, int ld,
                          float *d_x2, int ld_out);
 
+/* The order-3 product of one layer on its own (contexts created with order == 3; Eq. 26 at k = 3):
+ * X3 = S0 S3 + S3 S0 + S1 S2 + S2 S1 for symmetric S0..S3, through the split + tcgen05 path of the order-3 pass
+ * (sigma = +1, no stopping test). */
+int dmpt_layer_products3(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, const float *d_s2, const float *d_s3,
+                         int ld, float *d_x3, int ld_out);
+
 /* A general product in the dual half-precision representation, on its own (the
  * congruence transforms either side of the hot path, H_orth = Z^T H Z and D = Z D_orth Z^T, PAPER.md:74-79,
  * A18, are two of these each): C = A.B^T = A_hi.B_hi^T + A_hi.B_lo^T + A_lo.B_hi^T for ANY n x n device
@@ -163,6 +180,26 @@ int dmpt_layer_products2(dmpt_ctx *ctx, const float *d_s0, const float *d_s1, co
  * products; each operand is split after its own power-of-two scale (max|.| into [8, 16)).  Contexts of
  * order >= 1.  C may alias A or B (both are copied into the workspace before C is written). */
 int dmpt_product_nt(dmpt_ctx *ctx, const float *d_a, const float *d_b, int ld, float *d_c, int ld_out);
+
+/* The congruence transforms of PAPER.md:74-79, 541 (Eq. 81), A17-A18, each two dmpt_product_nt products chained on
+ * the device: transpose_z != 0: C = Z^T X Z (H_orth = Z^T H Z, Eq. 81);  transpose_z == 0: C = Z X Z^T (D = Z D_orth Z^T).
+ * Z is any n x n device matrix, X a SYMMETRIC one (both fp32, leading dimension ld); where Z^T is needed as the row
+ * operand it is transposed by the library's own copy kernel on the way into the workspace.  C may alias X or Z.
+ * Contexts of order >= 1; uses the workspace's staging buffer (not concurrently with dmpt_run_host). */
+int dmpt_congruence(dmpt_ctx *ctx, const float *d_z, const float *d_x, int ld, int transpose_z, float *d_c, int ld_out);
+
+/* Finite-difference response from ground-state runs: the comparison the paper
+ * draws in Fig. 5, built in as a validation / benchmark workload.  Contexts of order == 0.  For points == 2 (Eq. 83)
+ *     D1 ~ [D(H0 + h H1) - D(H0 - h H1)] / 2h                                                  + O(h^2),
+ * for points == 4 (Eq. 84)
+ *     D1 ~ [-D(H0 + 2h H1) + 8 D(H0 + h H1) - 8 D(H0 - h H1) + D(H0 - 2h H1)] / 12h            + O(h^4),
+ * every D(.) one run of the ground-state recursion (order 0) of this library on H0 + t H1 (formed on the device in
+ * fp64, rounded once).  Cost in the paper's count: 2 products per layer and run, i.e. 4 (8) per layer
+ * against 5 for the first-order recursion.  d_d1: device output (leading dimension ld_out); h_layers: host array of
+ * `points` layer counts (may be NULL), in the order of the stencil terms above; *h_ms: CUDA-event time of all runs.
+ * Returns the first non-zero status of the runs. */
+int dmpt_fd_response(dmpt_ctx *ctx, const float *d_h0, const float *d_h1, int ld, int n_occ, double h, int points,
+                     float *d_d1, int ld_out, int *h_layers, double *h_ms);
 
 /* Inverse factor of a symmetric positive definite overlap matrix S (device, fp32, leading dimension ld):
  * Z with Z^T S Z = I by the third-order recursion of PAPER.md:693-703 (A19-A21),
@@ -193,6 +230,28 @@ int dmpt_split(dmpt_ctx *ctx, const float *d_x, int ld, int shift, int diag_half
                uint16_t *d_hi, uint16_t *d_lo, int ld_out);
 
 int dmpt_destroy(dmpt_ctx *ctx);
+
+/* Order-parallel pair (Sec. III.C "parallelizing the matrix multiplications over
+ * multiple GPU devices", 548-550): device0 computes f^(0) = S0^2 with the trace criterion and Algorithm 2, device1
+ * computes f^(1) = S0 S1 + S1 S0 with Algorithm 3.  Information flows one way: per layer the fp16 operand pair of
+ * S0_{n-1} (4 N^2 bytes) and a 40-byte decision record go from device0 to device1 by cudaMemcpyPeerAsync on a copy
+ * stream, overlapping the products of both sides; there is no reduction and no collective.  After Algorithm 2 fired
+ * the order-0 side is done and the order-1 side runs on alone (sigma flips).
+ *   device0 == device1 is allowed (two streams of one GPU, device-local copies): the results - D0, D1, layer counts,
+ *   per-layer records - are bit-identical to dmpt_run on the same inputs in both set-ups.
+ * Workspaces: dmpt_pair_workspace_bytes(n, side) bytes on the respective device (side 0: order-0 side), 256-byte
+ * aligned, caller-owned.  d_h0 and d_d0 live on device0, d_h1 and d_d1 on device1.  The pair owns its streams.
+ * opt: as for dmpt_create with order 1 and one field (NULL for defaults).  The host keeps two layers of work queued
+ * on either side and looks at one pinned flag per layer; it never waits for the layer it has just enqueued. */
+typedef struct dmpt_pair dmpt_pair;
+size_t dmpt_pair_workspace_bytes(int n, int side);
+int dmpt_pair_create(dmpt_pair **pair, int n, const dmpt_options *opt,
+                     int device0, void *d_workspace0, size_t workspace0_bytes,
+                     int device1, void *d_workspace1, size_t workspace1_bytes);
+int dmpt_pair_set_hamiltonian(dmpt_pair *pair, const float *d_h0, const float *d_h1, int ld, int n_occ);
+int dmpt_pair_run(dmpt_pair *pair, float *d_d0, float *d_d1, int ld, dmpt_result *res);
+int dmpt_pair_destroy(dmpt_pair *pair);
+const char *dmpt_pair_last_cuda_error(const dmpt_pair *pair);
 
 const char *dmpt_strerror(int code);
 /* Text of the last CUDA error seen by this context (empty string if none). */

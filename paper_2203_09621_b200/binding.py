@@ -17,6 +17,9 @@ EXPORTED_SYMBOLS = (
     "dmpt_run", "dmpt_run_host", "dmpt_layer_products", "dmpt_destroy", "dmpt_strerror",
     "dmpt_last_cuda_error", "dmpt_spectral_bounds", "dmpt_initial_transform", "dmpt_split",
     "dmpt_layer_products2", "dmpt_product_nt", "dmpt_inverse_factor", "dmpt_workspace_bytes_fields", "dmpt_set_hamiltonian_fields", "dmpt_run_fields",
+    "dmpt_run_orders", "dmpt_layer_products3", "dmpt_congruence", "dmpt_fd_response",
+    "dmpt_pair_workspace_bytes", "dmpt_pair_create", "dmpt_pair_set_hamiltonian", "dmpt_pair_run", "dmpt_pair_destroy",
+    "dmpt_pair_last_cuda_error",
 )
 
 DMPT_OK, DMPT_EINVAL, DMPT_ESTATE, DMPT_ECUDA = 0, -1, -2, -3
@@ -76,6 +79,29 @@ def lib():
         L.dmpt_set_hamiltonian_fields.restype = C.c_int
         L.dmpt_run_fields.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_int, C.POINTER(_CResult)]
         L.dmpt_run_fields.restype = C.c_int
+        L.dmpt_run_orders.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.c_int, C.POINTER(_CResult)]
+        L.dmpt_run_orders.restype = C.c_int
+        L.dmpt_layer_products3.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
+                                           C.c_void_p, C.c_int]
+        L.dmpt_layer_products3.restype = C.c_int
+        L.dmpt_congruence.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
+        L.dmpt_congruence.restype = C.c_int
+        L.dmpt_fd_response.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int,
+                                       C.c_void_p, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double)]
+        L.dmpt_fd_response.restype = C.c_int
+        L.dmpt_pair_workspace_bytes.argtypes = [C.c_int, C.c_int]
+        L.dmpt_pair_workspace_bytes.restype = C.c_size_t
+        L.dmpt_pair_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.POINTER(DmptOptions), C.c_int, C.c_void_p,
+                                       C.c_size_t, C.c_int, C.c_void_p, C.c_size_t]
+        L.dmpt_pair_create.restype = C.c_int
+        L.dmpt_pair_set_hamiltonian.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int]
+        L.dmpt_pair_set_hamiltonian.restype = C.c_int
+        L.dmpt_pair_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(_CResult)]
+        L.dmpt_pair_run.restype = C.c_int
+        L.dmpt_pair_destroy.argtypes = [C.c_void_p]
+        L.dmpt_pair_destroy.restype = C.c_int
+        L.dmpt_pair_last_cuda_error.argtypes = [C.c_void_p]
+        L.dmpt_pair_last_cuda_error.restype = C.c_char_p
         L.dmpt_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.POINTER(DmptOptions), C.c_void_p,
                                   C.c_size_t, C.c_void_p]
         L.dmpt_create.restype = C.c_int
@@ -140,6 +166,61 @@ def dmpt_set_hamiltonian_fields(ctx, h0_ptr: int, h1_ptrs, ld: int, n_occ: int) 
 def dmpt_run_fields(ctx, d0_ptr: int, d1_ptrs, ld: int, res) -> int:
     arr = (C.c_void_p * len(d1_ptrs))(*[C.c_void_p(p) for p in d1_ptrs])
     return int(lib().dmpt_run_fields(ctx, C.c_void_p(d0_ptr), arr, int(ld), C.byref(res) if res is not None else None))
+
+
+def dmpt_run_orders(ctx, d_ptrs, ld: int, res) -> int:
+    arr = (C.c_void_p * len(d_ptrs))(*[C.c_void_p(p) for p in d_ptrs])
+    return int(lib().dmpt_run_orders(ctx, arr, int(ld), C.byref(res) if res is not None else None))
+
+
+def dmpt_layer_products3(ctx, s0_ptr, s1_ptr, s2_ptr, s3_ptr, ld, x3_ptr, ld_out) -> int:
+    return int(lib().dmpt_layer_products3(ctx, C.c_void_p(s0_ptr), C.c_void_p(s1_ptr), C.c_void_p(s2_ptr),
+                                          C.c_void_p(s3_ptr), int(ld), C.c_void_p(x3_ptr), int(ld_out)))
+
+
+def dmpt_congruence(ctx, z_ptr, x_ptr, ld, transpose_z, c_ptr, ld_out) -> int:
+    return int(lib().dmpt_congruence(ctx, C.c_void_p(z_ptr), C.c_void_p(x_ptr), int(ld), int(transpose_z),
+                                     C.c_void_p(c_ptr), int(ld_out)))
+
+
+def dmpt_fd_response(ctx, h0_ptr, h1_ptr, ld, n_occ, h, points, d1_ptr, ld_out):
+    layers = (C.c_int * 4)()
+    ms = C.c_double()
+    rc = int(lib().dmpt_fd_response(ctx, C.c_void_p(h0_ptr), C.c_void_p(h1_ptr), int(ld), int(n_occ), float(h),
+                                    int(points), C.c_void_p(d1_ptr), int(ld_out), layers, C.byref(ms)))
+    return rc, list(layers[:int(points)]) if points in (2, 4) else [], ms.value
+
+
+def dmpt_pair_workspace_bytes(n: int, side: int) -> int:
+    return int(lib().dmpt_pair_workspace_bytes(int(n), int(side)))
+
+
+def dmpt_pair_create(n, opt, device0, ws0_ptr, ws0_bytes, device1, ws1_ptr, ws1_bytes):
+    h = C.c_void_p()
+    rc = lib().dmpt_pair_create(C.byref(h), int(n), C.byref(opt) if opt is not None else None, int(device0),
+                                C.c_void_p(ws0_ptr), int(ws0_bytes), int(device1), C.c_void_p(ws1_ptr), int(ws1_bytes))
+    if rc != DMPT_OK:
+        raise DmptError(rc, "dmpt_pair_create")
+    return h
+
+
+def dmpt_pair_set_hamiltonian(pair, h0_ptr, h1_ptr, ld, n_occ) -> None:
+    rc = lib().dmpt_pair_set_hamiltonian(pair, C.c_void_p(h0_ptr), C.c_void_p(h1_ptr), int(ld), int(n_occ))
+    if rc != DMPT_OK:
+        raise DmptError(rc, "dmpt_pair_set_hamiltonian")
+
+
+def dmpt_pair_run(pair, d0_ptr, d1_ptr, ld, res) -> int:
+    return int(lib().dmpt_pair_run(pair, C.c_void_p(d0_ptr), C.c_void_p(d1_ptr), int(ld),
+                                   C.byref(res) if res is not None else None))
+
+
+def dmpt_pair_destroy(pair) -> None:
+    lib().dmpt_pair_destroy(pair)
+
+
+def dmpt_pair_last_cuda_error(pair) -> str:
+    return lib().dmpt_pair_last_cuda_error(pair).decode()
 
 
 def dmpt_strerror(code: int) -> str:
@@ -248,6 +329,7 @@ class DmptResult:
     d0: object = None
     d1: object = None
     d2: object = None
+    d3: object = None
 
 
 class Dmpt:
@@ -324,8 +406,8 @@ class Dmpt:
                           sigma=list(bufs["sigma"][:nl]), tr_s=list(bufs["tr_s"][:nl]),
                           tr_x=list(bufs["tr_x"][:nl]), id_err=list(bufs["id_err"][:nl]),
                           fro_err1=list(bufs["fro_err1"][:nl]),
-                          fro_err2=list(bufs["fro_err2"][:nl]) if (self.order == 2 or self.num_fields > 1) else [],
-                          fro_err3=list(bufs["fro_err3"][:nl]) if self.num_fields > 2 else [],
+                          fro_err2=list(bufs["fro_err2"][:nl]) if (self.order >= 2 or self.num_fields > 1) else [],
+                          fro_err3=list(bufs["fro_err3"][:nl]) if (self.num_fields > 2 or self.order == 3) else [],
                           layers_d2=r.layers_d2, layers_d3=r.layers_d3, d0=d0, d1=d1, d2=d2)
 
     def _check_outputs(self, where, cuda, *mats):
@@ -356,6 +438,27 @@ class Dmpt:
         rc = dmpt_run(self.ctx, d0.data_ptr(), d1.data_ptr() if d1 is not None else 0,
                       d2.data_ptr() if d2 is not None else 0, d0.stride(0), r)
         return self._wrap(rc, r, bufs, d0, d1, d2, check)
+
+    def run_orders(self, check=True) -> DmptResult:
+        """D0 .. D_order through dmpt_run_orders (any supported order; the only run call for order 3)."""
+        t = self.torch
+        n = self.n
+        ds = [t.empty((n, n), dtype=t.float32, device=self.device) for _ in range(self.order + 1)]
+        r, bufs = self._new_result()
+        rc = dmpt_run_orders(self.ctx, [m.data_ptr() for m in ds], n, r)
+        ds += [None] * (4 - len(ds))
+        out = self._wrap(rc, r, bufs, ds[0], ds[1], ds[2], check)
+        out.d3 = ds[3]
+        return out
+
+    def layer_products3(self, s0, s1, s2, s3):
+        t = self.torch
+        x3 = t.empty((self.n, self.n), dtype=t.float32, device=self.device)
+        rc = dmpt_layer_products3(self.ctx, s0.data_ptr(), s1.data_ptr(), s2.data_ptr(), s3.data_ptr(), s0.stride(0),
+                                  x3.data_ptr(), self.n)
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_layer_products3", dmpt_last_cuda_error(self.ctx))
+        return x3
 
     def set_hamiltonian_fields(self, h0, h1s, n_occ):
         """h1s: num_fields perturbations sharing h0 (row-major fp32 CUDA matrices with h0's leading dimension)."""
@@ -444,10 +547,29 @@ class Dmpt:
             raise DmptError(rc, "dmpt_inverse_factor", dmpt_last_cuda_error(self.ctx))
         return z, it, err
 
-    def congruence(self, z, h):
-        """Z^T H Z for symmetric h: T = Z^T H = (Z^T).(H)^T, then T.Z = T.(Z^T)^T."""
-        zt = z.t().contiguous()
-        return self.product_nt(self.product_nt(zt, h), zt)
+    def congruence(self, z, x, transpose_z=True):
+        """Z^T X Z (transpose_z, Eq. 81) or Z X Z^T for symmetric x: one dmpt_congruence call."""
+        t = self.torch
+        if z.stride(0) != x.stride(0):
+            raise DmptError(DMPT_EINVAL, "congruence", "z and x need the same leading dimension")
+        c = t.empty((self.n, self.n), dtype=t.float32, device=self.device)
+        rc = dmpt_congruence(self.ctx, z.data_ptr(), x.data_ptr(), z.stride(0), 1 if transpose_z else 0, c.data_ptr(),
+                             self.n)
+        if rc != DMPT_OK:
+            raise DmptError(rc, "dmpt_congruence", dmpt_last_cuda_error(self.ctx))
+        return c
+
+    def fd_response(self, h0, h1, n_occ, h, points=2, check=True):
+        """(D1 by the 2- or 4-point stencil of PAPER.md Eqs. 83-84, layer counts of the runs, ms): order-0 contexts."""
+        t = self.torch
+        if h0.stride(0) != h1.stride(0):
+            raise DmptError(DMPT_EINVAL, "fd_response", "h0 and h1 need the same leading dimension")
+        d1 = t.empty((self.n, self.n), dtype=t.float32, device=self.device)
+        rc, layers, ms = dmpt_fd_response(self.ctx, h0.data_ptr(), h1.data_ptr(), h0.stride(0), n_occ, h, points,
+                                          d1.data_ptr(), self.n)
+        if rc != DMPT_OK and check:
+            raise DmptError(rc, "dmpt_fd_response", dmpt_last_cuda_error(self.ctx))
+        return d1, layers, ms
 
     def spectral_bounds(self, h0):
         rc, lo, hi = dmpt_spectral_bounds(self.ctx, h0.data_ptr(), h0.stride(0))
@@ -480,6 +602,83 @@ class Dmpt:
             dmpt_destroy(self.ctx)
             self.ctx = None
             self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class DmptPair:
+    """Order-parallel pair (dmpt_pair_*): the order-0 side on `device0`, the order-1 side on `device1` (the same
+    device is allowed).  Owns both torch-allocated workspaces.  Marshalling only."""
+
+    def __init__(self, n, device0="cuda:0", device1="cuda:0", max_layers=200, s0_shift=-1, s1_autoscale=True,
+                 bounds=None, wave_sync=True, epilogue_direct=False):
+        import torch
+
+        self.torch = torch
+        self.n = int(n)
+        self.order = 1
+        self.num_fields = 1
+        self.dev = [torch.device(device0), torch.device(device1)]
+        if any(d.type != "cuda" for d in self.dev):
+            raise DmptError(DMPT_ECUDA, "DmptPair", "CUDA devices are required; there is no CPU path")
+        opt = dmpt_default_options()
+        opt.max_layers = min(int(max_layers) if int(max_layers) > 0 else 200, 1024)
+        opt.order = 1
+        opt.s0_shift = int(s0_shift)
+        opt.s1_autoscale = 1 if s1_autoscale else 0
+        opt.wave_sync = 1 if wave_sync else 0
+        opt.epilogue_direct = 1 if epilogue_direct else 0
+        if bounds is not None:
+            opt.bounds = 1
+            opt.eps_min, opt.eps_max = float(bounds[0]), float(bounds[1])
+        self.max_layers = opt.max_layers
+        self.ws = []
+        for side, d in enumerate(self.dev):
+            nbytes = dmpt_pair_workspace_bytes(self.n, side)
+            if nbytes == 0:
+                raise DmptError(DMPT_EINVAL, "dmpt_pair_workspace_bytes")
+            self.ws.append(torch.empty(nbytes, dtype=torch.uint8, device=d))
+        idx = [d.index if d.index is not None else torch.cuda.current_device() for d in self.dev]
+        self.pair = dmpt_pair_create(self.n, opt, idx[0], self.ws[0].data_ptr(), self.ws[0].numel(),
+                                     idx[1], self.ws[1].data_ptr(), self.ws[1].numel())
+        self._h = None
+
+    _new_result = Dmpt._new_result
+    _wrap_result = Dmpt._wrap
+
+    def set_hamiltonian(self, h0, h1, n_occ):
+        t = self.torch
+        for m, d in ((h0, self.dev[0]), (h1, self.dev[1])):
+            if not (m.is_cuda and m.dtype == t.float32 and m.dim() == 2 and m.stride(1) == 1
+                    and m.stride(0) == h0.stride(0) and m.device.index == (d.index if d.index is not None else 0)):
+                raise DmptError(DMPT_EINVAL, "DmptPair.set_hamiltonian",
+                                "need row-major fp32 matrices, h0 on device0 and h1 on device1, one leading dimension")
+        self._h = (h0, h1)
+        dmpt_pair_set_hamiltonian(self.pair, h0.data_ptr(), h1.data_ptr(), h0.stride(0), n_occ)
+
+    def run(self, check=True) -> DmptResult:
+        t = self.torch
+        n = self.n
+        for d in self.dev:            # inputs may have been produced on torch's streams; the pair owns its own
+            t.cuda.synchronize(d)
+        d0 = t.empty((n, n), dtype=t.float32, device=self.dev[0])
+        d1 = t.empty((n, n), dtype=t.float32, device=self.dev[1])
+        r, bufs = self._new_result()
+        rc = dmpt_pair_run(self.pair, d0.data_ptr(), d1.data_ptr(), n, r)
+        if rc not in (DMPT_OK, DMPT_ENOCONV) and check:
+            raise DmptError(rc, "dmpt_pair_run", dmpt_pair_last_cuda_error(self.pair))
+        self.ctx = None
+        return self._wrap_result(rc, r, bufs, d0, d1, None, False)
+
+    def close(self):
+        if getattr(self, "pair", None) is not None:
+            dmpt_pair_destroy(self.pair)
+            self.pair = None
+            self.ws = []
 
     def __del__(self):
         try:

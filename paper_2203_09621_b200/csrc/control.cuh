@@ -62,6 +62,7 @@ struct DmptCtl {
     unsigned int ticket;  // CTA arrival counter of the running launch
     unsigned int wave;    // wave-boundary arrivals of the running launch (LayerParams::wave_sync)
     unsigned int wave2;   // the same for the order-2 pass of the layer
+    unsigned int wave3;   // the same for the order-3 pass of the layer
     double n_s;     // Tr S0_{n-1}
     double n_x;     // ||S0_{n-1}||_F^2
     double fro0;    // FroErr0
@@ -82,6 +83,24 @@ struct DmptLogs {   // device arrays, max_layers entries, entry n-1 for layer n
 struct DmptProblem {
     int n, n_pad, n_occ, order, max_layers, s0_shift, s1_autoscale;
     int nfields;     // 1..3 perturbations sharing H0 (order 1 only above 1)
+    int pair_side;   // order-parallel pair: 0 = the whole path on one device;
+                     // 1 = the order-0 side (S0^2, sigma_n, Algorithm 2); 2 = the order-1 side (S0.S1 + S1.S0, Algorithm 3)
+};
+
+// Order-parallel pair: what the order-0 side hands to the order-1 side for layer n, next to the operand pair
+// (Mhi, Mlo) of S0_{n-1}.  One record per layer, written by the order-0 side's control step when it decides layer n,
+// copied device to device, read by the order-1 side's launch of layer n.  valid = 0: the order-0 side had already
+// finished (S0 frozen) - the order-1 side then flips sigma itself.
+struct DmptHandoff {
+    int valid;
+    int sigma;      // sigma_n
+    int conv0;      // Algorithm 2 has fired (on layer n or before): FroErr1_n is wanted
+    int n_c;
+    int s0_buf;     // operand buffer holding M of S0_{n-1}
+    int done;       // the order-0 side stopped with an error (status below)
+    int status;
+    int pad_;
+    double fro0;    // FroErr0 (known from layer n_c + 1 on)
 };
 
 // exact power of two 2^e bringing m into [8, 16); 0 when m is 0 or not finite
@@ -126,7 +145,7 @@ __device__ inline void control_decide(DmptCtl& c, const DmptLogs& L, const DmptP
             c.conv0 = 1;
             c.n_c = n;
             c.mode0 = MODE_STOP;      // X0 is still formed once, for FroErr0 (R4)
-            if (pb.order == 0) {      // ground-state mode: D0 = S0_{n-1} is the answer, nothing left to measure
+            if (pb.order == 0 && pb.pair_side == 0) {      // ground-state mode: D0 = S0_{n-1} is the answer, nothing left to measure
                 c.layers = n;         // counted like the oracle's loop: the pass on which the test fired
                 c.fro0 = nan("");
                 c.done = 1;
@@ -175,10 +194,43 @@ __device__ inline void response_step(DmptCtl& c, const DmptProblem& pb, int n, b
     }
 }
 
+// Order-parallel pair, order-1 side: overlay the order-0 side's decision for layer c.layer on the local state.
+// This side never forms S0^2: for its launch S0 is always "frozen", whatever the other side is doing with it.
+__device__ inline void handoff_merge(DmptCtl& c, const DmptHandoff& h) {
+    c.mode0 = MODE_FROZEN;
+    if (!h.valid) return;
+    c.sigma = h.sigma;
+    c.conv0 = h.conv0;
+    c.n_c = h.n_c;
+    c.s0_buf = h.s0_buf;
+    c.fro0 = h.fro0;
+    if (h.done && h.status != 0) {
+        c.done = 1;
+        c.status = h.status;
+    }
+}
+
+// Order-0 side: publish the decision just taken for layer c.layer.
+__device__ inline void handoff_publish(const DmptCtl& c, DmptHandoff* out) {
+    DmptHandoff h;
+    h.valid = 1;
+    h.sigma = c.sigma;
+    h.conv0 = c.conv0;
+    h.n_c = c.n_c;
+    h.s0_buf = c.s0_buf;
+    h.done = c.done;
+    h.status = c.status;
+    h.pad_ = 0;
+    h.fro0 = c.fro0;
+    out[c.layer] = h;
+}
+
 // After layer n = ctl.layer ran: fold its reductions into the state, apply Algorithm 3
-// (cascade for order 2, reading R15) and decide layer n+1.
+// (cascade for orders 2 and 3, reading R15) and decide layer n+1.
+// `handoff`: order-parallel pair only (DmptProblem::pair_side): the records the order-0 side writes (side 1) or the
+// copies of them the order-1 side reads (side 2; the caller has already merged handoff[n] into c).
 __device__ inline void control_finalize(DmptCtl& c, const DmptLogs& L, const DmptProblem& pb,
-                                        const double* red /* RED_COUNT sums */) {
+                                        const double* red /* RED_COUNT sums */, DmptHandoff* handoff = nullptr) {
     const int n = c.layer;
     c.layers = n;
     if (c.single_shot) {
@@ -192,16 +244,39 @@ __device__ inline void control_finalize(DmptCtl& c, const DmptLogs& L, const Dmp
     } else if (c.mode0 == MODE_STOP) {
         c.fro0 = sqrt(red[RED_FRO0]);
     }
+    if (pb.pair_side == 1) {
+        // ---- order-0 side of a pair: after the stop layer (FroErr0 measured) nothing is left to do here; the
+        //      last record tells the other side that S0 is frozen and what FroErr0 is
+        L.fro1[n - 1] = nan("");
+        if (c.mode0 == MODE_STOP) {
+            if (!isfinite(c.fro0)) c.status = -6;
+            c.layer = n + 1;
+            c.sigma = -c.sigma;
+            c.mode0 = MODE_FROZEN;
+            c.done = 1;
+            handoff_publish(c, handoff);
+            return;
+        }
+        c.layer = n + 1;
+        control_decide(c, L, pb);
+        handoff_publish(c, handoff);
+        return;
+    }
+    if (pb.pair_side == 2) L.sigma[n - 1] = c.sigma;       // this side's log: the flips after the freeze start from it
     // ---- first order (slot 1): Algorithm 3, tested from layer n_c + 2 on
     if (pb.order >= 1)
         response_step(c, pb, n, c.conv0 != 0, c.n_c, c.conv1, c.n_c1, c.s1_buf, c.e1_in, c.e1_out, c.s1_max,
                       red[RED_FRO1], red[RED_MAX1], L.fro1);
     else
         L.fro1[n - 1] = nan("");
-    if (pb.order == 2) {
+    if (pb.order >= 2) {
         // ---- second order (slot 2): the same test cascaded behind the D1 stop (reading R15)
         response_step(c, pb, n, c.conv1 != 0, c.n_c1, c.conv2, c.n_c2, c.s2_buf, c.e2_in, c.e2_out, c.s2_max,
                       red[RED_FRO2], red[RED_MAX2], L.fro2);
+        // ---- third order (slot 3): cascaded once more, behind the D2 stop
+        if (pb.order >= 3)
+            response_step(c, pb, n, c.conv2 != 0, c.n_c2, c.conv3, c.n_c3, c.s3_buf, c.e3_in, c.e3_out, c.s3_max,
+                          red[RED_FRO3], red[RED_MAX3], L.fro3);
     } else if (pb.nfields >= 2) {
         // ---- further first-order fields (slots 2, 3): each runs Algorithm 3 on its own, like slot 1
         response_step(c, pb, n, c.conv0 != 0, c.n_c, c.conv2, c.n_c2, c.s2_buf, c.e2_in, c.e2_out, c.s2_max,
@@ -215,11 +290,19 @@ __device__ inline void control_finalize(DmptCtl& c, const DmptLogs& L, const Dmp
         return;
     }
     const bool all_fields = c.conv1 && (pb.nfields < 2 || c.conv2) && (pb.nfields < 3 || c.conv3);
-    if (pb.order == 2 ? c.conv2 != 0 : (pb.order == 1 && all_fields)) {
+    if (pb.order == 3 ? c.conv3 != 0 : (pb.order == 2 ? c.conv2 != 0 : (pb.order == 1 && all_fields))) {
         c.done = 1;
         return;
     }
     c.layer = n + 1;
+    if (pb.pair_side == 2 && !c.conv0) {
+        // the decision for layer n + 1 arrives from the order-0 side with that layer's operands
+        if (c.layer > pb.max_layers) {
+            c.done = 1;
+            c.status = -5;  // DMPT_ENOCONV
+        }
+        return;
+    }
     control_decide(c, L, pb);
 }
 

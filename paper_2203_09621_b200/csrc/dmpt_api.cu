@@ -37,7 +37,8 @@ struct Carve {
 
 struct Layout {
     int n, n_pad, order, nfields, num_tiles;
-    size_t ctl, bounds, h1max, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, fro3, partials, partials2, tiles, tiles_full;
+    size_t ctl, bounds, h1max, s2_est, sigma, tr_s, tr_x, id_err, fro1, fro2, fro3, partials, partials2, partials3, handoff,
+        tiles, tiles_full;
     size_t s0, s1[2], s2[2], s3[2];
     size_t h[2][8];          // [buffer][S0hi, S0lo, S1hi, S1lo, slot-2 hi, lo, slot-3 hi, lo]
     size_t stage_h0, stage_h1;
@@ -51,8 +52,8 @@ int num_tiles_for(int nb) {
     return t;
 }
 
-// response slots in use: 1 (order 1), 2 (order 2, or two fields), 3 (three fields); 0 at order 0
-int num_slots(int order, int nfields) { return order == 2 ? 2 : (order == 1 ? nfields : 0); }
+// response slots in use: 1 (order 1), 2 (order 2, or two fields), 3 (order 3, or three fields); 0 at order 0
+int num_slots(int order, int nfields) { return order >= 2 ? order : (order == 1 ? nfields : 0); }
 
 Layout make_layout(int n, int order, int nfields) {
     Layout L{};
@@ -67,7 +68,7 @@ Layout make_layout(int n, int order, int nfields) {
     L.ctl = c.take(sizeof(DmptCtl));
     L.bounds = c.take(2 * sizeof(long long));
     L.h1max = c.take(4 * sizeof(unsigned int));
-    L.s2_est = c.take(sizeof(unsigned long long));
+    L.s2_est = c.take(4 * sizeof(unsigned long long));
     L.sigma = c.take(kMaxLayersCap * sizeof(int));
     L.tr_s = c.take(kMaxLayersCap * sizeof(double));
     L.tr_x = c.take(kMaxLayersCap * sizeof(double));
@@ -77,6 +78,8 @@ Layout make_layout(int n, int order, int nfields) {
     L.fro3 = c.take(kMaxLayersCap * sizeof(double));
     L.partials = c.take(kPartialDoubles * sizeof(double));
     L.partials2 = c.take(kPartialDoubles * sizeof(double));
+    L.partials3 = c.take(kPartialDoubles * sizeof(double));
+    L.handoff = c.take((kMaxLayersCap + 2) * sizeof(DmptHandoff));
     L.tiles = c.take((size_t)L.num_tiles * sizeof(uint32_t));
     L.tiles_full = c.take((size_t)(nb / 2) * nb * sizeof(uint32_t));
     L.s0 = c.take(np2 * 4);
@@ -189,7 +192,7 @@ extern "C" void dmpt_default_options(dmpt_options* opt) {
 }
 
 extern "C" size_t dmpt_workspace_bytes(int n, int order) {
-    if (n <= 0 || order < 0 || order > 2 || n > 65535 * kTile) return 0;
+    if (n <= 0 || order < 0 || order > 3 || n > 65535 * kTile) return 0;
     return make_layout(n, order, 1).total;
 }
 
@@ -270,13 +273,22 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
     return DMPT_OK;
 }
 
+static int create_impl(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_workspace, size_t workspace_bytes,
+                       void* cuda_stream, int pair_side);
+
 extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_workspace,
                            size_t workspace_bytes, void* cuda_stream) {
+    return create_impl(out, n, opt, d_workspace, workspace_bytes, cuda_stream, 0);
+}
+
+// pair_side: 0 = a context of its own; 1, 2 = the two sides of an order-parallel pair (dmpt_pair_create)
+static int create_impl(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_workspace, size_t workspace_bytes,
+                       void* cuda_stream, int pair_side) {
     if (!out) return DMPT_EINVAL;
     *out = nullptr;
     dmpt_options o;
     if (opt) o = *opt; else dmpt_default_options(&o);
-    if (n <= 0 || o.order < 0 || o.order > 2 || !d_workspace) return DMPT_EINVAL;
+    if (n <= 0 || o.order < 0 || o.order > 3 || !d_workspace) return DMPT_EINVAL;
     if (o.max_layers <= 0) o.max_layers = 200;
     if (o.max_layers > kMaxLayersCap) o.max_layers = kMaxLayersCap;
     if (o.s0_shift > 15) return DMPT_EINVAL;
@@ -334,6 +346,7 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<1>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<2>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<3>()));
+    CKC(cudaFuncSetAttribute(dmpt_layer_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<4>()));
 
     const Layout& L = ctx->L;
     const int nb = L.n_pad / kTile;
@@ -391,6 +404,9 @@ extern "C" int dmpt_create(dmpt_ctx** out, int n, const dmpt_options* opt, void*
     lp.logs.fro3 = ctx->at<double>(L.fro3);
     lp.partials = ctx->at<double>(L.partials);
     lp.partials2 = ctx->at<double>(L.partials2);
+    lp.partials3 = ctx->at<double>(L.partials3);
+    lp.handoff = pair_side ? ctx->at<DmptHandoff>(L.handoff) : nullptr;
+    lp.pb.pair_side = pair_side;
     lp.pb.n = n;
     lp.pb.n_pad = L.n_pad;
     lp.pb.n_occ = 0;
@@ -462,7 +478,13 @@ extern "C" int dmpt_set_hamiltonian_fields(dmpt_ctx* ctx, const float* d_h0, con
 }
 
 static int launch_layer(dmpt_ctx* ctx, int* launches) {
-    if (ctx->opt.order == 2) {
+    if (ctx->opt.order >= 2) {
+        // highest order first: every pass reads the iterates the lower-order passes of this layer are about to replace
+        if (ctx->opt.order == 3) {
+            int rc = launch_pass<4>(ctx);
+            if (rc) return rc;
+            ++*launches;
+        }
         int rc = launch_pass<1>(ctx);
         if (rc) return rc;
         ++*launches;
@@ -552,17 +574,22 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     int tgrid = 0;
     int rc0 = launch_transform_split(ctx, d_h0, h1p, ld, nf, &tgrid);
     if (rc0) return rc0;
-    dmpt_control_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.logs, ctx->lp.pb, partials, tgrid);
+    dmpt_control_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.logs, ctx->lp.pb, partials, tgrid, ctx->lp.handoff);
     CK(cudaGetLastError());
     CK(cudaEventRecord(ctx->ev_t[5], st));
     *launches += 4;
-    if (ctx->opt.order == 2) {      // S2_0 = 0 (H2 = 0): fp32 iterate and its operands
+    if (ctx->opt.order >= 2) {      // S2_0 = 0 (H2 = 0): fp32 iterate and its operands
         const size_t np2 = (size_t)np * np;
         CK(cudaMemsetAsync(ctx->lp.s2[0], 0, np2 * 4, st));
         CK(cudaMemsetAsync(ctx->lp.h[0][4], 0, np2 * 2, st));
         CK(cudaMemsetAsync(ctx->lp.h[0][5], 0, np2 * 2, st));
+        if (ctx->opt.order == 3) {  // S3_0 = 0 likewise
+            CK(cudaMemsetAsync(ctx->lp.s3[0], 0, np2 * 4, st));
+            CK(cudaMemsetAsync(ctx->lp.h[0][6], 0, np2 * 2, st));
+            CK(cudaMemsetAsync(ctx->lp.h[0][7], 0, np2 * 2, st));
+        }
         unsigned long long* est = ctx->at<unsigned long long>(L.s2_est);
-        CK(cudaMemsetAsync(est, 0, sizeof *est, st));
+        CK(cudaMemsetAsync(est, 0, 4 * sizeof *est, st));
         dmpt_rowsq_max_kernel<<<elementwise_grid(ctx, (long long)np * 32, 256), 256, 0, st>>>(ctx->lp.s1[0], np, est);
         CK(cudaGetLastError());
         dmpt_s2_scale_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, est);
@@ -580,6 +607,20 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
         for (int i = 0; i < chunk_len && launched < max_layers; ++i, ++launched) {
             int rc = launch_layer(ctx, launches);
             if (rc) return rc;
+            if (ctx->opt.order == 3 && launched == 0) {
+                // S3_0 = S3_1 = 0: the first non-zero iterate is S3_2 = sigma_2 (S1_1 S2_1 + S2_1 S1_1), written by
+                // layer 2, and the scale of its split has no predecessor to go by.  Cauchy-Schwarz on the rows:
+                // max|S3_2| <= 2 max_i ||row_i S1_1|| max_j ||row_j S2_1||; two HBM passes (reading R12 at order 3).
+                unsigned long long* est = ctx->at<unsigned long long>(L.s2_est);
+                const int rg = elementwise_grid(ctx, (long long)np * 32, 256);
+                dmpt_rowsq_max_kernel<<<rg, 256, 0, st>>>(ctx->lp.s1[1], np, est + 1);
+                CK(cudaGetLastError());
+                dmpt_rowsq_max_kernel<<<rg, 256, 0, st>>>(ctx->lp.s2[1], np, est + 2);
+                CK(cudaGetLastError());
+                dmpt_s3_scale_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, est + 1, est + 2);
+                CK(cudaGetLastError());
+                *launches += 3;
+            }
         }
         CK(cudaMemcpyAsync(&ctx->h_flags[chunks % kFlagSlots], &ctl->done, sizeof(int), cudaMemcpyDeviceToHost, st));
         if (h_d0_early)
@@ -648,15 +689,15 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
             if (res->tr_x) CK(cudaMemcpy(res->tr_x, ctx->at<double>(L.tr_x), nl * sizeof(double), cudaMemcpyDeviceToHost));
             if (res->id_err) CK(cudaMemcpy(res->id_err, ctx->at<double>(L.id_err), nl * sizeof(double), cudaMemcpyDeviceToHost));
             if (res->fro_err1) CK(cudaMemcpy(res->fro_err1, ctx->at<double>(L.fro1), nl * sizeof(double), cudaMemcpyDeviceToHost));
-            if (res->fro_err2 && (ctx->opt.order == 2 || ctx->opt.num_fields > 1))
+            if (res->fro_err2 && (ctx->opt.order >= 2 || ctx->opt.num_fields > 1))
                 CK(cudaMemcpy(res->fro_err2, ctx->at<double>(L.fro2), nl * sizeof(double), cudaMemcpyDeviceToHost));
-            if (res->fro_err3 && ctx->opt.num_fields > 2)
+            if (res->fro_err3 && (ctx->opt.num_fields > 2 || ctx->opt.order == 3))
                 CK(cudaMemcpy(res->fro_err3, ctx->at<double>(L.fro3), nl * sizeof(double), cudaMemcpyDeviceToHost));
             // the norms were taken on the prescaled iterates (DmptCtl::p1..p3; 0 in all but extreme cases)
-            const int pw[3] = {c.p1, ctx->opt.order == 2 ? 2 * c.p1 : c.p2, c.p3};
+            const int pw[3] = {c.p1, ctx->opt.order >= 2 ? 2 * c.p1 : c.p2, ctx->opt.order == 3 ? 3 * c.p1 : c.p3};
             double* logs[3] = {res->fro_err1, res->fro_err2, res->fro_err3};
             for (int k = 0; k < 3; ++k)
-                if (logs[k] && pw[k] != 0 && (k == 0 || ctx->opt.order == 2 || ctx->opt.num_fields > k))
+                if (logs[k] && pw[k] != 0 && (k == 0 || ctx->opt.order > k || ctx->opt.num_fields > k))
                     for (int i = 0; i < nl; ++i) logs[k][i] = ldexp(logs[k][i], -pw[k]);
         }
     }
@@ -677,9 +718,9 @@ static int unscale_outputs(dmpt_ctx* ctx, int* launches) {
     const int np = ctx->L.n_pad;
     const int order = ctx->opt.order, nf = ctx->opt.num_fields;
     float* buf[3] = {order >= 1 ? ctx->lp.s1[c.s1_buf & 1] : nullptr,
-                     (order == 2 || nf >= 2) ? ctx->lp.s2[c.s2_buf & 1] : nullptr,
-                     nf >= 3 ? ctx->lp.s3[c.s3_buf & 1] : nullptr};
-    const int pw[3] = {c.p1, order == 2 ? 2 * c.p1 : c.p2, c.p3};
+                     (order >= 2 || nf >= 2) ? ctx->lp.s2[c.s2_buf & 1] : nullptr,
+                     (order == 3 || nf >= 3) ? ctx->lp.s3[c.s3_buf & 1] : nullptr};
+    const int pw[3] = {c.p1, order >= 2 ? 2 * c.p1 : c.p2, order == 3 ? 3 * c.p1 : c.p3};
     for (int k = 0; k < 3; ++k)
         if (buf[k] && pw[k] != 0) {
             dmpt_unscale_kernel<<<elementwise_grid(ctx, (long long)np * np, 256), 256, 0, ctx->stream>>>(buf[k], np, -pw[k]);
@@ -689,10 +730,11 @@ static int unscale_outputs(dmpt_ctx* ctx, int* launches) {
     return DMPT_OK;
 }
 
-extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, int ld, dmpt_result* res) {
-    if (!ctx || !d_d0 || (!d_d1 && ctx->opt.order != 0)) return DMPT_EINVAL;
+static int run_orders_impl(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, float* d_d3, int ld, dmpt_result* res) {
+    const int order = ctx->opt.order;
+    if (!d_d0 || (!d_d1 && order >= 1) || (!d_d2 && order >= 2) || (!d_d3 && order >= 3)) return DMPT_EINVAL;
     if (!ctx->d_h0) return DMPT_ESTATE;
-    if (ld < ctx->n || (ctx->opt.order == 2 && !d_d2) || ctx->opt.num_fields > 1) return DMPT_EINVAL;
+    if (ld < ctx->n || ctx->opt.num_fields > 1) return DMPT_EINVAL;
     const Layout& L = ctx->L;
     const size_t n = ctx->n, np = L.n_pad;
     int launches = 0;
@@ -702,13 +744,28 @@ extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, in
     if ((rc = fetch_ctl(ctx))) return rc;
     if ((rc = unscale_outputs(ctx, &launches))) return rc;
     CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
-    if (ctx->opt.order >= 1)
+    if (order >= 1)
         CK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
                              cudaMemcpyDeviceToDevice, ctx->stream));
-    if (ctx->opt.order == 2)
+    if (order >= 2)
         CK(cudaMemcpy2DAsync(d_d2, (size_t)ld * 4, ctx->lp.s2[ctx->h_ctl->s2_buf & 1], np * 4, n * 4, n,
                              cudaMemcpyDeviceToDevice, ctx->stream));
+    if (order >= 3)
+        CK(cudaMemcpy2DAsync(d_d3, (size_t)ld * 4, ctx->lp.s3[ctx->h_ctl->s3_buf & 1], np * 4, n * 4, n,
+                             cudaMemcpyDeviceToDevice, ctx->stream));
     return finish(ctx, res, launches);
+}
+
+extern "C" int dmpt_run(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2, int ld, dmpt_result* res) {
+    if (!ctx || ctx->opt.order > 2) return DMPT_EINVAL;          // order 3 has one more output: dmpt_run_orders
+    return run_orders_impl(ctx, d_d0, d_d1, d_d2, nullptr, ld, res);
+}
+
+extern "C" int dmpt_run_orders(dmpt_ctx* ctx, float* const* d_d, int ld, dmpt_result* res) {
+    if (!ctx || !d_d) return DMPT_EINVAL;
+    const int order = ctx->opt.order;
+    return run_orders_impl(ctx, d_d[0], order >= 1 ? d_d[1] : nullptr, order >= 2 ? d_d[2] : nullptr,
+                           order >= 3 ? d_d[3] : nullptr, ld, res);
 }
 
 extern "C" int dmpt_run_fields(dmpt_ctx* ctx, float* d_d0, float* const* d_d1, int ld, dmpt_result* res) {
@@ -740,7 +797,7 @@ extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1
     if (!ctx || !h_h0 || !h_d0) return DMPT_EINVAL;
     if (ctx->opt.order != 0 && (!h_h1 || !h_d1)) return DMPT_EINVAL;
     if (ld_in < ctx->n || ld_out < ctx->n || n_occ <= 0 || n_occ >= ctx->n) return DMPT_EINVAL;
-    if ((ctx->opt.order == 2 && !h_d2) || ctx->opt.num_fields > 1) return DMPT_EINVAL;
+    if ((ctx->opt.order == 2 && !h_d2) || ctx->opt.num_fields > 1 || ctx->opt.order > 2) return DMPT_EINVAL;
     const Layout& L = ctx->L;
     const size_t n = ctx->n, np = L.n_pad;
     float* s_h0 = ctx->at<float>(L.stage_h0);
@@ -775,12 +832,15 @@ extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1
 // ---------------------------------------------------------------------------------------------
 namespace {
 __global__ void single_shot_init_kernel(DmptCtl* ctl, DmptProblem pb, const double* __restrict__ partials,
-                                        const double* __restrict__ partials2 /* max|S2| or NULL */, int nblocks) {
+                                        const double* __restrict__ partials2 /* max|S2| or NULL */,
+                                        const double* __restrict__ partials3 /* max|S3| or NULL */, int nblocks) {
     if (threadIdx.x | blockIdx.x) return;
-    double m = 0.0, m2 = 0.0;
+    double m = 0.0, m2 = 0.0, m3 = 0.0;
     for (int b = 0; b < nblocks; ++b) m = fmax(m, partials[b]);
     if (partials2)
         for (int b = 0; b < nblocks; ++b) m2 = fmax(m2, partials2[b]);
+    if (partials3)
+        for (int b = 0; b < nblocks; ++b) m3 = fmax(m3, partials3[b]);
     DmptCtl c;
     memset(&c, 0, sizeof c);
     c.layer = 1;
@@ -791,6 +851,8 @@ __global__ void single_shot_init_kernel(DmptCtl* ctl, DmptProblem pb, const doub
     c.e1_in = c.e1_out = pb.s1_autoscale ? scale_exponent(m) : 0;
     c.s2_max = m2;
     c.e2_in = c.e2_out = pb.s1_autoscale ? scale_exponent(m2) : 0;
+    c.s3_max = m3;
+    c.e3_in = c.e3_out = pb.s1_autoscale ? scale_exponent(m3) : 0;
     *ctl = c;
 }
 }  // namespace
@@ -809,7 +871,7 @@ extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float
     CK(cudaGetLastError());
     dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s1, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
     CK(cudaGetLastError());
-    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, nullptr, grid);
+    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, nullptr, nullptr, grid);
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
@@ -828,7 +890,7 @@ extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float
 extern "C" int dmpt_layer_products2(dmpt_ctx* ctx, const float* d_s0, const float* d_s1, const float* d_s2, int ld,
                                     float* d_x2, int ld_out) {
     if (!ctx || !d_s0 || !d_s1 || !d_s2 || !d_x2) return DMPT_EINVAL;
-    if (ld < ctx->n || ld_out < ctx->n || ctx->opt.order != 2) return DMPT_EINVAL;
+    if (ld < ctx->n || ld_out < ctx->n || ctx->opt.order < 2) return DMPT_EINVAL;
     const Layout& L = ctx->L;
     const size_t n = ctx->n, np = L.n_pad;
     cudaStream_t st = ctx->stream;
@@ -842,7 +904,7 @@ extern "C" int dmpt_layer_products2(dmpt_ctx* ctx, const float* d_s0, const floa
     CK(cudaGetLastError());
     dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s2, (int)n, ld, (int)np, ctx->lp.s2[0], partials2);
     CK(cudaGetLastError());
-    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, partials2, grid);
+    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, partials2, nullptr, grid);
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
@@ -859,12 +921,51 @@ extern "C" int dmpt_layer_products2(dmpt_ctx* ctx, const float* d_s0, const floa
     return DMPT_OK;
 }
 
+extern "C" int dmpt_layer_products3(dmpt_ctx* ctx, const float* d_s0, const float* d_s1, const float* d_s2,
+                                    const float* d_s3, int ld, float* d_x3, int ld_out) {
+    if (!ctx || !d_s0 || !d_s1 || !d_s2 || !d_s3 || !d_x3) return DMPT_EINVAL;
+    if (ld < ctx->n || ld_out < ctx->n || ctx->opt.order != 3) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    double* partials = ctx->at<double>(L.partials);
+    double* partials2 = ctx->at<double>(L.partials2);
+    double* partials3 = ctx->at<double>(L.partials3);
+    const int grid = elementwise_grid(ctx, (long long)np * np, 256);
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s0, (int)n, ld, (int)np, ctx->lp.s0, partials);
+    CK(cudaGetLastError());
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s1, (int)n, ld, (int)np, ctx->lp.s1[0], partials);
+    CK(cudaGetLastError());
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s2, (int)n, ld, (int)np, ctx->lp.s2[0], partials2);
+    CK(cudaGetLastError());
+    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_s3, (int)n, ld, (int)np, ctx->lp.s3[0], partials3);
+    CK(cudaGetLastError());
+    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, partials2, partials3, grid);
+    CK(cudaGetLastError());
+    const long long c8 = (long long)np * np / 8;
+    const int sgrid = elementwise_grid(ctx, c8, 256);
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s0, (int)np, ctx->lp.h[0][0], ctx->lp.h[0][1], ctl, 0, ctx->s0_shift, 1);
+    CK(cudaGetLastError());
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s1[0], (int)np, ctx->lp.h[0][2], ctx->lp.h[0][3], ctl, 1, ctx->s0_shift, 0);
+    CK(cudaGetLastError());
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s2[0], (int)np, ctx->lp.h[0][4], ctx->lp.h[0][5], ctl, 2, ctx->s0_shift, 0);
+    CK(cudaGetLastError());
+    dmpt_split_kernel<<<sgrid, 256, 0, st>>>(ctx->lp.s3[0], (int)np, ctx->lp.h[0][6], ctx->lp.h[0][7], ctl, 3, ctx->s0_shift, 0);
+    CK(cudaGetLastError());
+    int rc = launch_pass<4>(ctx);
+    if (rc) return rc;
+    CK(cudaMemcpy2DAsync(d_x3, (size_t)ld_out * 4, ctx->lp.s3[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    return DMPT_OK;
+}
+
 // ---------------------------------------------------------------------------------------------
 // dmpt_product_nt: C = A.B^T for general n x n matrices in the dual half-precision representation
 // (the congruence transforms either side of the hot path are two of these)
 // ---------------------------------------------------------------------------------------------
 static int product_nt_impl(dmpt_ctx* ctx, const float* d_a, int lda, const float* d_b, int ldb, float* d_c, int ld_out,
-                           bool sync);
+                           bool sync, bool trans_a = false, bool trans_b = false);
 
 extern "C" int dmpt_product_nt(dmpt_ctx* ctx, const float* d_a, const float* d_b, int ld, float* d_c, int ld_out) {
     if (!ctx || !d_a || !d_b || !d_c) return DMPT_EINVAL;
@@ -873,8 +974,9 @@ extern "C" int dmpt_product_nt(dmpt_ctx* ctx, const float* d_a, const float* d_b
 }
 
 // C may alias A or B here: both are copied into the workspace before the product and C is written afterwards.
+// trans_a / trans_b: the operand is the TRANSPOSE of the caller's matrix (transposed while it is copied in).
 static int product_nt_impl(dmpt_ctx* ctx, const float* d_a, int lda, const float* d_b, int ldb, float* d_c, int ld_out,
-                           bool sync) {
+                           bool sync, bool trans_a, bool trans_b) {
     const Layout& L = ctx->L;
     const size_t n = ctx->n, np = L.n_pad;
     cudaStream_t st = ctx->stream;
@@ -883,11 +985,13 @@ static int product_nt_impl(dmpt_ctx* ctx, const float* d_a, int lda, const float
     double* partials2 = ctx->at<double>(L.partials2);
     const int grid = elementwise_grid(ctx, (long long)np * np, 256);
     // A -> the S0 buffers (operand pair 0, scale 2^e2), B -> the S1 buffers (operand pair 1, scale 2^e1)
-    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_a, (int)n, lda, (int)np, ctx->lp.s0, partials2);
+    if (trans_a) dmpt_pad_copy_t_kernel<<<grid, 256, 0, st>>>(d_a, (int)n, lda, (int)np, ctx->lp.s0, partials2);
+    else dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_a, (int)n, lda, (int)np, ctx->lp.s0, partials2);
     CK(cudaGetLastError());
-    dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_b, (int)n, ldb, (int)np, ctx->lp.s1[0], partials);
+    if (trans_b) dmpt_pad_copy_t_kernel<<<grid, 256, 0, st>>>(d_b, (int)n, ldb, (int)np, ctx->lp.s1[0], partials);
+    else dmpt_pad_copy_kernel<<<grid, 256, 0, st>>>(d_b, (int)n, ldb, (int)np, ctx->lp.s1[0], partials);
     CK(cudaGetLastError());
-    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, partials2, grid);
+    single_shot_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.pb, partials, partials2, nullptr, grid);
     CK(cudaGetLastError());
     const long long c8 = (long long)np * np / 8;
     const int sgrid = elementwise_grid(ctx, c8, 256);
@@ -900,6 +1004,67 @@ static int product_nt_impl(dmpt_ctx* ctx, const float* d_a, int lda, const float
     CK(cudaMemcpy2DAsync(d_c, (size_t)ld_out * 4, ctx->lp.s1[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     if (sync) CK(cudaStreamSynchronize(st));
     return DMPT_OK;
+}
+
+// Congruence transforms either side of the hot path (Eq. 81, A17-A18), two products each:
+//   transpose_z != 0:  C = Z^T X Z   (H_orth = Z^T H Z):  T = Z^T X^T (A = Z transposed on the way in, B = X), C = T (Z^T)^T
+//   transpose_z == 0:  C = Z X Z^T   (D = Z D_orth Z^T):  T = Z X^T,  C = T Z^T
+// X symmetric (X^T = X).  T lives in the workspace's staging buffer.
+extern "C" int dmpt_congruence(dmpt_ctx* ctx, const float* d_z, const float* d_x, int ld, int transpose_z, float* d_c,
+                               int ld_out) {
+    if (!ctx || !d_z || !d_x || !d_c) return DMPT_EINVAL;
+    if (ld < ctx->n || ld_out < ctx->n || ctx->opt.order < 1) return DMPT_EINVAL;
+    const int n = ctx->n;
+    float* t = ctx->at<float>(ctx->L.stage_h0);
+    int rc = product_nt_impl(ctx, d_z, ld, d_x, ld, t, n, false, transpose_z != 0, false);
+    if (rc) return rc;
+    return product_nt_impl(ctx, t, n, d_z, ld, d_c, ld_out, true, false, transpose_z != 0);
+}
+
+// ---------------------------------------------------------------------------------------------
+// dmpt_fd_response: D1 by finite differences of ground-state runs (Eqs. 83-84)
+// ---------------------------------------------------------------------------------------------
+extern "C" int dmpt_fd_response(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld, int n_occ, double h,
+                                int points, float* d_d1, int ld_out, int* h_layers, double* h_ms) {
+    if (!ctx || !d_h0 || !d_h1 || !d_d1 || ctx->opt.order != 0) return DMPT_EINVAL;
+    if (ld < ctx->n || ld_out < ctx->n || n_occ <= 0 || n_occ >= ctx->n || !(h > 0.0) || !isfinite(h)) return DMPT_EINVAL;
+    if (points != 2 && points != 4) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const int n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    float* hp = ctx->at<float>(L.stage_h0);          // H0 + t H1
+    // Eq. 83: (D(+h) - D(-h)) / 2h;   Eq. 84: (-D(+2h) + 8 D(+h) - 8 D(-h) + D(-2h)) / 12h
+    const double t2[2] = {1.0, -1.0}, w2[2] = {0.5, -0.5};
+    const double t4[4] = {2.0, 1.0, -1.0, -2.0}, w4[4] = {-1.0 / 12.0, 8.0 / 12.0, -8.0 / 12.0, 1.0 / 12.0};
+    const double* ts = points == 2 ? t2 : t4;
+    const double* ws = points == 2 ? w2 : w4;
+    ctx->n_occ = n_occ;
+    ctx->lp.pb.n_occ = n_occ;
+    const int egrid = elementwise_grid(ctx, (long long)n * n, 256);
+    double ms_sum = 0.0;
+    int status = DMPT_OK;
+    for (int k = 0; k < points; ++k) {
+        int launches = 0;
+        CK(cudaEventRecord(ctx->ev_t[0], st));
+        dmpt_axpy_kernel<<<egrid, 256, 0, st>>>(d_h0, d_h1, n, ld, ts[k] * h, hp);
+        CK(cudaGetLastError());
+        int rc = run_core(ctx, hp, nullptr, n, &launches);
+        if (rc) return rc;
+        if ((rc = fetch_ctl(ctx))) return rc;
+        dmpt_fd_accum_kernel<<<egrid, 256, 0, st>>>(ctx->lp.s0, n, np, ws[k] / h, k == 0, d_d1, ld_out);
+        CK(cudaGetLastError());
+        CK(cudaEventRecord(ctx->ev_t[3], st));
+        CK(cudaStreamSynchronize(st));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, ctx->ev_t[0], ctx->ev_t[3]));
+        ms_sum += ms;
+        const DmptCtl& c = *ctx->h_ctl;
+        if (h_layers) h_layers[k] = c.layers;
+        if (c.status != 0) status = c.status;
+        else if (!c.done && status == DMPT_OK) status = DMPT_ENOCONV;
+    }
+    if (h_ms) *h_ms = ms_sum;
+    return status;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1050,4 +1215,369 @@ extern "C" int dmpt_split(dmpt_ctx* ctx, const float* d_x, int ld, int shift, in
     CK(cudaMemcpy2DAsync(d_lo, (size_t)ld_out * 2, ctx->lp.h[0][1], np * 2, n * 2, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaStreamSynchronize(st));
     return DMPT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Order-parallel pair (Sec. III.C, 548-550): the order-0 side computes
+// f^(0) = S0^2 (sigma_n, Algorithm 2), the order-1 side f^(1) = S0.S1 + S1.S0 (Algorithm 3).  Per layer one one-way
+// hand-off: the operand pair (Mhi, Mlo) of S0_{n-1}, 4 N^2 bytes, and a DmptHandoff record, by cudaMemcpyPeerAsync on
+// a copy stream, so that it overlaps the products of both sides.  With both sides on one device the copies are
+// device-local and the two launches of a layer take turns on the SMs; the results are bit-identical to dmpt_run
+// either way (same kernels, same operands, same decisions).
+//
+//   events:  A_n  order-0 side finished layer n          (A_0: its initial transform)
+//            C_n  hand-off for layer n has landed        (operands of S0_{n-1}: written by the order-0 side's layer n-1)
+//            B_n  order-1 side finished layer n
+//   copy(n)  waits A_{n-1}, B_{n-2} (it overwrites the operand buffer layer n-2 of the order-1 side read; B_0 = that
+//            side's set-up)
+//   side 0, layer n  waits C_{n-1} (it overwrites the operand buffer copy(n-1) read)
+//   side 1, layer n  waits C_n
+// The host stays two layers ahead of either side (events A_{n-2}, B_{n-2}), so that no copy is issued once the
+// order-0 side has finished: a later copy would target the buffer the order-1 side keeps reading.
+// ---------------------------------------------------------------------------------------------
+namespace {
+constexpr int kPairRing = 4;
+}
+
+struct dmpt_pair {
+    dmpt_ctx* side[2] = {nullptr, nullptr};
+    int dev[2] = {0, 0};
+    int n = 0;
+    cudaStream_t st[2] = {nullptr, nullptr};
+    cudaStream_t copy = nullptr;                 // on dev[0]
+    cudaEvent_t evA[kPairRing]{}, evC[kPairRing]{}, evB[kPairRing]{};
+    cudaEvent_t ev_bounds = nullptr;
+    int* h_done[2] = {nullptr, nullptr};         // pinned, kPairRing entries each
+    char err[256] = {0};
+};
+
+#define PK(call)                                                                                     \
+    do {                                                                                             \
+        cudaError_t e_ = (call);                                                                     \
+        if (e_ != cudaSuccess) {                                                                     \
+            snprintf(pr->err, sizeof pr->err, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_),       \
+                     __FILE__, __LINE__);                                                            \
+            return DMPT_ECUDA;                                                                       \
+        }                                                                                            \
+    } while (0)
+
+extern "C" size_t dmpt_pair_workspace_bytes(int n, int side) {
+    if (n <= 0 || side < 0 || side > 1 || n > 65535 * kTile) return 0;
+    return make_layout(n, side, 1).total;
+}
+
+extern "C" const char* dmpt_pair_last_cuda_error(const dmpt_pair* pr) {
+    if (!pr) return "";
+    if (pr->err[0]) return pr->err;
+    for (int s = 0; s < 2; ++s)
+        if (pr->side[s] && pr->side[s]->err[0]) return pr->side[s]->err;
+    return "";
+}
+
+extern "C" int dmpt_pair_destroy(dmpt_pair* pr) {
+    if (!pr) return DMPT_EINVAL;
+    int cur = 0;
+    cudaGetDevice(&cur);
+    for (int s = 0; s < 2; ++s) {
+        cudaSetDevice(pr->dev[s]);
+        if (pr->st[s]) cudaStreamSynchronize(pr->st[s]);
+        if (s == 0 && pr->copy) cudaStreamSynchronize(pr->copy);
+        if (pr->side[s]) dmpt_destroy(pr->side[s]);
+        if (pr->h_done[s]) cudaFreeHost(pr->h_done[s]);
+    }
+    cudaSetDevice(pr->dev[0]);
+    for (auto& e : pr->evA) if (e) cudaEventDestroy(e);
+    for (auto& e : pr->evC) if (e) cudaEventDestroy(e);
+    if (pr->ev_bounds) cudaEventDestroy(pr->ev_bounds);
+    if (pr->copy) cudaStreamDestroy(pr->copy);
+    if (pr->st[0]) cudaStreamDestroy(pr->st[0]);
+    cudaSetDevice(pr->dev[1]);
+    for (auto& e : pr->evB) if (e) cudaEventDestroy(e);
+    if (pr->st[1]) cudaStreamDestroy(pr->st[1]);
+    cudaSetDevice(cur);
+    delete pr;
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_pair_create(dmpt_pair** out, int n, const dmpt_options* opt, int device0, void* d_workspace0,
+                                size_t workspace0_bytes, int device1, void* d_workspace1, size_t workspace1_bytes) {
+    if (!out) return DMPT_EINVAL;
+    *out = nullptr;
+    dmpt_options o;
+    if (opt) o = *opt; else dmpt_default_options(&o);
+    if (n <= 0 || o.order != 1 || o.num_fields > 1 || !d_workspace0 || !d_workspace1) return DMPT_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device0 < 0 || device1 < 0 || device0 >= ndev || device1 >= ndev)
+        return ndev == 0 ? DMPT_ECUDA : DMPT_EINVAL;
+    int cur = 0;
+    cudaGetDevice(&cur);
+    dmpt_pair* pr = new dmpt_pair();
+    pr->n = n;
+    pr->dev[0] = device0;
+    pr->dev[1] = device1;
+    auto fail = [&](int code) {
+        fprintf(stderr, "dmpt_pair_create: %s\n", dmpt_pair_last_cuda_error(pr));
+        dmpt_pair_destroy(pr);
+        cudaSetDevice(cur);
+        return code;
+    };
+#define PKC(call)                                                                          \
+    do {                                                                                   \
+        cudaError_t e_ = (call);                                                           \
+        if (e_ != cudaSuccess) {                                                           \
+            snprintf(pr->err, sizeof pr->err, "%s: %s", #call, cudaGetErrorString(e_));    \
+            return fail(DMPT_ECUDA);                                                       \
+        }                                                                                  \
+    } while (0)
+    void* ws[2] = {d_workspace0, d_workspace1};
+    const size_t wsb[2] = {workspace0_bytes, workspace1_bytes};
+    for (int s = 0; s < 2; ++s) {
+        PKC(cudaSetDevice(pr->dev[s]));
+        PKC(cudaStreamCreateWithFlags(&pr->st[s], cudaStreamNonBlocking));
+        PKC(cudaHostAlloc(&pr->h_done[s], kPairRing * sizeof(int), cudaHostAllocDefault));
+        if (s == 0) {
+            PKC(cudaStreamCreateWithFlags(&pr->copy, cudaStreamNonBlocking));
+            for (auto& e : pr->evA) PKC(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            for (auto& e : pr->evC) PKC(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            PKC(cudaEventCreateWithFlags(&pr->ev_bounds, cudaEventDisableTiming));
+        } else {
+            for (auto& e : pr->evB) PKC(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        }
+        dmpt_options os = o;
+        os.order = s;                      // side 0: S0 alone; side 1: the response product alone
+        os.num_fields = 1;
+        const int rc = create_impl(&pr->side[s], n, &os, ws[s], wsb[s], pr->st[s], s + 1);
+        if (rc != DMPT_OK) {
+            snprintf(pr->err, sizeof pr->err, "side %d: %s", s, dmpt_strerror(rc));
+            return fail(rc);
+        }
+    }
+    if (device0 != device1) {
+        // direct NVLink path for the hand-off when the devices are peers (the copies work without it, staged)
+        for (int s = 0; s < 2; ++s) {
+            int can = 0;
+            PKC(cudaDeviceCanAccessPeer(&can, pr->dev[s], pr->dev[s ^ 1]));
+            if (can) {
+                PKC(cudaSetDevice(pr->dev[s]));
+                const cudaError_t e = cudaDeviceEnablePeerAccess(pr->dev[s ^ 1], 0);
+                if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) {
+                    snprintf(pr->err, sizeof pr->err, "cudaDeviceEnablePeerAccess: %s", cudaGetErrorString(e));
+                    return fail(DMPT_ECUDA);
+                }
+                cudaGetLastError();
+            }
+        }
+    }
+#undef PKC
+    cudaSetDevice(cur);
+    *out = pr;
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_pair_set_hamiltonian(dmpt_pair* pr, const float* d_h0, const float* d_h1, int ld, int n_occ) {
+    if (!pr || !d_h0 || !d_h1 || ld < pr->n || n_occ <= 0 || n_occ >= pr->n) return DMPT_EINVAL;
+    for (int s = 0; s < 2; ++s) {
+        dmpt_ctx* c = pr->side[s];
+        c->d_h0 = s == 0 ? d_h0 : nullptr;
+        c->d_h1 = s == 1 ? d_h1 : nullptr;
+        c->ld_in = ld;
+        c->n_occ = n_occ;
+        c->lp.pb.n_occ = n_occ;
+    }
+    return DMPT_OK;
+}
+
+extern "C" int dmpt_pair_run(dmpt_pair* pr, float* d_d0, float* d_d1, int ld, dmpt_result* res) {
+    if (!pr || !d_d0 || !d_d1 || ld < pr->n) return DMPT_EINVAL;
+    dmpt_ctx* c0 = pr->side[0];
+    dmpt_ctx* c1 = pr->side[1];
+    if (!c0->d_h0 || !c1->d_h1) return DMPT_ESTATE;
+    const Layout& L0 = c0->L;
+    const Layout& L1 = c1->L;
+    const size_t n = pr->n, np = L0.n_pad;
+    const size_t op_bytes = np * np * 2;
+    int cur = 0;
+    cudaGetDevice(&cur);
+    struct Restore { int d; ~Restore() { cudaSetDevice(d); } } restore{cur};
+    int launches = 0;
+    DmptCtl* ctl0 = c0->at<DmptCtl>(L0.ctl);
+    DmptCtl* ctl1 = c1->at<DmptCtl>(L1.ctl);
+    const H1Ptrs none{{nullptr, nullptr, nullptr}};
+
+    // ---- order-0 side: a1, then a2 + a3 for S0 alone, then the decision for layer 1 (handoff[1])
+    PK(cudaSetDevice(pr->dev[0]));
+    {
+        cudaStream_t st = pr->st[0];
+        PK(cudaEventRecord(c0->ev_t[0], st));
+        dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl0, c0->at<long long>(L0.bounds), c0->at<unsigned int>(L0.h1max));
+        PK(cudaGetLastError());
+        PK(cudaMemsetAsync(c0->lp.handoff, 0, (kMaxLayersCap + 2) * sizeof(DmptHandoff), st));
+        if (!c0->opt.bounds) {
+            dmpt_gershgorin_kernel<<<elementwise_grid(c0, (long long)n * 32, 256), 256, 0, st>>>(
+                c0->d_h0, none, (int)n, c0->ld_in, c0->at<long long>(L0.bounds), c0->at<unsigned int>(L0.h1max));
+            PK(cudaGetLastError());
+            ++launches;
+        }
+        dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(c0->at<long long>(L0.bounds), c0->at<unsigned int>(L0.h1max), ctl0,
+                                                    c0->lp.pb, c0->opt.bounds, c0->opt.eps_min, c0->opt.eps_max);
+        PK(cudaGetLastError());
+        PK(cudaEventRecord(pr->ev_bounds, st));
+        PK(cudaEventRecord(c0->ev_t[4], st));
+        int tgrid = 0;
+        if (launch_transform_split(c0, c0->d_h0, none, c0->ld_in, 0, &tgrid)) {
+            snprintf(pr->err, sizeof pr->err, "%s", c0->err);
+            return DMPT_ECUDA;
+        }
+        dmpt_control_init_kernel<<<1, 32, 0, st>>>(ctl0, c0->lp.logs, c0->lp.pb, c0->at<double>(L0.partials), tgrid,
+                                                   c0->lp.handoff);
+        PK(cudaGetLastError());
+        PK(cudaEventRecord(c0->ev_t[5], st));
+        PK(cudaEventRecord(c0->ev_t[1], st));
+        PK(cudaEventRecord(pr->evA[0], st));
+        launches += 4;
+    }
+    // ---- order-1 side: max|H1|, the bounds of the other side (16 bytes), a2 + a3 for S1 alone
+    PK(cudaSetDevice(pr->dev[1]));
+    {
+        cudaStream_t st = pr->st[1];
+        const H1Ptrs h1p{{c1->d_h1, nullptr, nullptr}};
+        PK(cudaEventRecord(c1->ev_t[0], st));
+        dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl1, c1->at<long long>(L1.bounds), c1->at<unsigned int>(L1.h1max));
+        PK(cudaGetLastError());
+        PK(cudaMemsetAsync(c1->lp.handoff, 0, (kMaxLayersCap + 2) * sizeof(DmptHandoff), st));
+        dmpt_gershgorin_kernel<<<elementwise_grid(c1, (long long)n * 32, 256), 256, 0, st>>>(
+            nullptr, h1p, (int)n, c1->ld_in, c1->at<long long>(L1.bounds), c1->at<unsigned int>(L1.h1max));
+        PK(cudaGetLastError());
+        PK(cudaStreamWaitEvent(st, pr->ev_bounds, 0));
+        // eps_min, eps_max as the order-0 side settled them (Gershgorin or caller-supplied)
+        PK(cudaMemcpyPeerAsync(&ctl1->eps_min, pr->dev[1], &ctl0->eps_min, pr->dev[0], 2 * sizeof(double), st));
+        dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(c1->at<long long>(L1.bounds), c1->at<unsigned int>(L1.h1max), ctl1,
+                                                    c1->lp.pb, 2, 0.0, 0.0);
+        PK(cudaGetLastError());
+        PK(cudaEventRecord(c1->ev_t[4], st));
+        int tgrid = 0;
+        if (launch_transform_split(c1, nullptr, h1p, c1->ld_in, 1, &tgrid)) {
+            snprintf(pr->err, sizeof pr->err, "%s", c1->err);
+            return DMPT_ECUDA;
+        }
+        dmpt_control_init_kernel<<<1, 32, 0, st>>>(ctl1, c1->lp.logs, c1->lp.pb, c1->at<double>(L1.partials), tgrid,
+                                                   c1->lp.handoff);
+        PK(cudaGetLastError());
+        PK(cudaEventRecord(c1->ev_t[5], st));
+        PK(cudaEventRecord(c1->ev_t[1], st));
+        PK(cudaEventRecord(pr->evB[0], st));          // B_0: this side's set-up is done (its handoff array is cleared)
+        launches += 5;
+    }
+
+    // ---- layers
+    const int max_layers = c1->opt.max_layers;
+    bool side0_live = true;
+    for (int l = 1; l <= max_layers; ++l) {
+        bool copied = false;
+        if (side0_live && l >= 3) {
+            PK(cudaEventSynchronize(pr->evA[(l - 2) % kPairRing]));
+            if (pr->h_done[0][(l - 2) % kPairRing]) side0_live = false;
+        }
+        if (side0_live) {
+            PK(cudaSetDevice(pr->dev[0]));
+            const int b = (l - 1) & 1;                  // operand buffer of S0_{l-1} while S0 is being updated
+            PK(cudaStreamWaitEvent(pr->copy, pr->evA[(l - 1) % kPairRing], 0));
+            PK(cudaStreamWaitEvent(pr->copy, pr->evB[l >= 3 ? (l - 2) % kPairRing : 0], 0));
+            PK(cudaMemcpyPeerAsync(c1->lp.h[b][MH], pr->dev[1], c0->lp.h[b][MH], pr->dev[0], op_bytes, pr->copy));
+            PK(cudaMemcpyPeerAsync(c1->lp.h[b][ML], pr->dev[1], c0->lp.h[b][ML], pr->dev[0], op_bytes, pr->copy));
+            PK(cudaMemcpyPeerAsync(c1->lp.handoff + l, pr->dev[1], c0->lp.handoff + l, pr->dev[0], sizeof(DmptHandoff),
+                                   pr->copy));
+            PK(cudaEventRecord(pr->evC[l % kPairRing], pr->copy));
+            copied = true;
+            if (l >= 2) PK(cudaStreamWaitEvent(pr->st[0], pr->evC[(l - 1) % kPairRing], 0));
+            if (launch_pass<0>(c0)) {
+                snprintf(pr->err, sizeof pr->err, "%s", c0->err);
+                return DMPT_ECUDA;
+            }
+            ++launches;
+            PK(cudaMemcpyAsync(&pr->h_done[0][l % kPairRing], &ctl0->done, sizeof(int), cudaMemcpyDeviceToHost, pr->st[0]));
+            PK(cudaEventRecord(pr->evA[l % kPairRing], pr->st[0]));
+        }
+        PK(cudaSetDevice(pr->dev[1]));
+        if (copied) PK(cudaStreamWaitEvent(pr->st[1], pr->evC[l % kPairRing], 0));
+        if (launch_pass<0>(c1)) {
+            snprintf(pr->err, sizeof pr->err, "%s", c1->err);
+            return DMPT_ECUDA;
+        }
+        ++launches;
+        PK(cudaMemcpyAsync(&pr->h_done[1][l % kPairRing], &ctl1->done, sizeof(int), cudaMemcpyDeviceToHost, pr->st[1]));
+        PK(cudaEventRecord(pr->evB[l % kPairRing], pr->st[1]));
+        if (l >= 3) {
+            PK(cudaEventSynchronize(pr->evB[(l - 2) % kPairRing]));
+            if (pr->h_done[1][(l - 2) % kPairRing]) break;
+        }
+    }
+
+    // ---- results: D0 from the order-0 side, D1 (the last ACCEPTED iterate) from the order-1 side
+    PK(cudaSetDevice(pr->dev[1]));
+    PK(cudaEventRecord(c1->ev_t[2], pr->st[1]));
+    if (fetch_ctl(c1)) { snprintf(pr->err, sizeof pr->err, "%s", c1->err); return DMPT_ECUDA; }
+    if (unscale_outputs(c1, &launches)) { snprintf(pr->err, sizeof pr->err, "%s", c1->err); return DMPT_ECUDA; }
+    PK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, c1->lp.s1[c1->h_ctl->s1_buf & 1], np * 4, n * 4, n,
+                         cudaMemcpyDeviceToDevice, pr->st[1]));
+    PK(cudaEventRecord(c1->ev_t[3], pr->st[1]));
+    PK(cudaSetDevice(pr->dev[0]));
+    PK(cudaStreamSynchronize(pr->copy));
+    if (fetch_ctl(c0)) { snprintf(pr->err, sizeof pr->err, "%s", c0->err); return DMPT_ECUDA; }
+    PK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, c0->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, pr->st[0]));
+    PK(cudaStreamSynchronize(pr->st[0]));
+    PK(cudaSetDevice(pr->dev[1]));
+    PK(cudaStreamSynchronize(pr->st[1]));
+
+    const DmptCtl& k0 = *c0->h_ctl;
+    const DmptCtl& k1 = *c1->h_ctl;
+    int status = k1.status != 0 ? k1.status : k0.status;
+    if (status == 0 && !k1.done) status = DMPT_ENOCONV;
+    if (res) {
+        res->status = status;
+        res->layers = k1.layers;
+        res->layers_d0 = k0.n_c;
+        res->layers_d1 = k1.n_c1;
+        res->layers_d2 = res->layers_d3 = 0;
+        res->launches = launches;
+        res->eps_min = k0.eps_min;
+        res->eps_max = k0.eps_max;
+        res->fro_err0 = k0.fro0;
+        float ms = 0.f;
+        PK(cudaEventElapsedTime(&ms, c1->ev_t[0], c1->ev_t[3]));
+        res->ms_total = ms;
+        PK(cudaEventElapsedTime(&ms, c1->ev_t[1], c1->ev_t[2]));
+        res->ms_loop = ms;
+        PK(cudaEventElapsedTime(&ms, c1->ev_t[0], c1->ev_t[4]));
+        res->ms_bounds = ms;
+        PK(cudaEventElapsedTime(&ms, c1->ev_t[4], c1->ev_t[5]));
+        res->ms_transform = ms;
+        res->ms_split = 0.0;
+        const int nl = k1.layers, nl0 = k0.layers < nl ? k0.layers : nl;
+        if (nl > 0) {
+            std::vector<int> sg(nl);
+            std::vector<double> tmp(nl);
+            if (res->sigma) {
+                PK(cudaMemcpy(sg.data(), c1->at<int>(L1.sigma), nl * sizeof(int), cudaMemcpyDeviceToHost));
+                for (int i = 0; i < nl; ++i) res->sigma[i] = (int8_t)sg[i];
+            }
+            if (res->fro_err1) {
+                PK(cudaMemcpy(res->fro_err1, c1->at<double>(L1.fro1), nl * sizeof(double), cudaMemcpyDeviceToHost));
+                if (k1.p1 != 0)
+                    for (int i = 0; i < nl; ++i) res->fro_err1[i] = ldexp(res->fro_err1[i], -k1.p1);
+            }
+            PK(cudaSetDevice(pr->dev[0]));
+            double* dst[3] = {res->tr_s, res->tr_x, res->id_err};
+            const size_t src[3] = {L0.tr_s, L0.tr_x, L0.id_err};
+            for (int k = 0; k < 3; ++k) {
+                if (!dst[k]) continue;
+                for (int i = 0; i < nl; ++i) dst[k][i] = NAN;
+                if (nl0 > 0) PK(cudaMemcpy(dst[k], c0->at<double>(src[k]), nl0 * sizeof(double), cudaMemcpyDeviceToHost));
+            }
+            // N_S is constant once S0 froze
+            if (res->tr_s && nl0 > 0)
+                for (int i = nl0; i < nl; ++i) res->tr_s[i] = res->tr_s[nl0 - 1];
+        }
+    }
+    return status;
 }

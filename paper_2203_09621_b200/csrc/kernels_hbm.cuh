@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(256) dmpt_transform_split_kernel(const Transfo
     const float scale0 = exp2f((float)a.s0_shift);
     const int n = a.n, ld = a.ld, n_pad = a.n_pad;
     const int c8_per_row = n_pad >> 3;
+    const bool with0 = a.h0 != nullptr;      // nullptr: the perturbations only (order-1 side of an order-parallel pair)
     bool vec = (ld & 3) == 0 && (reinterpret_cast<uintptr_t>(a.h0) & 15) == 0;
 #pragma unroll
     for (int f = 0; f < NF; ++f) vec = vec && (reinterpret_cast<uintptr_t>(a.h1[f]) & 15) == 0;
@@ -185,9 +186,11 @@ __global__ void __launch_bounds__(256) dmpt_transform_split_kernel(const Transfo
             if (row < n && col < n) {
                 const size_t off = (size_t)row * ld + col;
                 if (vec && col + 7 < n) {
-                    const float4 u0 = ldg_stream4(a.h0 + off), u1 = ldg_stream4(a.h0 + off + 4);
-                    x0[0] = u0.x; x0[1] = u0.y; x0[2] = u0.z; x0[3] = u0.w;
-                    x0[4] = u1.x; x0[5] = u1.y; x0[6] = u1.z; x0[7] = u1.w;
+                    if (with0) {
+                        const float4 u0 = ldg_stream4(a.h0 + off), u1 = ldg_stream4(a.h0 + off + 4);
+                        x0[0] = u0.x; x0[1] = u0.y; x0[2] = u0.z; x0[3] = u0.w;
+                        x0[4] = u1.x; x0[5] = u1.y; x0[6] = u1.z; x0[7] = u1.w;
+                    }
 #pragma unroll
                     for (int f = 0; f < NF; ++f) {
                         const float4 w0 = ldg_stream4(a.h1[f] + off), w1 = ldg_stream4(a.h1[f] + off + 4);
@@ -198,7 +201,7 @@ __global__ void __launch_bounds__(256) dmpt_transform_split_kernel(const Transfo
 #pragma unroll
                     for (int t = 0; t < 8; ++t)
                         if (col + t < n) {
-                            x0[t] = a.h0[off + t];
+                            if (with0) x0[t] = a.h0[off + t];
 #pragma unroll
                             for (int f = 0; f < NF; ++f) x1[f][t] = a.h1[f][off + t];
                         }
@@ -219,10 +222,12 @@ __global__ void __launch_bounds__(256) dmpt_transform_split_kernel(const Transfo
             }
             fro += (double)fsum[0] + (double)fsum[1];
             const size_t i8 = (size_t)row * n_pad + col;
-            *reinterpret_cast<float4*>(a.s0 + i8) = make_float4(o0[0], o0[1], o0[2], o0[3]);
-            *reinterpret_cast<float4*>(a.s0 + i8 + 4) = make_float4(o0[4], o0[5], o0[6], o0[7]);
-            *reinterpret_cast<uint4*>(a.mh + i8) = *reinterpret_cast<const uint4*>(hh);
-            *reinterpret_cast<uint4*>(a.ml + i8) = *reinterpret_cast<const uint4*>(ll);
+            if (with0) {
+                *reinterpret_cast<float4*>(a.s0 + i8) = make_float4(o0[0], o0[1], o0[2], o0[3]);
+                *reinterpret_cast<float4*>(a.s0 + i8 + 4) = make_float4(o0[4], o0[5], o0[6], o0[7]);
+                *reinterpret_cast<uint4*>(a.mh + i8) = *reinterpret_cast<const uint4*>(hh);
+                *reinterpret_cast<uint4*>(a.ml + i8) = *reinterpret_cast<const uint4*>(ll);
+            }
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
                 float o1[8];
@@ -285,6 +290,71 @@ __global__ void __launch_bounds__(256) dmpt_pad_copy_kernel(const float* __restr
     }
 }
 
+// the same copy of the TRANSPOSE of a caller matrix (dmpt_congruence: Z^T as the row operand of a product), through a
+// 32 x 33 shared-memory tile so that both the reads and the writes are full lines.  grid = (n_pad/32)^2 tiles,
+// grid-stride; 256 threads = 32 x 8.
+__global__ void __launch_bounds__(256) dmpt_pad_copy_t_kernel(const float* __restrict__ src, int n, int ld, int n_pad,
+                                                              float* __restrict__ dst,
+                                                              double* __restrict__ partials /* [grid] max */) {
+    __shared__ float tile[32][33];
+    __shared__ double sh[8];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int tiles_per_row = n_pad >> 5;
+    const long long num_tiles = (long long)tiles_per_row * tiles_per_row;
+    float mx = 0.f;
+    for (long long t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+        const int bi = (int)(t / tiles_per_row), bj = (int)(t - (long long)bi * tiles_per_row);   // dst tile (bi, bj)
+        // dst[bi*32 + r][bj*32 + c] = src[bj*32 + c][bi*32 + r]
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int sr = bj * 32 + ty + 8 * k, sc = bi * 32 + tx;
+            tile[ty + 8 * k][tx] = (sr < n && sc < n) ? src[(size_t)sr * ld + sc] : 0.f;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const float v = tile[tx][ty + 8 * k];
+            dst[(size_t)(bi * 32 + ty + 8 * k) * n_pad + bj * 32 + tx] = v;
+            mx = fmaxf(mx, fabsf(v));
+        }
+    }
+    double dmx = warp_max((double)mx);
+    if (tx == 0) sh[ty] = dmx;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double m = 0.0;
+        for (int w = 0; w < 8; ++w) m = fmax(m, sh[w]);
+        partials[blockIdx.x] = m;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Finite-difference response from ground-state runs (Eqs. 83-84): the two elementwise steps.
+//   dmpt_axpy_kernel:     out = H0 + t H1, formed in fp64 and rounded once (n x n, dense, leading dimension n)
+//   dmpt_fd_accum_kernel: acc = (first ? 0 : acc) + w D, w = stencil weight / (denominator h), fp64 per element
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dmpt_axpy_kernel(const float* __restrict__ h0, const float* __restrict__ h1, int n,
+                                                        int ld, double t, float* __restrict__ out) {
+    const long long total = (long long)n * n;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int row = (int)(i / n), col = (int)(i - (long long)row * n);
+        const size_t o = (size_t)row * ld + col;
+        out[i] = (float)((double)h0[o] + t * (double)h1[o]);
+    }
+}
+
+__global__ void __launch_bounds__(256) dmpt_fd_accum_kernel(const float* __restrict__ d, int n, int ld_d, double w, int first,
+                                                            float* __restrict__ acc, int ld_acc) {
+    const long long total = (long long)n * n;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int row = (int)(i / n), col = (int)(i - (long long)row * n);
+        const size_t oa = (size_t)row * ld_acc + col;
+        const double prev = first ? 0.0 : (double)acc[oa];
+        acc[oa] = (float)(prev + w * (double)d[(size_t)row * ld_d + col]);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Scalar set-up between the transform and the first layer: spectral bounds -> ctl (before the
 // transform), then first reductions -> ctl and the decision for layer 1 (after it).
@@ -307,8 +377,10 @@ __global__ void dmpt_bounds_to_ctl_kernel(const long long* __restrict__ bounds, 
                                           DmptCtl* ctl, DmptProblem pb, int use_given, double eps_min, double eps_max) {
     if (threadIdx.x | blockIdx.x) return;
     DmptCtl c = *ctl;
-    const double lo = use_given ? eps_min : ordered_to_dbl(bounds[0]);
-    const double hi = use_given ? eps_max : ordered_to_dbl(bounds[1]);
+    // use_given: 0 = the Gershgorin discs in `bounds`; 1 = the caller's numbers; 2 = already in ctl (order-parallel
+    // pair: copied from the order-0 side)
+    const double lo = use_given == 2 ? c.eps_min : (use_given ? eps_min : ordered_to_dbl(bounds[0]));
+    const double hi = use_given == 2 ? c.eps_max : (use_given ? eps_max : ordered_to_dbl(bounds[1]));
     c.eps_min = lo;
     c.eps_max = hi;
     const double w = hi - lo;
@@ -348,7 +420,7 @@ __global__ void dmpt_bounds_to_ctl_kernel(const long long* __restrict__ bounds, 
 
 // First reductions -> ctl and the decision for layer 1.  One warp, fixed summation order.
 __global__ void dmpt_control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProblem pb,
-                                         const double* __restrict__ partials, int nblocks) {
+                                         const double* __restrict__ partials, int nblocks, DmptHandoff* handoff) {
     if (blockIdx.x || threadIdx.x >= 32) return;
     double t = 0.0, f = 0.0;
     for (int b = threadIdx.x; b < nblocks; b += 32) {
@@ -362,7 +434,12 @@ __global__ void dmpt_control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProble
     c.n_s = t;
     c.n_x = f;
     c.layer = 1;
+    if (pb.pair_side == 2) {        // the decision for layer 1 arrives from the order-0 side
+        *ctl = c;
+        return;
+    }
     if (!c.done) control_decide(c, logs, pb);
+    if (pb.pair_side == 1) handoff_publish(c, handoff);
     *ctl = c;
 }
 
@@ -396,6 +473,17 @@ __global__ void dmpt_s2_scale_init_kernel(DmptCtl* ctl, DmptProblem pb, const un
     ctl->s2_max = m;
     ctl->e2_in = 0;
     ctl->e2_out = pb.s1_autoscale ? scale_exponent(m) : 0;
+}
+
+// Order 3: the scale of the first split of a non-zero S3 (S3_2, written by layer 2) from the row norms of S1_1 and
+// S2_1: max|S1_1 S2_1 + S2_1 S1_1| <= 2 sqrt(max_i sum_k (S1_1)_ik^2) sqrt(max_j sum_k (S2_1)_jk^2).
+__global__ void dmpt_s3_scale_init_kernel(DmptCtl* ctl, DmptProblem pb, const unsigned long long* __restrict__ est1,
+                                          const unsigned long long* __restrict__ est2) {
+    if (threadIdx.x | blockIdx.x) return;
+    const double r1 = __longlong_as_double((long long)*est1), r2 = __longlong_as_double((long long)*est2);
+    const double m = 2.0 * sqrt(r1) * sqrt(r2);
+    ctl->s3_max = m;
+    ctl->e3_out = pb.s1_autoscale ? scale_exponent(m) : 0;
 }
 
 // ---------------------------------------------------------------------------------------------

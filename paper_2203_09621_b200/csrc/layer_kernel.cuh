@@ -39,7 +39,7 @@
 // (2 x [P0 | P1] x 128 columns): the drain of chunk c overlaps the MMAs of chunk c + 1.
 //
 // Orders: PASS 0 of the kernel does orders 0 and 1 (order 0 alone when the context was created
-// with order = 0: ground-state mode); PASS 1 is the order-2 pass of a layer (a9).
+// with order = 0: ground-state mode); PASS 1 is the order-2 pass of a layer (a9); PASS 4 the order-3 pass.
 #pragma once
 #include <cuda_fp16.h>
 
@@ -67,6 +67,10 @@ template <> struct PassCfg<2> { static constexpr int kOps = 6, kStages = 3; };
 // (positions 0, 1), the B side B hi/lo of column block 2 JP (positions 2, 3) and of 2 JP + 1 (positions 4, 5);
 // one accumulator per column block, six MMAs per 32 KiB staged.
 template <> struct PassCfg<3> { static constexpr int kOps = 6, kStages = 3; };
+// PASS 4: the order-3 pass of a layer (Eq. 26 at k = 3 with the symmetry saving of
+// PAPER.md:325-329): X3 - S3 = (M.S3 + S3.M) + (S1.S2 + S2.S1).  Four operand pairs (M, S1, S2, S3) per side:
+// 96 KiB per k-block and CTA, two stages; twelve MMAs per k-step into two accumulators.
+template <> struct PassCfg<4> { static constexpr int kOps = 8, kStages = 2; };
 constexpr int kChunkK = 128;               // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
@@ -121,6 +125,10 @@ struct LayerParams {
     DmptProblem pb;
     double* partials;           // [gridDim.x][kNumEpiWarps][RED_COUNT], written by PASS 0
     double* partials2;          // same shape, written by PASS 1 / PASS 2 (RED_FRO2, RED_MAX2, RED_FRO3, RED_MAX3)
+    double* partials3;          // same shape, written by PASS 4 (RED_FRO3, RED_MAX3)
+    // order-parallel pair (DmptProblem::pair_side): per-layer records from the order-0 side; side 1 writes them in
+    // its control step, side 2 reads its copies at the start of every launch.  NULL otherwise.
+    DmptHandoff* handoff;
 };
 
 __device__ __forceinline__ uint32_t pack2(__half a, __half b) {
@@ -356,10 +364,19 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     constexpr int kStageBytes = kOps * (kABytes + kBBytes);
     constexpr int kBOff = kOps * kABytes;          // B tiles follow the A tiles inside a stage
     // ---- the decision for this layer, taken by the previous launch (both CTAs of a pair read the same)
-    const DmptCtl c = *p.ctl;
-    if (c.done) return;
+    DmptCtl c_in = *p.ctl;
+    if (c_in.done) return;
+    if (PASS == 0 && p.pb.pair_side == 2) {
+        handoff_merge(c_in, p.handoff[c_in.layer]);
+        if (c_in.done) {            // the order-0 side stopped with an error: pass it on and stop
+            if (blockIdx.x == 0 && threadIdx.x == 0) { p.ctl->status = c_in.status; p.ctl->done = 1; }
+            return;
+        }
+    }
+    const DmptCtl c = c_in;
     // order 2 after the D1 stop: S0 and S1 are frozen, pass 0 only runs the control step
-    const bool idle = PASS == 0 && c.conv1 != 0;
+    // (order 3 after the D2 stop: the order-2 pass has nothing left to do either)
+    const bool idle = (PASS == 0 && c.conv1 != 0) || (PASS == 1 && c.conv2 != 0);
 
     extern __shared__ uint8_t smem_raw[];
     constexpr bool kTmaEpi = TmaEpilogue<PASS>::value;
@@ -392,18 +409,18 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     // accumulator 0 / 1 in use.  PASS 0: P0 until S0 froze / P1 unless order 0 (ground state only).
     // PASS 2: one accumulator per extra field, until that field's stopping test fired.
     // PASS 3: accumulator 0 only, fed by A hi/lo (positions 0, 1, A side) and B hi/lo (positions 2, 3, B side).
-    const bool with_p0 = PASS == 3 ? true : (PASS == 0 ? c.mode0 != MODE_FROZEN : (PASS == 1 || c.conv2 == 0));
-    const bool with_p1 = PASS == 3 ? true
+    const bool with_p0 = (PASS == 3 || PASS == 4) ? true : (PASS == 0 ? c.mode0 != MODE_FROZEN : (PASS == 1 || c.conv2 == 0));
+    const bool with_p1 = (PASS == 3 || PASS == 4) ? true
                                    : (PASS == 0 ? p.pb.order >= 1 : (PASS == 1 || (p.pb.nfields >= 3 && c.conv3 == 0)));
     const int nops = (with_p1 || PASS == 3) ? kOps : kOps - 2;    // the last operand pair only feeds accumulator 1
-    unsigned int* wave_ctr = PASS == 0 ? &p.ctl->wave : &p.ctl->wave2;
+    unsigned int* wave_ctr = PASS == 0 ? &p.ctl->wave : (PASS == 4 ? &p.ctl->wave3 : &p.ctl->wave2);
 
     if (warp == 0 && lane == 0) {
         for (int m = 0; m < 2; ++m) {
             prefetch_tensormap(&p.maps[c.s0_buf][m]);
             prefetch_tensormap(&p.maps[c.s1_buf][2 + m]);
-            if (PASS == 1 || PASS == 2) prefetch_tensormap(&p.maps[c.s2_buf][S2H + m]);       // only maps that were encoded
-            if (PASS == 2 && p.pb.nfields >= 3) prefetch_tensormap(&p.maps[c.s3_buf][S3H + m]);
+            if (PASS == 1 || PASS == 2 || PASS == 4) prefetch_tensormap(&p.maps[c.s2_buf][S2H + m]);       // only maps that were encoded
+            if ((PASS == 2 && p.pb.nfields >= 3) || PASS == 4) prefetch_tensormap(&p.maps[c.s3_buf][S3H + m]);
         }
         for (int s = 0; s < kStages; ++s) {
             mbar_init(full_bar(s), 1);                       // leader's: its producer's arrive + both CTAs' bytes
@@ -432,13 +449,14 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     if (warp == 0) {
         // =========================== TMA producer (both CTAs) ===========================
         {
-            // staged operand pairs: PASS 0: M, S1;  PASS 1: M, S1, S2;  PASS 2: M, slot 2, slot 3
-            const CUtensorMap* maps[6] = {
+            // staged operand pairs: PASS 0: M, S1;  PASS 1: M, S1, S2;  PASS 2: M, slot 2, slot 3;  PASS 4: M, S1, S2, S3
+            const CUtensorMap* maps[8] = {
                 &p.maps[c.s0_buf][MH], &p.maps[c.s0_buf][ML],
                 PASS == 2 ? &p.maps[c.s2_buf][S2H] : &p.maps[c.s1_buf][S1H],
                 PASS == 2 ? &p.maps[c.s2_buf][S2L] : &p.maps[c.s1_buf][S1L],
                 PASS == 2 ? &p.maps[c.s3_buf][S3H] : &p.maps[c.s2_buf][S2H],
-                PASS == 2 ? &p.maps[c.s3_buf][S3L] : &p.maps[c.s2_buf][S2L]};
+                PASS == 2 ? &p.maps[c.s3_buf][S3L] : &p.maps[c.s2_buf][S2L],
+                &p.maps[c.s3_buf][S3H], &p.maps[c.s3_buf][S3L]};
             const int num_kb = p.n_pad / kBK;
             int stage = 0;
             uint32_t phase = 0;
@@ -524,15 +542,16 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                                     umma_f16<2>(d, a[xh] + adv, b[xl] + adv, idesc, 1);
                                     umma_f16<2>(d, a[xl] + adv, b[xh] + adv, idesc, 1);
                                 };
-                                // CROSS(M, Y): M.Y + Y.M, three partial products each        (Eqs. 44-46)
-                                auto cross = [&](uint32_t d, int yh, int yl) {
-                                    umma_f16<2>(d, a[PM_H] + adv, b[yh] + adv, idesc, accum);   // Mhi.Yhi
-                                    umma_f16<2>(d, a[yh] + adv, b[PM_H] + adv, idesc, 1);       // Yhi.Mhi
-                                    umma_f16<2>(d, a[PM_H] + adv, b[yl] + adv, idesc, 1);       // Mhi.Ylo
-                                    umma_f16<2>(d, a[PM_L] + adv, b[yh] + adv, idesc, 1);       // Mlo.Yhi
-                                    umma_f16<2>(d, a[yh] + adv, b[PM_L] + adv, idesc, 1);       // Yhi.Mlo
-                                    umma_f16<2>(d, a[yl] + adv, b[PM_H] + adv, idesc, 1);       // Ylo.Mhi
+                                // CROSS(X, Y): X.Y + Y.X, three partial products each        (Eqs. 44-46)
+                                auto cross2 = [&](uint32_t d, int xh, int xl, int yh, int yl) {
+                                    umma_f16<2>(d, a[xh] + adv, b[yh] + adv, idesc, accum);     // Xhi.Yhi
+                                    umma_f16<2>(d, a[yh] + adv, b[xh] + adv, idesc, 1);         // Yhi.Xhi
+                                    umma_f16<2>(d, a[xh] + adv, b[yl] + adv, idesc, 1);         // Xhi.Ylo
+                                    umma_f16<2>(d, a[xl] + adv, b[yh] + adv, idesc, 1);         // Xlo.Yhi
+                                    umma_f16<2>(d, a[yh] + adv, b[xl] + adv, idesc, 1);         // Yhi.Xlo
+                                    umma_f16<2>(d, a[yl] + adv, b[xh] + adv, idesc, 1);         // Ylo.Xhi
                                 };
+                                auto cross = [&](uint32_t d, int yh, int yl) { cross2(d, PM_H, PM_L, yh, yl); };
                                 if (PASS == 0) {            // P0 = M.M, P1 = M.S1 + S1.M
                                     if (with_p0) square(d0, PM_H, PM_L);
                                     if (with_p1) cross(d1, PY_H, PY_L);
@@ -546,6 +565,9 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                                 } else if (PASS == 1) {     // Q = S1.S1, P2 = M.S2 + S2.M
                                     square(d0, PY_H, PY_L);
                                     cross(d1, PZ_H, PZ_L);
+                                } else if (PASS == 4) {     // Q3 = S1.S2 + S2.S1, P3 = M.S3 + S3.M
+                                    cross2(d0, PY_H, PY_L, PZ_H, PZ_L);
+                                    cross(d1, kOps > 6 ? 6 : 0, kOps > 6 ? 7 : 1);
                                 } else {                    // two more first-order fields: M.Y + Y.M, M.Z + Z.M
                                     if (with_p0) cross(d0, PY_H, PY_L);
                                     if (with_p1) cross(d1, PZ_H, PZ_L);
@@ -576,7 +598,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         const float unscale2 = exp2f(-(float)(p.pb.s0_shift + c.e2_in));          // M.S2 + S2.M sums
         const float scale2 = exp2f((float)c.e2_out);
         const float unscale3 = exp2f(-(float)(p.pb.s0_shift + c.e3_in));          // PASS 2: M.Z + Z.M sums
-        const float unscale_ab = exp2f(-(float)(c.e2_in + c.e1_in));              // PASS 3: A scaled by 2^e2, B by 2^e1
+        const float unscale_ab = exp2f(-(float)(c.e2_in + c.e1_in));              // PASS 3: A scaled by 2^e2, B by 2^e1; PASS 4: S1.S2 + S2.S1 sums
         const float scale3 = exp2f((float)c.e3_out);
         const bool upd0 = c.mode0 == MODE_ACTIVE;
         const bool conv0 = c.conv0 != 0;                // FroErr1 wanted (stop layer or frozen)
@@ -594,6 +616,10 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             o0.dst = nullptr; o0.old = nullptr; o0.hi = nullptr; o0.lo = nullptr;
             o1.dst = p.s2[c.s2_buf ^ 1]; o1.old = p.s2[c.s2_buf];
             o1.hi = p.h[c.s2_buf ^ 1][S2H]; o1.lo = p.h[c.s2_buf ^ 1][S2L];
+        } else if (PASS == 4) {
+            o0.dst = nullptr; o0.old = nullptr; o0.hi = nullptr; o0.lo = nullptr;
+            o1.dst = p.s3[c.s3_buf ^ 1]; o1.old = p.s3[c.s3_buf];
+            o1.hi = p.h[c.s3_buf ^ 1][S3H]; o1.lo = p.h[c.s3_buf ^ 1][S3L];
         } else {
             o0.dst = p.s2[c.s2_buf ^ 1]; o0.old = p.s2[c.s2_buf];
             o0.hi = p.h[c.s2_buf ^ 1][S2H]; o0.lo = p.h[c.s2_buf ^ 1][S2L];
@@ -713,6 +739,12 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 if (with_p1)
                     final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, unscale3, scale3, conv0, r_dummy,
                                       r_dummy, r_f1, r_mx1);
+            } else if (PASS == 4) {
+                // V3 = 2^-(a+e3) P3 + 2^-(e1+e2) Q3: both factors are powers of two, one fp32 rounding per element
+#pragma unroll
+                for (int j = 0; j < kHalfCols; ++j) a1[j] = fmaf(unscale_ab, a0[j], unscale3 * a1[j]);
+                final_epilogue<1>(a1, o1, ld, gr, gc_base, diag, true, sig, 1.f, scale3, true, r_dummy, r_dummy,
+                                  r_f1, r_mx1);
             } else {
                 // V2 = 2^-(a+e2) P2 + 2^-(2 e1) Q: both factors are powers of two, one fp32 rounding per element
 #pragma unroll
@@ -730,7 +762,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         const double mx1 = warp_max((double)r_mx1);
         const double mx0 = warp_max((double)r_mx0);
         if (lane == 0) {
-            double* out = (PASS == 0 ? p.partials : p.partials2) +
+            double* out = (PASS == 0 ? p.partials : (PASS == 4 ? p.partials3 : p.partials2)) +
                           ((size_t)blockIdx.x * kNumEpiWarps + (warp - kEpiWarp0)) * RED_COUNT;
             out[RED_TR_S0] = r_tr;
             out[RED_FRO_S0] = r_fs0;
@@ -739,8 +771,8 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             out[RED_MAX1] = PASS == 0 ? mx1 : 0.0;
             out[RED_FRO2] = PASS == 1 ? r_f1 : (PASS == 2 ? r_f0 : 0.0);      // slot 2: S2, or field 2
             out[RED_MAX2] = PASS == 1 ? mx1 : (PASS == 2 ? mx0 : 0.0);
-            out[RED_FRO3] = PASS == 2 ? r_f1 : 0.0;                            // slot 3: field 3
-            out[RED_MAX3] = PASS == 2 ? mx1 : 0.0;
+            out[RED_FRO3] = (PASS == 2 || PASS == 4) ? r_f1 : 0.0;             // slot 3: field 3, or S3
+            out[RED_MAX3] = (PASS == 2 || PASS == 4) ? mx1 : 0.0;
         }
     }
 
@@ -771,12 +803,16 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         for (int s = lane; s < nslots; s += 32) {
             const volatile double* in = p.partials + (size_t)s * RED_COUNT;
             const volatile double* in2 = p.partials2 + (size_t)s * RED_COUNT;
+            const volatile double* in3 = p.partials3 + (size_t)s * RED_COUNT;
 #pragma unroll
             for (int k = 0; k < RED_COUNT; ++k) {
-                const bool second = p.pb.order == 2 || p.pb.nfields >= 2;       // slots 2, 3 come from the other pass
+                const bool second = p.pb.order >= 2 || p.pb.nfields >= 2;       // slots 2, 3 come from the other passes
+                const bool third = p.pb.order == 3;                             // slot 3 from the order-3 pass
                 if (k == RED_MAX1) red[k] = fmax(red[k], in[k]);
-                else if (k == RED_MAX2 || k == RED_MAX3) { if (second) red[k] = fmax(red[k], in2[k]); }
-                else if (k == RED_FRO2 || k == RED_FRO3) { if (second) red[k] += in2[k]; }
+                else if (k == RED_MAX2) { if (second) red[k] = fmax(red[k], in2[k]); }
+                else if (k == RED_MAX3) { if (second) red[k] = fmax(red[k], third ? in3[k] : in2[k]); }
+                else if (k == RED_FRO2) { if (second) red[k] += in2[k]; }
+                else if (k == RED_FRO3) { if (second) red[k] += third ? in3[k] : in2[k]; }
                 else red[k] += in[k];
             }
         }
@@ -790,7 +826,9 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             nc.ticket = 0;
             nc.wave = 0;
             nc.wave2 = 0;
-            control_finalize(nc, p.logs, p.pb, red);
+            nc.wave3 = 0;
+            if (p.pb.pair_side == 2) handoff_merge(nc, p.handoff[nc.layer]);      // what this launch ran with
+            control_finalize(nc, p.logs, p.pb, red, p.handoff);
             *p.ctl = nc;
         }
     }

@@ -76,7 +76,7 @@ def test_host_only_entry_points():
         assert p.dmpt_strerror(code) not in ("ok", "unknown error code")
     assert p.dmpt_strerror(-99) == "unknown error code"
     # workspace: 3 fp32 + 8 fp16 padded matrices + 2 fp32 staging matrices + scalars
-    assert p.dmpt_workspace_bytes(0) == 0 and p.dmpt_workspace_bytes(-5) == 0 and p.dmpt_workspace_bytes(64, 3) == 0
+    assert p.dmpt_workspace_bytes(0) == 0 and p.dmpt_workspace_bytes(-5) == 0 and p.dmpt_workspace_bytes(64, 4) == 0
     for n in (1, 100, 256, 2048, 16384):
         npad = (n + 255) // 256 * 256            # CTA-pair tiles: 256 rows
         need = 3 * npad * npad * 4 + 8 * npad * npad * 2 + 2 * n * n * 4
@@ -86,7 +86,12 @@ def test_host_only_entry_points():
         # each further field: 2 fp32 + 4 fp16 padded matrices
         per_field = 2 * npad * npad * 4 + 4 * npad * npad * 2
         assert p.dmpt_workspace_bytes_fields(n, 3) - got == 2 * per_field
-    assert p.dmpt_workspace_bytes(2048, 2) > p.dmpt_workspace_bytes(2048, 1)
+    assert p.dmpt_workspace_bytes(2048, 3) > p.dmpt_workspace_bytes(2048, 2) > p.dmpt_workspace_bytes(2048, 1)
+    # order-parallel pair: each side has the workspace of a context of its own order
+    from paper_2203_09621_b200 import binding as B
+    assert B.dmpt_pair_workspace_bytes(2048, 0) == p.dmpt_workspace_bytes(2048, 0)
+    assert B.dmpt_pair_workspace_bytes(2048, 1) == p.dmpt_workspace_bytes(2048, 1)
+    assert B.dmpt_pair_workspace_bytes(2048, 2) == 0 and B.dmpt_pair_workspace_bytes(0, 0) == 0
     assert p.dmpt_workspace_bytes_fields(64, 0) == 0 and p.dmpt_workspace_bytes_fields(64, 4) == 0
 
 
@@ -105,6 +110,12 @@ def test_invalid_arguments_are_rejected_before_any_cuda_call():
     assert L.dmpt_destroy(None) == p.binding.DMPT_EINVAL
     assert L.dmpt_run(None, None, None, None, 0, None) == p.binding.DMPT_EINVAL
     assert L.dmpt_set_hamiltonian(None, None, None, 0, 0) == p.binding.DMPT_EINVAL
+    assert L.dmpt_run_orders(None, None, 0, None) == p.binding.DMPT_EINVAL
+    assert L.dmpt_pair_create(None, 256, None, 0, None, 0, 0, None, 0) == p.binding.DMPT_EINVAL
+    assert L.dmpt_pair_create(C.byref(h), 256, None, 0, None, 0, 0, None, 0) == p.binding.DMPT_EINVAL
+    assert L.dmpt_pair_run(None, None, None, 0, None) == p.binding.DMPT_EINVAL
+    assert L.dmpt_pair_set_hamiltonian(None, None, None, 0, 0) == p.binding.DMPT_EINVAL
+    assert L.dmpt_pair_destroy(None) == p.binding.DMPT_EINVAL
 
 
 def test_product_never_imports_the_oracle():

@@ -140,3 +140,47 @@ def test_max_layers_and_non_finite_state(driver):
     script[3][RED["FRO_S0"]] = float("nan")
     dec, end = _drive(driver, 1, 1, wl.n_occ, ref.tr_s[0], ref.tr_x[0], script)
     assert dec[-1][7] == 1 and dec[-1][8] == -6                                # DMPT_ENUMERIC
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 96), (2, 128), (4, 160)])
+def test_order_parallel_pair_takes_the_same_decisions(driver, cfg, n):
+    """the control flow split over the two sides of an order-parallel pair (order-0 side: sigma_n
+    and Algorithm 2, published per layer as DmptHandoff records; order-1 side: Algorithm 3, sigma flips after the
+    freeze) reproduces the single-context decisions and the oracle's sigma sequence and stop layers."""
+    from oracle.dnn_sp2_pt import dnn_sp2_pt
+    from workloads import make_config
+
+    wl = make_config(cfg, n=n)
+    ref = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ)
+    script = _script_from_oracle(ref, 1)
+    one, end1 = _drive(driver, 1, 1, wl.n_occ, ref.tr_s[0], ref.tr_x[0], script)
+    two, end2 = _drive(driver, 11, 1, wl.n_occ, ref.tr_s[0], ref.tr_x[0], script)
+    assert end2 is not None and end1[:3] == end2[:3] and float(end1[5]) == float(end2[5])
+    assert (int(end2[0]), int(end2[1]), int(end2[2])) == (ref.layers, ref.layers_d0, ref.layers_d1)
+    assert [d[1] for d in two[:ref.layers]] == ref.sigma
+    assert [(d[0], d[1], d[3]) for d in two[:ref.layers]] == [(d[0], d[1], d[3]) for d in one[:ref.layers]]
+    assert all(d[2] == 2 for d in two[:ref.layers])             # the order-1 side never forms S0^2 (MODE_FROZEN)
+    assert two[-1][7] == 1 and two[-1][8] == 0
+    # max_layers on the pair: DMPT_ENOCONV after 7 layers, like a single context
+    two, end2 = _drive(driver, 11, 1, wl.n_occ, ref.tr_s[0], ref.tr_x[0], script, max_layers=7)
+    assert two[-1][7] == 1 and two[-1][8] == -5 and int(end2[0]) == 7
+
+
+def test_third_order_cascade(driver):
+    """Order 3: the stop of every order opens the gate of the next, two layers apart at least
+    (reading R15); the oracle's order-3 records drive the device control to the same stop layers."""
+    from oracle.dnn_sp2_pt import dnn_sp2_pt
+    from workloads import make_config
+
+    wl = make_config(1, n=96)
+    ref = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, order=3)
+    assert ref.status == "ok"
+    layers = _script_from_oracle(ref, 2)
+    for n in range(1, ref.layers + 1):
+        f3 = ref.fro_errk[3][n - 1]
+        layers[n - 1][RED["FRO3"]] = 0.0 if math.isnan(f3) else f3 ** 2
+        layers[n - 1][RED["MAX3"]] = 1.0
+    dec, end = _drive(driver, 3, 1, wl.n_occ, ref.tr_s[0], ref.tr_x[0], layers)
+    assert end is not None
+    assert [int(end[1]), int(end[2]), int(end[3]), int(end[4])] == ref.layers_dk and int(end[0]) == ref.layers
+    assert [d[1] for d in dec[:ref.layers]] == ref.sigma
