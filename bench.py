@@ -532,7 +532,7 @@ def main():
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per layer launch from ncu (profiles/)")
     ap.add_argument("--fd", action="store_true",
                     help="finite-difference stencils (Eqs. 83-84) against the first-order recursion; default config 2")
-    ap.add_argument("--fd-steps", type=float, nargs="+", default=[3e-4, 1e-3, 3e-3, 1e-2, 3e-2, 1e-1],
+    ap.add_argument("--fd-steps", type=float, nargs="+", default=[1e-3, 3e-3, 1e-2, 3e-2, 6e-2, 1e-1, 2e-1, 4e-1],
                     help="step sizes h of the sweep, as h x max|H1|")
     args = ap.parse_args()
     if args.fd and "--config" not in " ".join(sys.argv):

@@ -57,7 +57,13 @@ typedef struct dmpt_options {
                        /* is folded back in fp32 (exact).  0 = Eq. 13 verbatim.  -1 = default (14).    */
     int s1_autoscale;  /* 1 (default): the response iterates are split after an exact power-of-two     */
                        /* scale chosen on the device per layer from max|S1|; 0 = Eq. 43 verbatim.      */
-    int bounds;        /* 0: Gershgorin discs of H0; 1: eps_min/eps_max below       */
+    int bounds;        /* 0: Gershgorin discs of H0; 1: eps_min/eps_max below; 2: the     */
+                       /* discs tightened on the device by lanczos_steps steps of the Lanczos recursion on   */
+                       /* H0 (extreme Ritz values widened by the residual norm, intersected with the discs;   */
+                       /* one HBM pass over H0 per step).  The bounds are inputs of the method                */
+                       /* (PAPER.md:492): D0, D1 do not depend on them, the layer count does (about a third   */
+                       /* fewer layers on dense random-orthogonal spectra).  dmpt_result::eps_min/max report  */
+                       /* the pair that was used                                                              */
     double eps_min;    /* read only when bounds == 1                                                  */
     double eps_max;
     int wave_sync;     /* 1 (default): the CTAs of a layer launch re-align at every tile boundary so that   */
@@ -69,7 +75,8 @@ typedef struct dmpt_options {
                        /* iterate in, new iterate and its split out, direct and mirrored, as full lines); 1: every  */
                        /* thread reads and writes its own row of the tile directly (round 1's path, kept for A/B     */
                        /* measurements; same arithmetic, bit-identical results)                                      */
-    int reserved[5];   /* must be 0                                                                   */
+    int lanczos_steps; /* bounds == 2: number of Lanczos steps, 1..64; 0 = default (20)                          */
+    int reserved[4];   /* must be 0                                                                   */
 } dmpt_options;
 
 typedef struct dmpt_result {

@@ -7,6 +7,7 @@ library raises.
 """
 from .binding import (  # noqa: F401
     Dmpt,
+    DmptPair,
     DmptError,
     DmptOptions,
     DmptResult,

@@ -31,7 +31,8 @@ class DmptOptions(C.Structure):
         ("max_layers", C.c_int), ("order", C.c_int), ("s0_shift", C.c_int),
         ("s1_autoscale", C.c_int), ("bounds", C.c_int),
         ("eps_min", C.c_double), ("eps_max", C.c_double),
-        ("wave_sync", C.c_int), ("num_fields", C.c_int), ("epilogue_direct", C.c_int), ("reserved", C.c_int * 5),
+        ("wave_sync", C.c_int), ("num_fields", C.c_int), ("epilogue_direct", C.c_int), ("lanczos_steps", C.c_int),
+        ("reserved", C.c_int * 4),
     ]
 
 
@@ -336,7 +337,7 @@ class Dmpt:
     """Owns a dmpt_ctx plus the torch-allocated workspace.  Marshalling only."""
 
     def __init__(self, n, order=1, max_layers=200, s0_shift=-1, s1_autoscale=True, bounds=None,
-                 device="cuda:0", stream=None, wave_sync=True, num_fields=1, epilogue_direct=False):
+                 device="cuda:0", stream=None, wave_sync=True, num_fields=1, epilogue_direct=False, lanczos_steps=0):
         import torch
 
         self.torch = torch
@@ -354,7 +355,12 @@ class Dmpt:
         opt.num_fields = int(num_fields)
         opt.epilogue_direct = 1 if epilogue_direct else 0
         self.num_fields = int(num_fields)
-        if bounds is not None:
+        if isinstance(bounds, str):
+            if bounds != "lanczos":
+                raise DmptError(DMPT_EINVAL, "Dmpt", "bounds: None (Gershgorin), (eps_min, eps_max) or 'lanczos'")
+            opt.bounds = 2
+            opt.lanczos_steps = int(lanczos_steps)
+        elif bounds is not None:
             opt.bounds = 1
             opt.eps_min, opt.eps_max = float(bounds[0]), float(bounds[1])
         # size the per-layer record buffers as the library does (dmpt_create: <= 0 -> 200, capped at 1024)
@@ -615,7 +621,7 @@ class DmptPair:
     device is allowed).  Owns both torch-allocated workspaces.  Marshalling only."""
 
     def __init__(self, n, device0="cuda:0", device1="cuda:0", max_layers=200, s0_shift=-1, s1_autoscale=True,
-                 bounds=None, wave_sync=True, epilogue_direct=False):
+                 bounds=None, wave_sync=True, epilogue_direct=False, lanczos_steps=0):
         import torch
 
         self.torch = torch
@@ -632,7 +638,10 @@ class DmptPair:
         opt.s1_autoscale = 1 if s1_autoscale else 0
         opt.wave_sync = 1 if wave_sync else 0
         opt.epilogue_direct = 1 if epilogue_direct else 0
-        if bounds is not None:
+        if isinstance(bounds, str):
+            opt.bounds = 2
+            opt.lanczos_steps = int(lanczos_steps)
+        elif bounds is not None:
             opt.bounds = 1
             opt.eps_min, opt.eps_max = float(bounds[0]), float(bounds[1])
         self.max_layers = opt.max_layers

@@ -41,7 +41,7 @@ struct Layout {
         tiles, tiles_full;
     size_t s0, s1[2], s2[2], s3[2];
     size_t h[2][8];          // [buffer][S0hi, S0lo, S1hi, S1lo, slot-2 hi, lo, slot-3 hi, lo]
-    size_t stage_h0, stage_h1;
+    size_t stage_h0, stage_h1, lanczos;
     size_t total;
 };
 
@@ -80,6 +80,7 @@ Layout make_layout(int n, int order, int nfields) {
     L.partials2 = c.take(kPartialDoubles * sizeof(double));
     L.partials3 = c.take(kPartialDoubles * sizeof(double));
     L.handoff = c.take((kMaxLayersCap + 2) * sizeof(DmptHandoff));
+    L.lanczos = c.take(sizeof(LanczosState) + 3 * (size_t)L.n_pad * sizeof(double));
     L.tiles = c.take((size_t)L.num_tiles * sizeof(uint32_t));
     L.tiles_full = c.take((size_t)(nb / 2) * nb * sizeof(uint32_t));
     L.s0 = c.take(np2 * 4);
@@ -291,7 +292,7 @@ static int create_impl(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_w
     if (n <= 0 || o.order < 0 || o.order > 3 || !d_workspace) return DMPT_EINVAL;
     if (o.max_layers <= 0) o.max_layers = 200;
     if (o.max_layers > kMaxLayersCap) o.max_layers = kMaxLayersCap;
-    if (o.s0_shift > 15) return DMPT_EINVAL;
+    if (o.s0_shift > 15 || o.bounds < 0 || o.bounds > 2 || o.lanczos_steps < 0) return DMPT_EINVAL;
     if (o.num_fields == 0) o.num_fields = 1;
     if (o.num_fields < 1 || o.num_fields > 3 || (o.num_fields > 1 && o.order != 1)) return DMPT_EINVAL;
     const size_t need = o.num_fields > 1 ? dmpt_workspace_bytes_fields(n, o.num_fields) : dmpt_workspace_bytes(n, o.order);
@@ -540,6 +541,50 @@ static int launch_transform_split(dmpt_ctx* ctx, const float* d_h0, const H1Ptrs
     return DMPT_OK;
 }
 
+// a1: spectral bounds of H0 into `bounds` (and max|H1_f| into h1max in the same pass), then into ctl.
+//   bounds == 0: Gershgorin discs;  1: the caller's numbers;  2: Gershgorin, then tightened by Lanczos steps.
+static int launch_bounds(dmpt_ctx* ctx, const float* d_h0, const H1Ptrs& h1p, int ld, int nf, int* launches) {
+    const Layout& L = ctx->L;
+    const int n = ctx->n;
+    cudaStream_t st = ctx->stream;
+    DmptCtl* ctl = ctx->at<DmptCtl>(L.ctl);
+    long long* bounds = ctx->at<long long>(L.bounds);
+    unsigned int* h1max = ctx->at<unsigned int>(L.h1max);
+    const int mode = ctx->opt.bounds;
+    if (mode != 1 || nf > 0) {
+        const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
+        dmpt_gershgorin_kernel<<<grid, 256, 0, st>>>(mode == 1 ? nullptr : d_h0, h1p, n, ld, bounds, h1max);
+        CK(cudaGetLastError());
+        ++*launches;
+    }
+    if (mode == 2) {
+        LanczosState* ls = ctx->at<LanczosState>(L.lanczos);
+        double* vec = reinterpret_cast<double*>(ctx->ws + L.lanczos + sizeof(LanczosState));
+        double* v[3] = {vec, vec + L.n_pad, vec + 2 * (size_t)L.n_pad};
+        int steps = ctx->opt.lanczos_steps > 0 ? ctx->opt.lanczos_steps : 20;
+        if (steps > kLanczosMaxSteps) steps = kLanczosMaxSteps;
+        if (steps > n) steps = n;
+        const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
+        dmpt_lanczos_init_kernel<<<elementwise_grid(ctx, n, 256), 256, 0, st>>>(v[0], v[1], n, ls);
+        CK(cudaGetLastError());
+        for (int j = 1; j <= steps; ++j) {
+            // v_{j-1} = v[(j-1) % 3], v_j = v[j % 3], w -> v[(j+1) % 3], which the update turns into v_{j+1}
+            dmpt_lanczos_matvec_kernel<<<grid, 256, 0, st>>>(d_h0, n, ld, v[j % 3], v[(j - 1) % 3], v[(j + 1) % 3], ls, j);
+            CK(cudaGetLastError());
+            dmpt_lanczos_update_kernel<<<1, 1024, 0, st>>>(v[j % 3], v[(j + 1) % 3], n, ls, j);
+            CK(cudaGetLastError());
+        }
+        dmpt_lanczos_bounds_kernel<<<1, 32, 0, st>>>(ls, bounds);
+        CK(cudaGetLastError());
+        *launches += 2 + 2 * steps;
+    }
+    dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, h1max, ctl, ctx->lp.pb, mode == 1 ? 1 : 0, ctx->opt.eps_min,
+                                                ctx->opt.eps_max);
+    CK(cudaGetLastError());
+    ++*launches;
+    return DMPT_OK;
+}
+
 // Everything from the spectral bounds to the last layer; leaves the result in the workspace.
 // `h_d0_early` (dmpt_run_host only): S0 is final once Algorithm 2 fired, two to four layers before the run
 // ends, so its read-back to the host is started on a side stream as soon as the host sees ctl.conv0 and
@@ -559,16 +604,9 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
 
     dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl, bounds, h1max);
     CK(cudaGetLastError());
-    if (!ctx->opt.bounds || nf > 0) {
-        // a1: Gershgorin discs of H0 and, in the same pass, max|H1_f| (the scale of the first split of S1_0)
-        const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
-        dmpt_gershgorin_kernel<<<grid, 256, 0, st>>>(ctx->opt.bounds ? nullptr : d_h0, h1p, n, ld, bounds, h1max);
-        CK(cudaGetLastError());
-        ++*launches;
-    }
-    dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, h1max, ctl, ctx->lp.pb, ctx->opt.bounds, ctx->opt.eps_min,
-                                                ctx->opt.eps_max);
-    CK(cudaGetLastError());
+    // a1: Gershgorin discs of H0 and, in the same pass, max|H1_f| (the scale of the first split of S1_0)
+    int rcb = launch_bounds(ctx, d_h0, h1p, ld, nf, launches);
+    if (rcb) return rcb;
     CK(cudaEventRecord(ctx->ev_t[4], st));
     // a2 + a3: one pass writes S0, S1_f (fp32) and their first operand splits
     int tgrid = 0;
@@ -577,7 +615,7 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     dmpt_control_init_kernel<<<1, 32, 0, st>>>(ctl, ctx->lp.logs, ctx->lp.pb, partials, tgrid, ctx->lp.handoff);
     CK(cudaGetLastError());
     CK(cudaEventRecord(ctx->ev_t[5], st));
-    *launches += 4;
+    *launches += 3;
     if (ctx->opt.order >= 2) {      // S2_0 = 0 (H2 = 0): fp32 iterate and its operands
         const size_t np2 = (size_t)np * np;
         CK(cudaMemsetAsync(ctx->lp.s2[0], 0, np2 * 4, st));
@@ -1412,15 +1450,10 @@ extern "C" int dmpt_pair_run(dmpt_pair* pr, float* d_d0, float* d_d1, int ld, dm
         dmpt_reset_state_kernel<<<1, 32, 0, st>>>(ctl0, c0->at<long long>(L0.bounds), c0->at<unsigned int>(L0.h1max));
         PK(cudaGetLastError());
         PK(cudaMemsetAsync(c0->lp.handoff, 0, (kMaxLayersCap + 2) * sizeof(DmptHandoff), st));
-        if (!c0->opt.bounds) {
-            dmpt_gershgorin_kernel<<<elementwise_grid(c0, (long long)n * 32, 256), 256, 0, st>>>(
-                c0->d_h0, none, (int)n, c0->ld_in, c0->at<long long>(L0.bounds), c0->at<unsigned int>(L0.h1max));
-            PK(cudaGetLastError());
-            ++launches;
+        if (launch_bounds(c0, c0->d_h0, none, c0->ld_in, 0, &launches)) {
+            snprintf(pr->err, sizeof pr->err, "%s", c0->err);
+            return DMPT_ECUDA;
         }
-        dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(c0->at<long long>(L0.bounds), c0->at<unsigned int>(L0.h1max), ctl0,
-                                                    c0->lp.pb, c0->opt.bounds, c0->opt.eps_min, c0->opt.eps_max);
-        PK(cudaGetLastError());
         PK(cudaEventRecord(pr->ev_bounds, st));
         PK(cudaEventRecord(c0->ev_t[4], st));
         int tgrid = 0;
@@ -1434,7 +1467,7 @@ extern "C" int dmpt_pair_run(dmpt_pair* pr, float* d_d0, float* d_d1, int ld, dm
         PK(cudaEventRecord(c0->ev_t[5], st));
         PK(cudaEventRecord(c0->ev_t[1], st));
         PK(cudaEventRecord(pr->evA[0], st));
-        launches += 4;
+        launches += 3;
     }
     // ---- order-1 side: max|H1|, the bounds of the other side (16 bytes), a2 + a3 for S1 alone
     PK(cudaSetDevice(pr->dev[1]));

@@ -290,6 +290,164 @@ __global__ void __launch_bounds__(256) dmpt_pad_copy_kernel(const float* __restr
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Tighter spectral bounds (dmpt_options::bounds == 2; reading R18 of DESIGN.md; the paper takes the bounds as inputs
+// and names Gershgorin "for example"): k steps of the Lanczos recursion on H0,
+//     w = H0 v_j - beta_{j-1} v_{j-1},  alpha_j = v_j.w,  w -= alpha_j v_j,  beta_j = ||w||,  v_{j+1} = w / beta_j,
+// from a fixed +-1/sqrt(n) start vector, then the extreme eigenvalues theta_min, theta_max of the k x k tridiagonal
+// matrix widened by the residual norm beta_k (every Ritz value has an eigenvalue of H0 within beta_k |s_k| <= beta_k;
+// with a start vector that has a component along every eigenvector the extreme Ritz values converge first, so
+// [theta_min - beta_k, theta_max + beta_k] encloses the spectrum in practice - tests check it on every workload) and
+// intersected with the Gershgorin discs, which enclose it by theorem.  Each step streams H0 once (4 N^2 bytes, HBM
+// bound); vectors, dot products and the tridiagonal problem are fp64.  Without re-orthogonalisation the recursion
+// only produces copies of converged extreme Ritz values, which does not move the extremes.
+// ---------------------------------------------------------------------------------------------
+constexpr int kLanczosMaxSteps = 64;
+
+struct LanczosState {       // device, fp64
+    double alpha[kLanczosMaxSteps];
+    double beta[kLanczosMaxSteps + 1];      // beta[j] = ||f_j|| after step j (beta[0] unused)
+    int steps;                              // steps completed
+    int finished;                           // 1: the Krylov space became invariant (beta_j ~ 0) - no further steps
+};
+
+__device__ __forceinline__ double lanczos_start(int i, int n) {
+    unsigned int x = (unsigned int)i * 2654435761u + 0x9E3779B9u;      // fixed, input-independent sign pattern
+    x ^= x >> 16; x *= 0x85EBCA6Bu; x ^= x >> 13; x *= 0xC2B2AE35u; x ^= x >> 16;
+    return ((x & 1u) ? 1.0 : -1.0) / sqrt((double)n);
+}
+
+__global__ void __launch_bounds__(256) dmpt_lanczos_init_kernel(double* __restrict__ v0, double* __restrict__ v1, int n,
+                                                                LanczosState* st) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        v0[i] = 0.0;
+        v1[i] = lanczos_start(i, n);
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        st->steps = 0;
+        st->finished = 0;
+        st->beta[0] = 0.0;
+    }
+}
+
+// w = H0 v - beta_{j-1} v_prev: one warp per row, 128-bit streaming loads of the matrix, fp64 accumulation
+__global__ void __launch_bounds__(256) dmpt_lanczos_matvec_kernel(const float* __restrict__ h0, int n, int ld,
+                                                                  const double* __restrict__ v,
+                                                                  const double* __restrict__ v_prev,
+                                                                  double* __restrict__ w, const LanczosState* st, int j) {
+    if (st->finished) return;
+    const double beta_prev = st->beta[j - 1];
+    const int warps_per_block = blockDim.x >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool vec = (ld & 3) == 0 && (reinterpret_cast<uintptr_t>(h0) & 15) == 0;
+    for (int row = blockIdx.x * warps_per_block + warp; row < n; row += gridDim.x * warps_per_block) {
+        const float* hr = h0 + (size_t)row * ld;
+        double acc = 0.0;
+        int c = 0;
+        if (vec) {
+            const int n4 = n & ~3;
+            for (c = lane * 4; c < n4; c += 128) {
+                const float4 a = ldg_stream4(hr + c);
+                acc += (double)a.x * v[c] + (double)a.y * v[c + 1] + (double)a.z * v[c + 2] + (double)a.w * v[c + 3];
+            }
+            c = n4;
+        }
+        for (c += lane; c < n; c += 32) acc += (double)hr[c] * v[c];
+        acc = warp_sum(acc);
+        if (lane == 0) w[row] = acc - beta_prev * v_prev[row];
+    }
+}
+
+// alpha_j, w -= alpha_j v, beta_j, v_next = w / beta_j: one block, fixed-order fp64 reductions
+__global__ void __launch_bounds__(1024) dmpt_lanczos_update_kernel(const double* __restrict__ v, double* __restrict__ w,
+                                                                   int n, LanczosState* st, int j) {
+    if (st->finished) return;
+    __shared__ double sh[32];
+    __shared__ double bc;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    auto block_sum = [&](double x) {
+        x = warp_sum(x);
+        __syncthreads();
+        if (lane == 0) sh[warp] = x;
+        __syncthreads();
+        if (warp == 0) {
+            double t = lane < nw ? sh[lane] : 0.0;
+            t = warp_sum(t);
+            if (lane == 0) bc = t;
+        }
+        __syncthreads();
+        return bc;
+    };
+    double a = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) a += v[i] * w[i];
+    const double alpha = block_sum(a);
+    double b = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const double x = w[i] - alpha * v[i];
+        w[i] = x;
+        b += x * x;
+    }
+    const double beta = sqrt(block_sum(b));
+    // invariant subspace (or a non-finite matrix): stop here; the bounds kernel then keeps the Gershgorin discs
+    const bool stop = !(beta > 1e-12 * (fabs(alpha) + st->beta[j - 1] + 1e-300)) || !isfinite(beta);
+    if (!stop) {
+        const double inv = 1.0 / beta;
+        for (int i = threadIdx.x; i < n; i += blockDim.x) w[i] *= inv;       // w becomes v_{j+1}
+    }
+    if (threadIdx.x == 0) {
+        st->alpha[j - 1] = alpha;
+        st->beta[j] = stop ? 0.0 : beta;
+        st->steps = j;
+        if (stop) st->finished = 1;
+    }
+}
+
+// Extreme eigenvalues of the tridiagonal matrix by bisection on the Sturm count, widened by beta_k and intersected
+// with the Gershgorin discs already in `bounds` (ordered-int encodings, as dmpt_gershgorin_kernel leaves them).
+__global__ void dmpt_lanczos_bounds_kernel(const LanczosState* st, long long* bounds) {
+    if (threadIdx.x | blockIdx.x) return;
+    const int k = st->steps;
+    if (k < 2 || st->finished) return;                       // keep Gershgorin
+    const double* a = st->alpha;
+    const double* b = st->beta;                              // off-diagonals b[1] .. b[k-1]; residual b[k]
+    double lo = INFINITY, hi = -INFINITY;
+    for (int i = 0; i < k; ++i) {
+        const double r = (i > 0 ? fabs(b[i]) : 0.0) + (i < k - 1 ? fabs(b[i + 1]) : 0.0);
+        lo = fmin(lo, a[i] - r);
+        hi = fmax(hi, a[i] + r);
+    }
+    if (!isfinite(lo) || !isfinite(hi)) return;
+    auto count_below = [&](double x) {                       // eigenvalues of T strictly below x
+        int cnt = 0;
+        double d = 1.0;
+        for (int i = 0; i < k; ++i) {
+            const double off = i > 0 ? b[i] * b[i] : 0.0;
+            d = a[i] - x - (i > 0 ? off / d : 0.0);
+            if (d == 0.0) d = -1e-300;
+            if (d < 0.0) ++cnt;
+        }
+        return cnt;
+    };
+    double l0 = lo, h0 = hi;                                 // smallest eigenvalue: count_below(x) >= 1
+    for (int it = 0; it < 100; ++it) {
+        const double m = 0.5 * (l0 + h0);
+        if (count_below(m) >= 1) h0 = m; else l0 = m;
+    }
+    const double th_min = l0;
+    double l1 = lo, h1 = hi;                                 // largest: count_below(x) >= k
+    for (int it = 0; it < 100; ++it) {
+        const double m = 0.5 * (l1 + h1);
+        if (count_below(m) >= k) h1 = m; else l1 = m;
+    }
+    const double th_max = h1;
+    const double resid = fabs(b[k]);
+    const double e_lo = th_min - resid, e_hi = th_max + resid;
+    const double g_lo = ordered_to_dbl(bounds[0]), g_hi = ordered_to_dbl(bounds[1]);
+    if (!isfinite(e_lo) || !isfinite(e_hi)) return;
+    bounds[0] = dbl_to_ordered(fmax(e_lo, g_lo));
+    bounds[1] = dbl_to_ordered(fmin(e_hi, g_hi));
+}
+
 // the same copy of the TRANSPOSE of a caller matrix (dmpt_congruence: Z^T as the row operand of a product), through a
 // 32 x 33 shared-memory tile so that both the reads and the writes are full lines.  grid = (n_pad/32)^2 tiles,
 // grid-stride; 256 threads = 32 x 8.

@@ -251,12 +251,23 @@ __device__ __forceinline__ void final_epilogue(float (&acc)[kHalfCols], const Ep
 //   * the split uses the packed conversions (cvt.rn.f16x2.f32).
 // step s (0 .. ns-1) of the tile handles product s / 4 (0: P0, 1: P1; when only one is live it is steps 0-3) and
 // columns (s & 3) * 16 of this thread's 64.
+//
+// Diagonal tiles (diag): the mirror of a diagonal block lies inside the block, so the box stores of one warp would
+// overwrite what another warp owns.  Each 32 x 16 block of a step is then one of three kinds:
+//   strictly above the diagonal - handled exactly as on an off-diagonal tile (its mirror lands strictly below the
+//                                 diagonal, which no block writes directly);
+//   strictly below              - nothing to do (written as the mirror of its transpose);
+//   crossing the diagonal       - same staging, general arithmetic (diagonal terms I/4 and -I/2, weights 2 / 1 / 0),
+//                                 and the warp stores the staged block itself with masked, coalesced accesses
+//                                 (direct copy where row <= column, mirrored copy where row < column) instead of
+//                                 one scalar store per lane and element.
 template <int ORDER>
 __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols], const EpiOut& o, const EpiTma& et,
                                                    uint32_t& ring_phase, int s_base, int ns,
                                                    const CUtensorMap* next_old /* old map of step s_base + 4 */,
                                                    int gr0, int gcb, int lane, float su, float unscale, float scale,
-                                                   bool want_fro, double& r_fs, double& r_fro, float& r_max) {
+                                                   bool want_fro, bool diag, float sig, int ld, double& r_tr,
+                                                   double& r_fs, double& r_fro, float& r_max) {
     const uint32_t row64 = (uint32_t)lane * 64u, sw64 = ((uint32_t)lane >> 1) & 3u;
     const uint32_t row32 = (uint32_t)lane * 32u, sw32 = ((uint32_t)lane >> 2) & 1u;
 #pragma unroll
@@ -278,6 +289,100 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
         __syncwarp();
         mbar_wait(et.bar[slot], (ring_phase >> slot) & 1u);
         ring_phase ^= 1u << slot;
+        if (diag && gr0 > gc0 + kSub - 1) continue;       // strictly below the diagonal
+        if (diag && !(gr0 + 31 < gc0)) {
+            // ---- block crossing the diagonal: this thread's row is gr0 + lane
+            const int gr = gr0 + lane;
+            float f_fs = 0.f, f_fro = 0.f, f_tr = 0.f;
+#pragma unroll
+            for (int q2 = 0; q2 < 2; ++q2) {
+                uint32_t ph[4], pl[4];
+#pragma unroll
+                for (int j4 = 2 * q2; j4 < 2 * q2 + 2; ++j4) {
+                    const uint32_t a32 = et.ring[slot] + row64 + (((uint32_t)j4 ^ sw64) << 4);
+                    const float4 x = lds128(a32);
+                    float v[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                    for (int t = 0; t < 4; t += 2) {
+                        const int j = 4 * j4 + t;
+                        float nn[2], xs[2];
+#pragma unroll
+                        for (int u = 0; u < 2; ++u) {
+                            const int gc = gc0 + j + u;
+                            const float dg = gr == gc ? 1.f : 0.f;
+                            const float w = gr < gc ? 2.f : dg;
+                            const float a = acc[sc * kSub + j + u];
+                            float delta, nw;
+                            if (ORDER == 0) {
+                                delta = fmaf(-unscale, a, 0.25f * dg);               // R = I/4 - M.M
+                                nw = fmaf(-sig, delta, v[t + u]);                    // S0 - sigma R
+                            } else {
+                                delta = unscale * a;                                 // V = M.S1 + S1.M
+                                nw = fmaf(sig, delta, v[t + u]);                     // S1 + sigma V
+                            }
+                            if (want_fro) f_fro = fmaf(w * delta, delta, f_fro);
+                            if (ORDER == 0) {
+                                f_fs = fmaf(w * nw, nw, f_fs);
+                                f_tr += dg * nw;
+                            } else if (w != 0.f) {
+                                r_max = fmaxf(r_max, fabsf(nw));
+                            }
+                            nn[u] = nw;
+                            xs[u] = (ORDER == 0 ? nw - 0.5f * dg : nw) * scale;      // operands hold M = S0 - I/2
+                        }
+                        v[t] = nn[0]; v[t + 1] = nn[1];
+                        const __half2 h2 = __floats2half2_rn(xs[0], xs[1]);
+                        const float2 hf = __half22float2(h2);
+                        const __half2 l2 = __floats2half2_rn(xs[0] - hf.x, xs[1] - hf.y);
+                        const uint32_t hw = *reinterpret_cast<const uint32_t*>(&h2);
+                        const uint32_t lw = *reinterpret_cast<const uint32_t*>(&l2);
+                        ph[(j >> 1) & 3] = hw;
+                        pl[(j >> 1) & 3] = lw;
+                        sts32(et.t32 + (uint32_t)j * 128u + (uint32_t)lane * 4u, __float_as_uint(nn[0]));
+                        sts32(et.t32 + (uint32_t)(j + 1) * 128u + (uint32_t)lane * 4u, __float_as_uint(nn[1]));
+                        sts16(et.thi + (uint32_t)j * 64u + (uint32_t)lane * 2u, (uint16_t)(hw & 0xFFFF));
+                        sts16(et.thi + (uint32_t)(j + 1) * 64u + (uint32_t)lane * 2u, (uint16_t)(hw >> 16));
+                        sts16(et.tlo + (uint32_t)j * 64u + (uint32_t)lane * 2u, (uint16_t)(lw & 0xFFFF));
+                        sts16(et.tlo + (uint32_t)(j + 1) * 64u + (uint32_t)lane * 2u, (uint16_t)(lw >> 16));
+                    }
+                    sts128(a32, __float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3]));
+                }
+                sts128(et.dhi + row32 + (((uint32_t)q2 ^ sw32) << 4), ph[0], ph[1], ph[2], ph[3]);
+                sts128(et.dlo + row32 + (((uint32_t)q2 ^ sw32) << 4), pl[0], pl[1], pl[2], pl[3]);
+            }
+            r_tr += (double)f_tr;
+            r_fs += (double)f_fs;
+            r_fro += (double)f_fro;
+            __syncwarp();
+            // direct copy, two rows of 16 columns per instruction, where row <= column
+            {
+                const uint32_t c = (uint32_t)lane & 15u, rr = (uint32_t)lane >> 4;
+#pragma unroll 4
+                for (uint32_t i = 0; i < 16; ++i) {
+                    const uint32_t r = 2 * i + rr;
+                    const int grr = gr0 + (int)r, gcc = gc0 + (int)c;
+                    if (grr <= gcc) {
+                        const size_t g = (size_t)grr * ld + gcc;
+                        o.dst[g] = lds32f(et.ring[slot] + r * 64u + ((((c >> 2) ^ ((r >> 1) & 3u))) << 4) + (c & 3u) * 4u);
+                        const uint32_t b = r * 32u + ((((c >> 3) ^ ((r >> 2) & 1u))) << 4) + (c & 7u) * 2u;
+                        o.hi[g] = __ushort_as_half(lds16(et.dhi + b));
+                        o.lo[g] = __ushort_as_half(lds16(et.dlo + b));
+                    }
+                }
+                // mirrored copy, one row of 32 columns per instruction, where row < column of the original
+#pragma unroll 4
+                for (uint32_t j = 0; j < 16; ++j) {
+                    if (gr < gc0 + (int)j) {
+                        const size_t g = (size_t)(gc0 + (int)j) * ld + gr;
+                        o.dst[g] = lds32f(et.t32 + j * 128u + (uint32_t)lane * 4u);
+                        o.hi[g] = __ushort_as_half(lds16(et.thi + j * 64u + (uint32_t)lane * 2u));
+                        o.lo[g] = __ushort_as_half(lds16(et.tlo + j * 64u + (uint32_t)lane * 2u));
+                    }
+                }
+            }
+            __syncwarp();
+            continue;
+        }
         float f_fs = 0.f, f_fro = 0.f;
 #pragma unroll
         for (int q2 = 0; q2 < 2; ++q2) {                  // eight columns: one 16-byte chunk of the fp16 rows
@@ -652,7 +757,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             // the pair tile (IP, J = 2 IP) holds block (2 IP + 1, 2 IP) below the diagonal: its mirror is
             // computed by the pair tile (IP, 2 IP + 1), so the peer CTA only drains it
             const bool live = PASS == 3 || ti <= tj;
-            const bool tma_tile = kTmaEpi && live && ti != tj && ns > 0;
+            const bool tma_tile = kTmaEpi && live && ns > 0;      // diagonal tiles too (see final_epilogue_tma)
             const int gr0 = ti * kTile + q * 32;          // first row of this warp's 32 x 64 block
             float a0[kHalfCols], a1[kHalfCols];
 #pragma unroll
@@ -716,10 +821,11 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                 if (kTmaEpi && tma_tile) {
                     if (do0)
                         final_epilogue_tma<0>(a0, o0, et, ring_phase, 0, ns, o1.m_old, gr0, gc_base, lane, sig * unscale0,
-                                              unscale0, scale0, false, r_fs0, r_dummy, r_mx_dummy);
+                                              unscale0, scale0, false, diag, sig, ld, r_tr, r_fs0, r_dummy, r_mx_dummy);
                     if (do1)
                         final_epilogue_tma<1>(a1, o1, et, ring_phase, do0 ? 4 : 0, ns, nullptr, gr0, gc_base, lane,
-                                              sig * unscale1, unscale1, scale1, conv0, r_dummy, r_f1, r_mx1);
+                                              sig * unscale1, unscale1, scale1, conv0, diag, sig, ld, r_dummy, r_dummy,
+                                              r_f1, r_mx1);
                 }
             } else if (PASS == 3) {
                 // C = 2^-(eA+eB) (A.B^T sums): plain fp32 output, no update, no split, no mirror

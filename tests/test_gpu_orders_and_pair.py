@@ -263,7 +263,7 @@ def test_finite_difference_stencils_against_the_first_order_recursion(dev):
     assert e_pt <= 1e-4                                  # the paper's ~5e-5 relative 2-norm
     gs = Dmpt(n, order=0, device=dev)
     scale = float(np.abs(wl.h1).max())
-    steps = [2.0 ** -k for k in range(2, 13)]            # h max|H1| from 0.25 down to 2.4e-4
+    steps = [2.0 ** -k for k in range(1, 13)]            # h max|H1| from 0.5 down to 2.4e-4
     err = {2: [], 4: []}
     for points in (2, 4):
         for hs in steps:
@@ -275,8 +275,15 @@ def test_finite_difference_stencils_against_the_first_order_recursion(dev):
     print("DMPT", e_pt, "2-point", err[2], "4-point", err[4])
     for points, rate in ((2, 4.0), (4, 16.0)):
         e = err[points]
-        ratios = [e[i] / e[i + 1] for i in range(len(e) - 1) if e[i + 1] > 30 * e_pt]      # truncation-dominated part
-        assert ratios and all(0.5 * rate <= q <= 1.6 * rate for q in ratios[-2:]), (points, ratios)
+        # the truncation-dominated part: the largest steps, while the error is still well above the stencil's own
+        # noise floor (measured at n = 768: 2-point 0.038, 0.0093, 0.0023, 5.7e-4, 2.0e-4, then up again;
+        # 4-point 0.0146, 6.8e-4, 1.4e-4, 1.0e-4, then up again; DNN-SP2-PT 7.5e-6)
+        ratios = []
+        for i in range(len(e) - 1):
+            if e[i + 1] < 5 * min(e):
+                break
+            ratios.append(e[i] / e[i + 1])
+        assert ratios and all(0.6 * rate <= q <= 2.0 * rate for q in ratios), (points, ratios, e)
         assert e[-1] > 2 * min(e)                          # too small a step: noise / h
     assert min(err[2]) >= 3 * e_pt
     assert min(err[4]) >= 1.0 * e_pt and min(err[4]) <= min(err[2])
@@ -320,3 +327,103 @@ def test_congruence_both_directions(dev):
         zd, xd = z.astype(np.float64), x.astype(np.float64)
         for c, ref in ((c1, zd.T @ xd @ zd), (c2, zd @ xd @ zd.T)):
             assert np.abs(c.double().cpu().numpy() - ref).max() <= 1e-5 * np.abs(ref).max()
+
+
+# ------------------------------------------------------------------------------------------ bounds = 2 (reading R18)
+@pytest.mark.parametrize("cfg,n", [(1, 256), (2, 512), (3, 768), (4, 1024), (5, 640), (1, 37)])
+def test_lanczos_bounds_enclose_the_spectrum_and_save_layers(dev, cfg, n):
+    """dmpt_options::bounds = 2: the Gershgorin discs tightened by Lanczos steps on the device.  The pair of numbers
+    the run reports (a) encloses the spectrum of H0 (numpy eigvalsh), (b) is much tighter than the discs, and - handed
+    to the oracle unchanged (R18) - (c) the run matches O2 (fp64) within the four tolerances and O2-dh's layer count,
+    in fewer layers than the Gershgorin run."""
+    from oracle.dnn_sp2_pt import DualHalfProduct, dnn_sp2_pt, gershgorin
+    from paper_2203_09621_b200 import Dmpt
+    from workloads import make_config
+
+    wl = make_config(cfg, n=n)
+    ev = np.linalg.eigvalsh(wl.h0.astype(np.float64))
+    g_lo, g_hi = gershgorin(wl.h0)
+    s = Dmpt(wl.n, device=dev, bounds="lanczos", order=1)
+    h0, h1 = torch.from_numpy(wl.h0).to(dev), torch.from_numpy(wl.h1).to(dev)
+    s.set_hamiltonian(h0, h1, wl.n_occ)
+    r = s.run()
+    d0, d1 = r.d0.double().cpu().numpy(), r.d1.double().cpu().numpy()
+    s.close()
+    assert r.status == 0
+    assert r.eps_min <= ev[0] and r.eps_max >= ev[-1], (r.eps_min, ev[0], ev[-1], r.eps_max)
+    assert g_lo - 1e-9 <= r.eps_min and r.eps_max <= g_hi + 1e-9
+    width, true = r.eps_max - r.eps_min, ev[-1] - ev[0]
+    assert width <= 2.0 * true, (width, true, g_hi - g_lo)
+    ref = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, bounds=(r.eps_min, r.eps_max))
+    assert ref.status == "ok"
+    assert np.abs(d0 - ref.d0).max() <= TOL_D0
+    assert np.abs(d1 - ref.d1).max() <= TOL_D1 * np.abs(ref.d1).max()
+    assert abs(np.trace(d0) - wl.n_occ) <= TOL_TR
+    dh = [dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, bounds=(r.eps_min, r.eps_max),
+                     product=DualHalfProduct(shift0=14, shift1="auto"), nx_mode=m) for m in ("trace", "fro")]
+    want = [x.layers for x in dh]
+    assert min(want) - 2 <= r.layers <= max(want) + 2, (r.layers, want, ref.layers)
+    g, _, _ = _run1(wl, dev)
+    assert r.layers <= g.layers and (g_hi - g_lo < 3 * true or r.layers <= g.layers - 2), (r.layers, g.layers)
+
+
+def test_lanczos_bounds_degenerate_and_options(dev):
+    """A diagonal H0 with two distinct levels: the Krylov space is invariant after two steps - the discs are kept
+    (they are exact for a diagonal matrix).  More steps never loosen the bounds beyond the discs; the pair carries the
+    option to its order-0 side; bad option values are refused."""
+    from paper_2203_09621_b200 import Dmpt
+    from paper_2203_09621_b200 import binding as B
+    from workloads import make_config
+
+    n, n_occ = 64, 24
+    h0 = np.diag(np.array([-1.0] * n_occ + [1.0] * (n - n_occ), dtype=np.float32))
+    rng = np.random.default_rng(5)
+    b = rng.standard_normal((n, n)).astype(np.float32)
+    h1 = ((b + b.T) / 2).astype(np.float32)
+    s = Dmpt(n, device=dev, bounds="lanczos")
+    s.set_hamiltonian(torch.from_numpy(h0).to(dev), torch.from_numpy(h1).to(dev), n_occ)
+    r = s.run()
+    s.close()
+    assert r.status == 0 and (r.eps_min, r.eps_max) == (-1.0, 1.0)
+    wl = make_config(1, n=200)
+    ev = np.linalg.eigvalsh(wl.h0.astype(np.float64))
+    widths = []
+    for steps in (4, 20, 64):
+        s = Dmpt(wl.n, device=dev, bounds="lanczos", lanczos_steps=steps)
+        s.set_hamiltonian(torch.from_numpy(wl.h0).to(dev), torch.from_numpy(wl.h1).to(dev), wl.n_occ)
+        r = s.run()
+        s.close()
+        assert r.status == 0 and r.eps_min <= ev[0] and r.eps_max >= ev[-1], steps
+        widths.append(r.eps_max - r.eps_min)
+    a, a0, a1 = _run1(wl, dev, bounds="lanczos")
+    b_, b0, b1 = _run_pair(wl, dev, bounds="lanczos")
+    assert (a.eps_min, a.eps_max, a.layers) == (b_.eps_min, b_.eps_max, b_.layers)
+    assert np.array_equal(a0, b0) and np.array_equal(a1, b1)
+    opt = B.dmpt_default_options()
+    ws = torch.empty(B.dmpt_workspace_bytes(64, 1), dtype=torch.uint8, device=dev)
+    for field, val in (("bounds", 3), ("bounds", -1), ("lanczos_steps", -2)):
+        o = B.dmpt_default_options()
+        setattr(o, field, val)
+        with pytest.raises(B.DmptError):
+            B.dmpt_create(64, o, ws.data_ptr(), ws.numel())
+
+
+# ------------------------------------------------------------------------------------------ the two final epilogues
+@pytest.mark.parametrize("cfg,n", [(1, 256), (2, 640), (4, 1284), (3, 200)])
+def test_epilogue_paths_are_bit_identical(dev, cfg, n):
+    """The final epilogue through shared memory and TMA (off-diagonal blocks: box stores; blocks the diagonal crosses:
+    masked coalesced stores from the same staging) and round 1's row-per-thread epilogue (epilogue_direct = 1) do the
+    same arithmetic: D0, D1 and the layer counts are equal bit for bit, the iterates stay exactly symmetric, and the
+    per-layer scalars (summed in a different order) agree to rounding."""
+    from workloads import make_config
+
+    wl = make_config(cfg, n=n)
+    a, a0, a1 = _run1(wl, dev)
+    b, b0, b1 = _run1(wl, dev, epilogue_direct=True)
+    assert a.status == 0 and b.status == 0
+    assert (a.layers, a.layers_d0, a.layers_d1, a.sigma) == (b.layers, b.layers_d0, b.layers_d1, b.sigma)
+    assert np.array_equal(a0, b0) and np.array_equal(a1, b1)
+    assert np.array_equal(a0, a0.T) and np.array_equal(a1, a1.T)
+    assert np.allclose(a.tr_s, b.tr_s, rtol=1e-12, atol=1e-9)
+    assert np.allclose(a.id_err[:a.layers_d0], b.id_err[:a.layers_d0], rtol=1e-6, atol=1e-7 * n)
+    assert abs(a.fro_err0 - b.fro_err0) <= 1e-5 * a.fro_err0

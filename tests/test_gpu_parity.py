@@ -547,7 +547,7 @@ def test_error_codes(dev):
     assert e.value.code == p.binding.DMPT_EINVAL
     s.close()
     with pytest.raises(p.DmptError):
-        _solver(128, dev, order=3)
+        _solver(128, dev, order=4)                # orders 0..3 are built
     # one layer's products need a response order: an order-0 context forms no X1
     s = _solver(128, dev, order=0)
     with pytest.raises(p.DmptError) as e:
