@@ -261,7 +261,7 @@ def run_ours(args):
         solver = Dmpt(n, order=1, device=dev, num_fields=nf)
         solver.set_hamiltonian_fields(h0, h1s, wl.n_occ)
     else:
-        solver = Dmpt(n, order=order, device=dev)
+        solver = Dmpt(n, order=order, device=dev, bounds="lanczos" if args.bounds == "lanczos" else None)
         solver.set_hamiltonian(h0, h1, wl.n_occ)
     d0 = torch.empty((n, n), dtype=torch.float32, device=dev)
     d1 = torch.empty((n, n), dtype=torch.float32, device=dev)
@@ -323,22 +323,41 @@ def run_ours(args):
     total_flops = sum_over_ranks(flops)
     value = total_flops / (ms * 1e-3) / 1e12
 
-    # ---- end-to-end arm: host buffers through dmpt_run_host, copies inside the timed region
-    # (the multi-field entry points take device matrices only: no end-to-end number with --fields > 1)
-    ms_e2e = e2e_value = None
-    if nf == 1:
-        for _ in range(1):
-            solver.run_host(h0_host, h1_host, wl.n_occ, out=outs_host)
-        barrier()
-        ev0.record()
-        e2e_flops = 0.0
-        for _ in range(args.steps):
+    # ---- end-to-end arm: host buffers through dmpt_run_host / dmpt_run_fields_host, copies inside the timed region
+    if nf > 1:
+        h1s_host = [h1_host] + [m.cpu().pin_memory() for m in h1s[1:]]
+        d1s_host = [d1_host] + [torch.empty((n, n), dtype=torch.float32).pin_memory() for _ in range(nf - 1)]
+
+    def one_run_host():
+        if nf == 1:
             r2 = solver.run_host(h0_host, h1_host, wl.n_occ, out=outs_host)
-            e2e_flops += flops_paper(n, r2.layers, r2.layers_d0, order, r2.layers_d1)
-        ev1.record()
-        barrier()
-        ms_e2e = max_over_ranks(ev0.elapsed_time(ev1))
-        e2e_value = sum_over_ranks(e2e_flops) / (ms_e2e * 1e-3) / 1e12
+            return flops_paper(n, r2.layers, r2.layers_d0, order, r2.layers_d1)
+        r2 = solver.run_fields_host(h0_host, h1s_host, wl.n_occ, out=(d0_host, d1s_host))
+        return sum(flops_paper(n, st, r2.layers_d0) for st in [r2.layers_d1, r2.layers_d2, r2.layers_d3][:nf])
+
+    one_run_host()
+    barrier()
+    ev0.record()
+    e2e_flops = 0.0
+    for _ in range(args.steps):
+        e2e_flops += one_run_host()
+    ev1.record()
+    barrier()
+    ms_e2e = max_over_ranks(ev0.elapsed_time(ev1))
+    e2e_value = sum_over_ranks(e2e_flops) / (ms_e2e * 1e-3) / 1e12
+
+    # ---- time-to-D1 with the optional tighter bounds (bounds = 2, R18), reported next to the headline
+    lanczos = None
+    if rank == 0 and nf == 1 and order == 1 and args.bounds == "gershgorin":
+        solver.close()
+        solver = Dmpt(n, order=order, device=dev, bounds="lanczos")
+        solver.set_hamiltonian(h0, h1, wl.n_occ)
+        solver.run(out=outs)
+        rl = [solver.run(out=outs) for _ in range(2)][-1]
+        lanczos = {"time_to_d1_ms": rl.ms_total, "layers": rl.layers, "layers_d0": rl.layers_d0, "ms_bounds": rl.ms_bounds,
+                   "eps_min": rl.eps_min, "eps_max": rl.eps_max,
+                   "note": "dmpt_options.bounds = 2: Gershgorin discs tightened by 20 Lanczos steps on the device; same "
+                           "D0, D1 in fewer layers; not the headline (the paper's example bounds are Gershgorin's)"}
 
     if rank == 0:
         traffic, traffic_src = ncu_traffic(n, order, nf, args.traffic)
@@ -370,13 +389,15 @@ def run_ours(args):
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": f"inputs larger than L2 ({n * n * 4 / 2**30:.2f} GiB per matrix); no flush needed",
                        "time_to_d1_ms": ms / args.steps, "loop_ms": ms_loop / args.steps,
+                       "bounds": args.bounds, "eps_min": res.eps_min, "eps_max": res.eps_max,
+                       "with_lanczos_bounds": lanczos,
                        "tflops_fma1_loop_only": flops / (ms_loop * 1e-3) / 1e12,
                        "frac_nominal_fp16_peak_fma1": value / NOMINAL_FP16_TFMA,
                        "paper_context": "~120 Tflops (FMA=1) on one A100, N=19008 (PAPER.md:546); another machine"},
             "clocks": clocks,
-            "e2e": ({"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
-                     "h2d_bytes_per_step": 2 * n * n * 4, "d2h_bytes_per_step": n_out * n * n * 4}
-                    if nf == 1 else None),
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / args.steps,
+                    "h2d_bytes_per_step": (1 + nf) * n * n * 4,
+                    "d2h_bytes_per_step": (n_out if nf == 1 else 1 + nf) * n * n * 4},
             "roofline": {"bound": "tensor", "kernel": "dmpt_layer_kernel", "achieved": achieved_tf, "peak": peak_tf,
                          "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": traffic,
                          "traffic_source": traffic_src,
@@ -530,6 +551,8 @@ def main():
     ap.add_argument("--fields", type=int, default=1,
                     help="perturbations sharing H0 in one run (1..3); value then counts every field as a run of its own")
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per layer launch from ncu (profiles/)")
+    ap.add_argument("--bounds", default="gershgorin", choices=["gershgorin", "lanczos"],
+                    help="spectral bounds of the timed runs (default: Gershgorin discs, the paper's example)")
     ap.add_argument("--fd", action="store_true",
                     help="finite-difference stencils (Eqs. 83-84) against the first-order recursion; default config 2")
     ap.add_argument("--fd-steps", type=float, nargs="+", default=[1e-3, 3e-3, 1e-2, 3e-2, 6e-2, 1e-1, 2e-1, 4e-1],

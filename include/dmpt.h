@@ -76,7 +76,9 @@ typedef struct dmpt_options {
                        /* thread reads and writes its own row of the tile directly (round 1's path, kept for A/B     */
                        /* measurements; same arithmetic, bit-identical results)                                      */
     int lanczos_steps; /* bounds == 2: number of Lanczos steps, 1..64; 0 = default (20)                          */
-    int reserved[4];   /* must be 0                                                                   */
+    int no_pdl;        /* 1: do not chain the layer launches by programmatic dependent launch (A/B measurements;   */
+                       /* results do not depend on it).  0 (default): launches that need no wave barrier are chained */
+    int reserved[3];   /* must be 0                                                                   */
 } dmpt_options;
 
 typedef struct dmpt_result {
@@ -152,6 +154,10 @@ int dmpt_run_orders(dmpt_ctx *ctx, float *const *d_d, int ld, dmpt_result *res);
  * fro_err1/2/3 belong to fields 1/2/3. */
 int dmpt_set_hamiltonian_fields(dmpt_ctx *ctx, const float *d_h0, const float *const *d_h1, int ld, int n_occ);
 int dmpt_run_fields(dmpt_ctx *ctx, float *d_d0, float *const *d_d1, int ld, dmpt_result *res);
+/* The multi-field run with HOST matrices (h_h1 / h_d1: host arrays of num_fields host matrix pointers; pinned memory
+ * recommended): as dmpt_run_host, copies inside the call, D0 read back early. */
+int dmpt_run_fields_host(dmpt_ctx *ctx, const float *h_h0, const float *const *h_h1, int ld_in, int n_occ,
+                         float *h_d0, float *const *h_d1, int ld_out, dmpt_result *res);
 
 /* The same call with HOST matrices (pinned memory recommended): copies H0, H1 to the device, runs,
  * and copies D0, D1 (D2) back.  ms_total then covers the copies too.  D0 is final as soon as Algorithm 2

@@ -18,6 +18,7 @@ EXPORTED_SYMBOLS = (
     "dmpt_last_cuda_error", "dmpt_spectral_bounds", "dmpt_initial_transform", "dmpt_split",
     "dmpt_layer_products2", "dmpt_product_nt", "dmpt_inverse_factor", "dmpt_workspace_bytes_fields", "dmpt_set_hamiltonian_fields", "dmpt_run_fields",
     "dmpt_run_orders", "dmpt_layer_products3", "dmpt_congruence", "dmpt_fd_response",
+    "dmpt_run_fields_host",
     "dmpt_pair_workspace_bytes", "dmpt_pair_create", "dmpt_pair_set_hamiltonian", "dmpt_pair_run", "dmpt_pair_destroy",
     "dmpt_pair_last_cuda_error",
 )
@@ -32,7 +33,7 @@ class DmptOptions(C.Structure):
         ("s1_autoscale", C.c_int), ("bounds", C.c_int),
         ("eps_min", C.c_double), ("eps_max", C.c_double),
         ("wave_sync", C.c_int), ("num_fields", C.c_int), ("epilogue_direct", C.c_int), ("lanczos_steps", C.c_int),
-        ("reserved", C.c_int * 4),
+        ("no_pdl", C.c_int), ("reserved", C.c_int * 3),
     ]
 
 
@@ -85,6 +86,9 @@ def lib():
         L.dmpt_layer_products3.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
                                            C.c_void_p, C.c_int]
         L.dmpt_layer_products3.restype = C.c_int
+        L.dmpt_run_fields_host.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_void_p,
+                                           C.POINTER(C.c_void_p), C.c_int, C.POINTER(_CResult)]
+        L.dmpt_run_fields_host.restype = C.c_int
         L.dmpt_congruence.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
         L.dmpt_congruence.restype = C.c_int
         L.dmpt_fd_response.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int,
@@ -177,6 +181,13 @@ def dmpt_run_orders(ctx, d_ptrs, ld: int, res) -> int:
 def dmpt_layer_products3(ctx, s0_ptr, s1_ptr, s2_ptr, s3_ptr, ld, x3_ptr, ld_out) -> int:
     return int(lib().dmpt_layer_products3(ctx, C.c_void_p(s0_ptr), C.c_void_p(s1_ptr), C.c_void_p(s2_ptr),
                                           C.c_void_p(s3_ptr), int(ld), C.c_void_p(x3_ptr), int(ld_out)))
+
+
+def dmpt_run_fields_host(ctx, h0_ptr, h1_ptrs, ld_in, n_occ, d0_ptr, d1_ptrs, ld_out, res) -> int:
+    a = (C.c_void_p * len(h1_ptrs))(*[C.c_void_p(p) for p in h1_ptrs])
+    b = (C.c_void_p * len(d1_ptrs))(*[C.c_void_p(p) for p in d1_ptrs])
+    return int(lib().dmpt_run_fields_host(ctx, C.c_void_p(h0_ptr), a, int(ld_in), int(n_occ), C.c_void_p(d0_ptr), b,
+                                          int(ld_out), C.byref(res) if res is not None else None))
 
 
 def dmpt_congruence(ctx, z_ptr, x_ptr, ld, transpose_z, c_ptr, ld_out) -> int:
@@ -337,7 +348,8 @@ class Dmpt:
     """Owns a dmpt_ctx plus the torch-allocated workspace.  Marshalling only."""
 
     def __init__(self, n, order=1, max_layers=200, s0_shift=-1, s1_autoscale=True, bounds=None,
-                 device="cuda:0", stream=None, wave_sync=True, num_fields=1, epilogue_direct=False, lanczos_steps=0):
+                 device="cuda:0", stream=None, wave_sync=True, num_fields=1, epilogue_direct=False, lanczos_steps=0,
+                 pdl=True):
         import torch
 
         self.torch = torch
@@ -354,6 +366,7 @@ class Dmpt:
         opt.wave_sync = 1 if wave_sync else 0
         opt.num_fields = int(num_fields)
         opt.epilogue_direct = 1 if epilogue_direct else 0
+        opt.no_pdl = 0 if pdl else 1
         self.num_fields = int(num_fields)
         if isinstance(bounds, str):
             if bounds != "lanczos":
@@ -487,6 +500,24 @@ class Dmpt:
         d1s = [t.empty((n, n), dtype=t.float32, device=self.device) for _ in range(self.num_fields)]
         r, bufs = self._new_result()
         rc = dmpt_run_fields(self.ctx, d0.data_ptr(), [m.data_ptr() for m in d1s], n, r)
+        return self._wrap(rc, r, bufs, d0, d1s, None, check)
+
+    def run_fields_host(self, h0, h1s, n_occ, out=None, check=True) -> DmptResult:
+        """h0, h1s: CPU fp32 tensors (pinned recommended) with one leading dimension; out = (d0, [d1_f]) CPU tensors."""
+        t = self.torch
+        n = self.n
+        h1s = list(h1s)
+        if len(h1s) != self.num_fields or any(m.stride(0) != h0.stride(0) for m in h1s):
+            raise DmptError(DMPT_EINVAL, "run_fields_host", f"need {self.num_fields} perturbations with h0's leading dimension")
+        if out is None:
+            d0 = t.empty((n, n), dtype=t.float32, pin_memory=True)
+            d1s = [t.empty((n, n), dtype=t.float32, pin_memory=True) for _ in range(self.num_fields)]
+        else:
+            d0, d1s = out[0], list(out[1])
+        self._check_outputs("run_fields_host", False, d0, *d1s)
+        r, bufs = self._new_result()
+        rc = dmpt_run_fields_host(self.ctx, h0.data_ptr(), [m.data_ptr() for m in h1s], h0.stride(0), n_occ,
+                                  d0.data_ptr(), [m.data_ptr() for m in d1s], d0.stride(0), r)
         return self._wrap(rc, r, bufs, d0, d1s, None, check)
 
     def run_host(self, h0, h1, n_occ, out=None, check=True) -> DmptResult:

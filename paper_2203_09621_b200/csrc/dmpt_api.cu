@@ -41,7 +41,7 @@ struct Layout {
         tiles, tiles_full;
     size_t s0, s1[2], s2[2], s3[2];
     size_t h[2][8];          // [buffer][S0hi, S0lo, S1hi, S1lo, slot-2 hi, lo, slot-3 hi, lo]
-    size_t stage_h0, stage_h1, lanczos;
+    size_t stage_h0, stage_h1, stage_hx[2], lanczos;
     size_t total;
 };
 
@@ -100,6 +100,7 @@ Layout make_layout(int n, int order, int nfields) {
         for (int m = 0; m < nh; ++m) L.h[b][m] = c.take(np2 * 2);
     L.stage_h0 = c.take((size_t)n * n * 4);
     L.stage_h1 = c.take((size_t)n * n * 4);
+    for (int f = 0; f < 2; ++f) L.stage_hx[f] = (order == 1 && nfields >= f + 2) ? c.take((size_t)n * n * 4) : 0;
     L.total = c.off;
     return L;
 }
@@ -456,11 +457,14 @@ static int launch_pass(dmpt_ctx* ctx) {
     cfg.blockDim = dim3(kNumThreads);
     cfg.dynamicSmemBytes = smem_bytes<PASS>();
     cfg.stream = ctx->stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeCooperative;
     attr[0].val.cooperative = ctx->lp.wave_sync ? 1 : 0;
+    // without the wave barrier (at most one tile per CTA pair): programmatic dependent launch, see the kernel's first lines
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = (ctx->lp.wave_sync || ctx->opt.no_pdl) ? 0 : 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = 2;
     CK(cudaLaunchKernelEx(&cfg, dmpt_layer_kernel<PASS>, ctx->lp));
     return DMPT_OK;
 }
@@ -827,6 +831,49 @@ extern "C" int dmpt_run_fields(dmpt_ctx* ctx, float* d_d0, float* const* d_d1, i
     CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
     for (int f = 0; f < nf; ++f)
         CK(cudaMemcpy2DAsync(d_d1[f], (size_t)ld * 4, src[f], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
+    return finish(ctx, res, launches);
+}
+
+extern "C" int dmpt_run_fields_host(dmpt_ctx* ctx, const float* h_h0, const float* const* h_h1, int ld_in, int n_occ,
+                                    float* h_d0, float* const* h_d1, int ld_out, dmpt_result* res) {
+    if (!ctx || !h_h0 || !h_h1 || !h_d0 || !h_d1 || ctx->opt.order != 1) return DMPT_EINVAL;
+    const int nf = ctx->opt.num_fields;
+    for (int f = 0; f < nf; ++f)
+        if (!h_h1[f] || !h_d1[f]) return DMPT_EINVAL;
+    if (ld_in < ctx->n || ld_out < ctx->n || n_occ <= 0 || n_occ >= ctx->n) return DMPT_EINVAL;
+    const Layout& L = ctx->L;
+    const size_t n = ctx->n, np = L.n_pad;
+    cudaStream_t st = ctx->stream;
+    float* s_h0 = ctx->at<float>(L.stage_h0);
+    float* s_h1[3] = {ctx->at<float>(L.stage_h1), nf > 1 ? ctx->at<float>(L.stage_hx[0]) : nullptr,
+                      nf > 2 ? ctx->at<float>(L.stage_hx[1]) : nullptr};
+    ctx->n_occ = n_occ;
+    ctx->lp.pb.n_occ = n_occ;
+    int launches = 0;
+    CK(cudaEventRecord(ctx->ev_t[0], st));
+    CK(cudaMemcpy2DAsync(s_h0, n * 4, h_h0, (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, st));
+    for (int f = 0; f < nf; ++f)
+        CK(cudaMemcpy2DAsync(s_h1[f], n * 4, h_h1[f], (size_t)ld_in * 4, n * 4, n, cudaMemcpyHostToDevice, st));
+    // run_core reads fields 2, 3 through the context: point it at the staged copies for this call
+    const float* keep[2] = {ctx->d_h1x[0], ctx->d_h1x[1]};
+    ctx->d_h1x[0] = s_h1[1];
+    ctx->d_h1x[1] = s_h1[2];
+    bool early = false;
+    int rc = run_core(ctx, s_h0, s_h1[0], (int)n, &launches, h_d0, ld_out, &early);
+    ctx->d_h1x[0] = keep[0];
+    ctx->d_h1x[1] = keep[1];
+    if (rc) return rc;
+    if ((rc = fetch_ctl(ctx))) return rc;
+    if ((rc = unscale_outputs(ctx, &launches))) return rc;
+    const DmptCtl& c = *ctx->h_ctl;
+    const float* src[3] = {ctx->lp.s1[c.s1_buf & 1], nf > 1 ? ctx->lp.s2[c.s2_buf & 1] : nullptr,
+                           nf > 2 ? ctx->lp.s3[c.s3_buf & 1] : nullptr};
+    if (early)
+        CK(cudaStreamWaitEvent(st, ctx->ev_side, 0));
+    else
+        CK(cudaMemcpy2DAsync(h_d0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToHost, st));
+    for (int f = 0; f < nf; ++f)
+        CK(cudaMemcpy2DAsync(h_d1[f], (size_t)ld_out * 4, src[f], np * 4, n * 4, n, cudaMemcpyDeviceToHost, st));
     return finish(ctx, res, launches);
 }
 

@@ -468,6 +468,11 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     constexpr int kStages = PassCfg<PASS>::kStages;
     constexpr int kStageBytes = kOps * (kABytes + kBBytes);
     constexpr int kBOff = kOps * kABytes;          // B tiles follow the A tiles inside a stage
+    // Layer launches that do not need the wave barrier are chained by programmatic dependent launch: the next launch
+    // is released at once (its CTAs become resident as SMs free up - at N = 256 straight away - and park in
+    // griddepcontrol.wait), so the stream's launch latency is off the critical path of a layer.
+    griddep_launch_dependents();
+    griddep_wait();
     // ---- the decision for this layer, taken by the previous launch (both CTAs of a pair read the same)
     DmptCtl c_in = *p.ctl;
     if (c_in.done) return;

@@ -70,7 +70,7 @@ def test_host_only_entry_points():
     o = p.dmpt_default_options()
     assert (o.max_layers, o.order, o.s0_shift, o.s1_autoscale, o.bounds, o.wave_sync, o.num_fields) == \
         (200, 1, -1, 1, 0, 1, 1)
-    assert list(o.reserved) == [0] * 4 and o.epilogue_direct == 0 and o.lanczos_steps == 0
+    assert list(o.reserved) == [0] * 3 and o.epilogue_direct == 0 and o.lanczos_steps == 0 and o.no_pdl == 0
     assert p.dmpt_strerror(0) == "ok"
     for code in range(-7, 0):
         assert p.dmpt_strerror(code) not in ("ok", "unknown error code")
@@ -83,8 +83,8 @@ def test_host_only_entry_points():
         got = p.dmpt_workspace_bytes(n, 1)
         assert need <= got <= need + (4 << 20), (n, need, got)
         assert p.dmpt_workspace_bytes(n, 0) == got and p.dmpt_workspace_bytes_fields(n, 1) == got
-        # each further field: 2 fp32 + 4 fp16 padded matrices
-        per_field = 2 * npad * npad * 4 + 4 * npad * npad * 2
+        # each further field: 2 fp32 + 4 fp16 padded matrices + one n x n staging matrix (dmpt_run_fields_host)
+        per_field = 2 * npad * npad * 4 + 4 * npad * npad * 2 + (n * n * 4 + 255) // 256 * 256
         assert p.dmpt_workspace_bytes_fields(n, 3) - got == 2 * per_field
     assert p.dmpt_workspace_bytes(2048, 3) > p.dmpt_workspace_bytes(2048, 2) > p.dmpt_workspace_bytes(2048, 1)
     # order-parallel pair: each side has the workspace of a context of its own order

@@ -873,7 +873,12 @@ def test_fields_argument_checks(dev):
     s.set_hamiltonian_fields(h0, hs, wl.n_occ)
     r = s.run(check=False)                           # the single-field call on a multi-field context
     assert r.status == p.binding.DMPT_EINVAL
-    assert s.run_fields().status == 0
+    ra = s.run_fields()
+    assert ra.status == 0
+    # the same run from host buffers (dmpt_run_fields_host): identical results
+    rb = s.run_fields_host(torch.from_numpy(wl.h0).pin_memory(), [torch.from_numpy(h).pin_memory() for h in h1s], wl.n_occ)
+    assert rb.status == 0 and rb.layers == ra.layers
+    assert torch.equal(ra.d0.cpu(), rb.d0) and all(torch.equal(x.cpu(), y) for x, y in zip(ra.d1, rb.d1))
     s.close()
 
 
