@@ -10,6 +10,7 @@ than the 126 MB L2, so no explicit L2 flush is needed (stated in `config`).
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--n 16384]
     python bench.py --impl reference      # the fp64 CPU oracle, bounded sample, same JSON line
     python bench.py --fd [--config 2]     # finite-difference stencils vs the first-order recursion (Fig. 5)
+    python bench.py --order-parallel      # the two-device variant of PAPER.md:287 (one device: both sides on it)
 
 value      paper-convention Tflops (one FMA = one flop, Eq. 82):
            (5 N^3 L_active + 3 N^3 L_frozen) / time of the whole dmpt_run, inputs resident in HBM.
@@ -421,6 +422,70 @@ def run_ours(args):
 
 
 # ---------------------------------------------------------------------------------------------
+# --order-parallel: the two-device variant of PAPER.md:287, 548-550
+# ---------------------------------------------------------------------------------------------
+def run_pair(args):
+    """The order-parallel pair (dmpt_pair_*) on the bench workload: the order-0 side on cuda:0, the order-1 side on
+    cuda:1 when the box has a second GPU, else on cuda:0 too (two streams, device-local hand-off: the two sides' launches
+    then take turns on the SMs and the line only shows that the path runs at full size).  Same metric as the default
+    line; the single-context run of the same input is timed beside it and the results are compared bit for bit."""
+    import torch
+
+    from paper_2203_09621_b200 import Dmpt, DmptPair
+    from workloads import make_config
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU path")
+    two = torch.cuda.device_count() > 1
+    dev0, dev1 = torch.device("cuda", 0), torch.device("cuda", 1 if two else 0)
+    wl = make_config(args.config, n=args.n, device="cuda:0" if args.n >= 8192 else None)
+    if wl.order != 1:
+        raise SystemExit("--order-parallel needs a first-order config")
+    n = wl.n
+    h0 = torch.from_numpy(wl.h0).to(dev0)
+    h1 = torch.from_numpy(wl.h1).to(dev1)
+    pair = DmptPair(n, device0=dev0, device1=dev1)
+    pair.set_hamiltonian(h0, h1, wl.n_occ)
+    for _ in range(max(1, args.warmup - 1)):
+        rp = pair.run()
+    sampler = ClockSampler(0)
+    sampler.start()
+    t0 = time.perf_counter()
+    ms = flops = 0.0
+    launches = 0
+    for _ in range(args.steps):
+        rp = pair.run()
+        ms += rp.ms_total
+        flops += flops_paper(n, rp.layers, rp.layers_d0)
+        launches += rp.launches
+    wall = time.perf_counter() - t0
+    clocks = sampler.stop()
+    d0p, d1p = rp.d0.clone(), rp.d1.to(dev0)
+    pair.close()
+    one = Dmpt(n, order=1, device=dev0)
+    one.set_hamiltonian(h0, h1.to(dev0), wl.n_occ)
+    one.run()
+    r1 = one.run()
+    same = bool(torch.equal(r1.d0, d0p) and torch.equal(r1.d1, d1p) and r1.layers == rp.layers)
+    one.close()
+    line = {"mode": "order-parallel", "metric": METRIC, "value": flops / (ms * 1e-3) / 1e12, "unit": UNIT,
+            "n_gpus": 2 if two else 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f16 x f16 -> f32 (dual-half), f64 scalars", "data": "synthetic", "gpu_launches": launches,
+            "config": {"workload": workload_name(args), "n": n, "layers": rp.layers, "layers_d0": rp.layers_d0,
+                       "parallelism": ("order-parallel pair: S0^2 on cuda:0, S0.S1 + S1.S0 on cuda:1, one hand-off of "
+                                       "4 N^2 bytes per layer (cudaMemcpyPeerAsync)") if two else
+                                      ("order-parallel pair with BOTH sides on cuda:0 (this box has one GPU): the two "
+                                       "sides' launches take turns on the SMs; not a scaling number"),
+                       "single_context_ms": r1.ms_total, "bit_identical_to_single_context": same,
+                       "wall_s": wall,
+                       "paper_context": "2 x A100: ~195 vs ~120 Tflops, +63 % (PAPER.md:550)"},
+            "clocks": clocks, "e2e": None}
+    print(json.dumps(line), flush=True)
+    return 0 if same else 1
+
+
+# ---------------------------------------------------------------------------------------------
 # --fd: the finite-difference comparison of PAPER.md:562-582 (Eqs. 83-84, Fig. 5) as a workload
 # ---------------------------------------------------------------------------------------------
 def run_fd(args):
@@ -553,6 +618,8 @@ def main():
     ap.add_argument("--traffic", type=float, default=None, help="dram bytes per layer launch from ncu (profiles/)")
     ap.add_argument("--bounds", default="gershgorin", choices=["gershgorin", "lanczos"],
                     help="spectral bounds of the timed runs (default: Gershgorin discs, the paper's example)")
+    ap.add_argument("--order-parallel", action="store_true",
+                    help="the order-parallel pair (PAPER.md:287): order 0 on cuda:0, order 1 on cuda:1 if present")
     ap.add_argument("--fd", action="store_true",
                     help="finite-difference stencils (Eqs. 83-84) against the first-order recursion; default config 2")
     ap.add_argument("--fd-steps", type=float, nargs="+", default=[1e-3, 3e-3, 1e-2, 3e-2, 6e-2, 1e-1, 2e-1, 4e-1],
@@ -570,6 +637,8 @@ def main():
         raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if args.fd:
         return run_fd(args)
+    if args.order_parallel:
+        return run_pair(args)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: warmup raised to 3 (timing rules)", file=sys.stderr)
         args.warmup = 3

@@ -134,7 +134,8 @@ int dmpt_set_hamiltonian(dmpt_ctx *ctx, const float *d_h0, const float *d_h1, in
 
 /* Run Algorithms 1-3 and write D0, D1 (and D2 when order == 2, else pass NULL) to device matrices
  * with leading dimension ld >= n.  `res` may be NULL.  On DMPT_ENOCONV the outputs hold the last
- * iterate.  Safe to call repeatedly. */
+ * iterate.  Safe to call repeatedly.  Contexts of order 3 have one more output: use dmpt_run_orders
+ * (dmpt_run and dmpt_run_host return DMPT_EINVAL for them). */
 int dmpt_run(dmpt_ctx *ctx, float *d_d0, float *d_d1, float *d_d2, int ld, dmpt_result *res);
 
 /* General response order (Eq. 26, 285 Eq. 40): the same run for a context of any

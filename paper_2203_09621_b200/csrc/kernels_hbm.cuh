@@ -266,19 +266,32 @@ __global__ void __launch_bounds__(256) dmpt_unscale_kernel(float* __restrict__ x
         x[i] = ldexpf(x[i], minus_p);
 }
 
-// zero-padded copy of a caller matrix into an n_pad x n_pad workspace matrix (dmpt_layer_products)
+// zero-padded copy of a caller matrix into an n_pad x n_pad workspace matrix (single-shot products, dmpt_product_nt)
+// and max|.| per block.  Block per row (grid-stride), four columns per thread: 128-bit accesses when the source allows.
 __global__ void __launch_bounds__(256) dmpt_pad_copy_kernel(const float* __restrict__ src, int n, int ld,
                                                        int n_pad, float* __restrict__ dst,
                                                        double* __restrict__ partials /* [grid] max */) {
-    const long long total = (long long)n_pad * n_pad;
+    const bool vec = (ld & 3) == 0 && (reinterpret_cast<uintptr_t>(src) & 15) == 0;
+    const int c4_per_row = n_pad >> 2;
     float mx = 0.f;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total;
-         i += (long long)gridDim.x * blockDim.x) {
-        const int row = (int)(i / n_pad), col = (int)(i - (long long)row * n_pad);
-        const float v = (row < n && col < n) ? src[(size_t)row * ld + col] : 0.f;
-        dst[i] = v;
-        mx = fmaxf(mx, fabsf(v));
-    }
+    for (int row = blockIdx.x; row < n_pad; row += gridDim.x)
+        for (int c4 = threadIdx.x; c4 < c4_per_row; c4 += blockDim.x) {
+            const int col = c4 << 2;
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (row < n && col < n) {
+                const float* s = src + (size_t)row * ld + col;
+                if (vec && col + 3 < n) {
+                    v = ldg_stream4(s);
+                } else {
+                    v.x = s[0];
+                    if (col + 1 < n) v.y = s[1];
+                    if (col + 2 < n) v.z = s[2];
+                    if (col + 3 < n) v.w = s[3];
+                }
+            }
+            *reinterpret_cast<float4*>(dst + (size_t)row * n_pad + col) = v;
+            mx = absmax4(mx, v);
+        }
     __shared__ double sh[8];
     double dmx = warp_max((double)mx);
     if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = dmx;

@@ -50,3 +50,44 @@ def test_multi_wave_launch_matches_the_oracle_itself(dev, cfg):
         assert abs(res.id_err[i] - ref.id_err[i]) <= 1e-3, (i, res.id_err[i], ref.id_err[i])
     print(f"config {cfg} @ n=4096: layers gpu {res.layers} (D0 {res.layers_d0}) O2 fp64 {ref.layers} (D0 {ref.layers_d0}) "
           f"max|D0 err| {e0:.2e} D1 {e1:.2e} tr {tr:.2e}")
+
+
+def test_pair_full_size_is_bit_identical_to_run(dev):
+    """SURVEY.md 8(f) f1 at N = 8192 (config 3; 1056 pair tiles, 14.3 waves, cooperative launches of the two sides
+    taking turns on one device): D0, D1 and the layer counts of the order-parallel pair equal dmpt_run's exactly."""
+    from paper_2203_09621_b200 import DmptPair
+    from workloads import make_config
+
+    wl = make_config(3, device="cuda")
+    a, a0, a1 = _run(wl, dev)
+    p = DmptPair(wl.n, device0=dev, device1=dev)
+    p.set_hamiltonian(torch.from_numpy(wl.h0).to(dev), torch.from_numpy(wl.h1).to(dev), wl.n_occ)
+    b = p.run()
+    assert a.status == 0 and b.status == 0
+    assert (a.layers, a.layers_d0, a.layers_d1, a.sigma) == (b.layers, b.layers_d0, b.layers_d1, b.sigma)
+    assert np.array_equal(a0, b.d0.double().cpu().numpy()) and np.array_equal(a1, b.d1.double().cpu().numpy())
+    p.close()
+
+
+def test_third_order_multi_wave_matches_the_oracle(dev):
+    """SURVEY.md 8(f) f2 at n = 2048 (config 2's size: 72 pair tiles, three launches per layer): D0 .. D3 against
+    oracle.dnn_sp2_pt run to order 3 (fp64, ~1 min on the host)."""
+    from oracle.dnn_sp2_pt import dnn_sp2_pt
+    from paper_2203_09621_b200 import Dmpt
+    from workloads import make_config
+
+    wl = make_config(2)
+    ref = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ, order=3)
+    assert ref.status == "ok"
+    s = Dmpt(wl.n, device=dev, order=3)
+    s.set_hamiltonian(torch.from_numpy(wl.h0).to(dev), torch.from_numpy(wl.h1).to(dev), wl.n_occ)
+    r = s.run_orders()
+    d = [m.double().cpu().numpy() for m in (r.d0, r.d1, r.d2, r.d3)]
+    s.close()
+    assert r.status == 0
+    assert np.abs(d[0] - ref.dk[0]).max() <= 5e-5 and abs(np.trace(d[0]) - wl.n_occ) <= 1e-3
+    errs = [np.abs(d[k] - ref.dk[k]).max() / np.abs(ref.dk[k]).max() for k in (1, 2, 3)]
+    assert all(e <= 5e-4 for e in errs), errs
+    got = [r.layers_d0, r.layers_d1, r.layers_d2, r.layers_d3]
+    assert all(w - 8 <= g <= w + 2 for g, w in zip(got, ref.layers_dk)), (got, ref.layers_dk)
+    print(f"order 3 @ n=2048: layers gpu {got} O2 fp64 {ref.layers_dk} errors D1..D3 {errs}")
