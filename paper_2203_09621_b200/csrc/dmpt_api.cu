@@ -569,8 +569,16 @@ static int launch_bounds(dmpt_ctx* ctx, const float* d_h0, const H1Ptrs& h1p, in
         if (steps > kLanczosMaxSteps) steps = kLanczosMaxSteps;
         if (steps > n) steps = n;
         const int grid = elementwise_grid(ctx, (long long)n * 32, 256);
-        dmpt_lanczos_init_kernel<<<elementwise_grid(ctx, n, 256), 256, 0, st>>>(v[0], v[1], n, ls);
-        CK(cudaGetLastError());
+        if (n <= 1024) {        // one block does the whole recursion
+            dmpt_lanczos_small_kernel<<<1, 1024, 0, st>>>(d_h0, n, ld, steps, ls);
+            CK(cudaGetLastError());
+            steps = 0;
+            *launches += 1;
+        } else {
+            dmpt_lanczos_init_kernel<<<1, 1024, 0, st>>>(v[0], v[1], n, ls);
+            CK(cudaGetLastError());
+            *launches += 1;
+        }
         for (int j = 1; j <= steps; ++j) {
             // v_{j-1} = v[(j-1) % 3], v_j = v[j % 3], w -> v[(j+1) % 3], which the update turns into v_{j+1}
             dmpt_lanczos_matvec_kernel<<<grid, 256, 0, st>>>(d_h0, n, ld, v[j % 3], v[(j - 1) % 3], v[(j + 1) % 3], ls, j);
@@ -580,7 +588,7 @@ static int launch_bounds(dmpt_ctx* ctx, const float* d_h0, const H1Ptrs& h1p, in
         }
         dmpt_lanczos_bounds_kernel<<<1, 32, 0, st>>>(ls, bounds);
         CK(cudaGetLastError());
-        *launches += 2 + 2 * steps;
+        *launches += 1 + 2 * steps;
     }
     dmpt_bounds_to_ctl_kernel<<<1, 32, 0, st>>>(bounds, h1max, ctl, ctx->lp.pb, mode == 1 ? 1 : 0, ctx->opt.eps_min,
                                                 ctx->opt.eps_max);

@@ -307,7 +307,7 @@ __global__ void __launch_bounds__(256) dmpt_pad_copy_kernel(const float* __restr
 // Tighter spectral bounds (dmpt_options::bounds == 2; reading R18 of DESIGN.md; the paper takes the bounds as inputs
 // and names Gershgorin "for example"): k steps of the Lanczos recursion on H0,
 //     w = H0 v_j - beta_{j-1} v_{j-1},  alpha_j = v_j.w,  w -= alpha_j v_j,  beta_j = ||w||,  v_{j+1} = w / beta_j,
-// from a fixed +-1/sqrt(n) start vector, then the extreme eigenvalues theta_min, theta_max of the k x k tridiagonal
+// from a fixed pseudo-random start vector (signs and magnitudes), then the extreme eigenvalues theta_min, theta_max of the k x k tridiagonal
 // matrix widened by the residual norm beta_k (every Ritz value has an eigenvalue of H0 within beta_k |s_k| <= beta_k;
 // with a start vector that has a component along every eigenvector the extreme Ritz values converge first, so
 // [theta_min - beta_k, theta_max + beta_k] encloses the spectrum in practice - tests check it on every workload) and
@@ -324,19 +324,41 @@ struct LanczosState {       // device, fp64
     int finished;                           // 1: the Krylov space became invariant (beta_j ~ 0) - no further steps
 };
 
-__device__ __forceinline__ double lanczos_start(int i, int n) {
-    unsigned int x = (unsigned int)i * 2654435761u + 0x9E3779B9u;      // fixed, input-independent sign pattern
+__device__ __forceinline__ double lanczos_start(int i) {
+    // fixed, input-independent pattern: pseudo-random sign AND magnitude in [0.5, 1), so that no eigenvector of a
+    // structured matrix (e.g. (e_1 - e_2)/sqrt(2)) is orthogonal to the start vector by symmetry
+    unsigned int x = (unsigned int)i * 2654435761u + 0x9E3779B9u;
     x ^= x >> 16; x *= 0x85EBCA6Bu; x ^= x >> 13; x *= 0xC2B2AE35u; x ^= x >> 16;
-    return ((x & 1u) ? 1.0 : -1.0) / sqrt((double)n);
+    const double mag = 0.5 + (double)(x >> 8) * (0.5 / 16777216.0);
+    return (x & 1u) ? mag : -mag;
 }
 
-__global__ void __launch_bounds__(256) dmpt_lanczos_init_kernel(double* __restrict__ v0, double* __restrict__ v1, int n,
-                                                                LanczosState* st) {
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        v0[i] = 0.0;
-        v1[i] = lanczos_start(i, n);
+// v_0 = 0, v_1 = the normalised start vector: one block (fixed-order norm)
+__global__ void __launch_bounds__(1024) dmpt_lanczos_init_kernel(double* __restrict__ v0, double* __restrict__ v1, int n,
+                                                                 LanczosState* st) {
+    __shared__ double sh[32];
+    __shared__ double bc;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    double q = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const double x = lanczos_start(i);
+        q += x * x;
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
+    q = warp_sum(q);
+    if (lane == 0) sh[warp] = q;
+    __syncthreads();
+    if (warp == 0) {
+        double t = lane < nw ? sh[lane] : 0.0;
+        t = warp_sum(t);
+        if (lane == 0) bc = 1.0 / sqrt(t);
+    }
+    __syncthreads();
+    const double inv = bc;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        v0[i] = 0.0;
+        v1[i] = lanczos_start(i) * inv;
+    }
+    if (threadIdx.x == 0) {
         st->steps = 0;
         st->finished = 0;
         st->beta[0] = 0.0;
@@ -412,6 +434,65 @@ __global__ void __launch_bounds__(1024) dmpt_lanczos_update_kernel(const double*
         st->beta[j] = stop ? 0.0 : beta;
         st->steps = j;
         if (stop) st->finished = 1;
+    }
+}
+
+// Small matrices (n <= 1024): the whole recursion in ONE block, one row per thread - at these sizes the 2 k launches
+// of the general path cost more than the layers they save.  H0 is symmetric, so thread i reads column i (H[k][i] over
+// k): consecutive threads read consecutive addresses.  Same arithmetic order per row as a sequential dot product.
+__global__ void __launch_bounds__(1024) dmpt_lanczos_small_kernel(const float* __restrict__ h0, int n, int ld, int steps,
+                                                                  LanczosState* st) {
+    __shared__ double v[1024];
+    __shared__ double sh[32];
+    __shared__ double bc;
+    const int i = threadIdx.x;
+    const int lane = i & 31, warp = i >> 5, nw = blockDim.x >> 5;
+    auto block_sum = [&](double x) {
+        x = warp_sum(x);
+        __syncthreads();
+        if (lane == 0) sh[warp] = x;
+        __syncthreads();
+        if (warp == 0) {
+            double t = lane < nw ? sh[lane] : 0.0;
+            t = warp_sum(t);
+            if (lane == 0) bc = t;
+        }
+        __syncthreads();
+        return bc;
+    };
+    const bool on = i < n;
+    double x = on ? lanczos_start(i) : 0.0;
+    const double nrm = sqrt(block_sum(x * x));
+    double v_cur = x / nrm, v_prev = 0.0, beta_prev = 0.0;
+    int done_steps = 0, finished = 0;
+    for (int j = 1; j <= steps; ++j) {
+        __syncthreads();
+        v[i] = v_cur;
+        __syncthreads();
+        double w = 0.0;
+        if (on) {
+#pragma unroll 8
+            for (int k = 0; k < n; ++k) w += (double)h0[(size_t)k * ld + i] * v[k];
+            w -= beta_prev * v_prev;
+        }
+        const double alpha = block_sum(on ? v_cur * w : 0.0);
+        w = on ? w - alpha * v_cur : 0.0;
+        const double beta = sqrt(block_sum(w * w));
+        const bool stop = !(beta > 1e-12 * (fabs(alpha) + beta_prev + 1e-300)) || !isfinite(beta);
+        if (i == 0) {
+            st->alpha[j - 1] = alpha;
+            st->beta[j] = stop ? 0.0 : beta;
+        }
+        done_steps = j;
+        if (stop) { finished = 1; break; }
+        v_prev = v_cur;
+        v_cur = w / beta;
+        beta_prev = beta;
+    }
+    if (i == 0) {
+        st->beta[0] = 0.0;
+        st->steps = done_steps;
+        st->finished = finished;
     }
 }
 

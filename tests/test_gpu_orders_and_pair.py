@@ -385,6 +385,18 @@ def test_lanczos_bounds_degenerate_and_options(dev):
     r = s.run()
     s.close()
     assert r.status == 0 and (r.eps_min, r.eps_max) == (-1.0, 1.0)
+    # extreme eigenvectors (e_1 -+ e_2)/sqrt(2), which a start vector of equal-magnitude entries can miss by symmetry
+    n2 = 96
+    hs = np.diag(rng.uniform(-1.0, 1.0, n2)).astype(np.float32)
+    hs[0, 0] = hs[1, 1] = 0.0
+    hs[0, 1] = hs[1, 0] = -3.0
+    evs = np.linalg.eigvalsh(hs.astype(np.float64))
+    b2 = rng.standard_normal((n2, n2)).astype(np.float32)
+    s = Dmpt(n2, device=dev, bounds="lanczos", lanczos_steps=30)
+    s.set_hamiltonian(torch.from_numpy(hs).to(dev), torch.from_numpy(((b2 + b2.T) / 2).astype(np.float32)).to(dev), 40)
+    r = s.run(check=False)
+    s.close()
+    assert r.eps_min <= evs[0] and r.eps_max >= evs[-1], (r.eps_min, evs[0], evs[-1], r.eps_max)
     wl = make_config(1, n=200)
     ev = np.linalg.eigvalsh(wl.h0.astype(np.float64))
     widths = []
@@ -427,3 +439,27 @@ def test_epilogue_paths_are_bit_identical(dev, cfg, n):
     assert np.allclose(a.tr_s, b.tr_s, rtol=1e-12, atol=1e-9)
     assert np.allclose(a.id_err[:a.layers_d0], b.id_err[:a.layers_d0], rtol=1e-6, atol=1e-7 * n)
     assert abs(a.fro_err0 - b.fro_err0) <= 1e-5 * a.fro_err0
+
+
+def test_bench_side_modes_print_one_json_line(dev):
+    """bench.py --fd and --order-parallel on the small configuration: one JSON line each, exit code 0 (the pair's line
+    also asserts bit-identity with the single-context run)."""
+    import json
+    import os
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for flags in (["--fd", "--config", "1", "--fd-steps", "0.01", "0.05", "0.2"],
+                  ["--order-parallel", "--config", "1", "--steps", "2", "--warmup", "2"]):
+        r = subprocess.run([sys.executable, os.path.join(root, "bench.py")] + flags, capture_output=True, text=True,
+                           timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+        assert len(lines) == 1
+        d = json.loads(lines[0])
+        assert d["mode"] in ("fd", "order-parallel") and d["gpu_launches"] > 0 and d["data"] == "synthetic"
+        if d["mode"] == "fd":
+            assert len(d["fd_sweep"]) == 6 and d["best"]["two_point_over_dmpt"] > 1.0 and d["cpu_baseline"]["kind"] == "oracle"
+        else:
+            assert d["config"]["bit_identical_to_single_context"] is True and d["value"] > 0
