@@ -78,7 +78,13 @@ typedef struct dmpt_options {
     int lanczos_steps; /* bounds == 2: number of Lanczos steps, 1..64; 0 = default (20)                          */
     int no_pdl;        /* 1: do not chain the layer launches by programmatic dependent launch (A/B measurements;   */
                        /* results do not depend on it).  0 (default): launches that need no wave barrier are chained */
-    int reserved[3];   /* must be 0                                                                   */
+    int loop_graph;    /* 1: the layer loop runs on the device - ONE launch of a CUDA graph whose conditional WHILE   */
+                       /* node has the launches of a layer as its body and the control step as its condition; the  */
+                       /* host enqueues nothing per layer and looks at no flag (dmpt_run, dmpt_run_orders,          */
+                       /* dmpt_run_fields; not the *_host calls, whose early read-back of D0 needs the host, nor    */
+                       /* order 3).  0 (default): launches enqueued in chunks of 2-8 layers, two chunks ahead,      */
+                       /* one pinned flag per chunk.  Same kernels, bit-identical results                           */
+    int reserved[2];   /* must be 0                                                                   */
 } dmpt_options;
 
 typedef struct dmpt_result {

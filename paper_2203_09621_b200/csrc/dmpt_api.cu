@@ -165,6 +165,12 @@ struct dmpt_ctx {
     cudaStream_t side = nullptr; // copy stream of dmpt_run_host's early D0 read-back
     cudaEvent_t ev_side = nullptr;
     DmptCtl* h_ctl = nullptr;    // pinned
+    // device-side loop (dmpt_options::loop_graph): one WHILE node whose body is the launches of a layer
+    cudaGraph_t loop_graph = nullptr;
+    cudaGraphExec_t loop_exec = nullptr;
+    cudaStream_t capture = nullptr;
+    int loop_n_occ = -1;         // the graph's kernel nodes hold a copy of LayerParams: rebuilt when n_occ changes
+    bool loop_used = false;      // the current run went through the graph
     char err[256] = {0};
 
     template <typename T>
@@ -294,6 +300,7 @@ static int create_impl(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_w
     if (o.max_layers <= 0) o.max_layers = 200;
     if (o.max_layers > kMaxLayersCap) o.max_layers = kMaxLayersCap;
     if (o.s0_shift > 15 || o.bounds < 0 || o.bounds > 2 || o.lanczos_steps < 0) return DMPT_EINVAL;
+    if (pair_side) o.loop_graph = 0;
     if (o.num_fields == 0) o.num_fields = 1;
     if (o.num_fields < 1 || o.num_fields > 3 || (o.num_fields > 1 && o.order != 1)) return DMPT_EINVAL;
     const size_t need = o.num_fields > 1 ? dmpt_workspace_bytes_fields(n, o.num_fields) : dmpt_workspace_bytes(n, o.order);
@@ -433,6 +440,9 @@ extern "C" int dmpt_destroy(dmpt_ctx* ctx) {
     if (ctx->h_ctl) cudaFreeHost(ctx->h_ctl);
     if (ctx->side) cudaStreamDestroy(ctx->side);
     if (ctx->ev_side) cudaEventDestroy(ctx->ev_side);
+    if (ctx->loop_exec) cudaGraphExecDestroy(ctx->loop_exec);
+    if (ctx->loop_graph) cudaGraphDestroy(ctx->loop_graph);
+    if (ctx->capture) cudaStreamDestroy(ctx->capture);
     delete ctx;
     return DMPT_OK;
 }
@@ -449,20 +459,20 @@ extern "C" int dmpt_set_hamiltonian(dmpt_ctx* ctx, const float* d_h0, const floa
 }
 
 template <int PASS>
-static int launch_pass(dmpt_ctx* ctx) {
+static int launch_pass(dmpt_ctx* ctx, cudaStream_t capture = nullptr) {
     // clusters of 2 come from the kernel's __cluster_dims__; the wave barrier needs every CTA resident:
     // a cooperative launch guarantees it or fails
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(ctx->grid_layer);
     cfg.blockDim = dim3(kNumThreads);
     cfg.dynamicSmemBytes = smem_bytes<PASS>();
-    cfg.stream = ctx->stream;
+    cfg.stream = capture ? capture : ctx->stream;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeCooperative;
     attr[0].val.cooperative = ctx->lp.wave_sync ? 1 : 0;
     // without the wave barrier (at most one tile per CTA pair): programmatic dependent launch, see the kernel's first lines
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[1].val.programmaticStreamSerializationAllowed = (ctx->lp.wave_sync || ctx->opt.no_pdl) ? 0 : 1;
+    attr[1].val.programmaticStreamSerializationAllowed = (ctx->lp.wave_sync || ctx->opt.no_pdl || capture) ? 0 : 1;
     cfg.attrs = attr;
     cfg.numAttrs = 2;
     CK(cudaLaunchKernelEx(&cfg, dmpt_layer_kernel<PASS>, ctx->lp));
@@ -482,24 +492,63 @@ extern "C" int dmpt_set_hamiltonian_fields(dmpt_ctx* ctx, const float* d_h0, con
     return DMPT_OK;
 }
 
-static int launch_layer(dmpt_ctx* ctx, int* launches) {
+static int launch_layer(dmpt_ctx* ctx, int* launches, cudaStream_t capture = nullptr) {
     if (ctx->opt.order >= 2) {
         // highest order first: every pass reads the iterates the lower-order passes of this layer are about to replace
         if (ctx->opt.order == 3) {
-            int rc = launch_pass<4>(ctx);
+            int rc = launch_pass<4>(ctx, capture);
             if (rc) return rc;
             ++*launches;
         }
-        int rc = launch_pass<1>(ctx);
+        int rc = launch_pass<1>(ctx, capture);
         if (rc) return rc;
         ++*launches;
     } else if (ctx->opt.num_fields > 1) {       // fields 2 (and 3): same ordering argument as the order-2 pass
-        int rc = launch_pass<2>(ctx);
+        int rc = launch_pass<2>(ctx, capture);
         if (rc) return rc;
         ++*launches;
     }
     ++*launches;
-    return launch_pass<0>(ctx);
+    return launch_pass<0>(ctx, capture);
+}
+
+static int passes_per_layer(const dmpt_ctx* ctx) {
+    return ctx->opt.order >= 2 ? ctx->opt.order : (ctx->opt.num_fields > 1 ? 2 : 1);
+}
+
+// Device-side layer loop: a CUDA graph with ONE conditional WHILE node; its body is the launches of a layer, captured
+// from launch_layer; the control step of pass 0 sets the condition (layer_kernel.cuh).  The host launches the graph
+// once per run and never looks at a flag.  The kernel nodes hold a copy of LayerParams, so the graph is rebuilt when
+// the problem (n_occ) changes.
+static int build_loop_graph(dmpt_ctx* ctx) {
+    if (ctx->loop_exec && ctx->loop_n_occ == ctx->lp.pb.n_occ) return DMPT_OK;
+    if (ctx->loop_exec) { cudaGraphExecDestroy(ctx->loop_exec); ctx->loop_exec = nullptr; }
+    if (ctx->loop_graph) { cudaGraphDestroy(ctx->loop_graph); ctx->loop_graph = nullptr; }
+    if (!ctx->capture) CK(cudaStreamCreateWithFlags(&ctx->capture, cudaStreamNonBlocking));
+    CK(cudaGraphCreate(&ctx->loop_graph, 0));
+    cudaGraphConditionalHandle handle;
+    CK(cudaGraphConditionalHandleCreate(&handle, ctx->loop_graph, 1, cudaGraphCondAssignDefault));
+    cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = handle;
+    np.conditional.type = cudaGraphCondTypeWhile;
+    np.conditional.size = 1;
+    cudaGraphNode_t node;
+    CK(cudaGraphAddNode(&node, ctx->loop_graph, nullptr, 0, &np));
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    ctx->lp.cond = handle;
+    ctx->lp.use_cond = 1;
+    CK(cudaStreamBeginCaptureToGraph(ctx->capture, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+    int dummy = 0;
+    const int rc = launch_layer(ctx, &dummy, ctx->capture);
+    cudaGraph_t out = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(ctx->capture, &out);
+    ctx->lp.use_cond = 0;
+    if (rc) return rc;
+    CK(e);
+    CK(cudaGraphInstantiate(&ctx->loop_exec, ctx->loop_graph, 0));
+    ctx->loop_n_occ = ctx->lp.pb.n_occ;
+    return DMPT_OK;
 }
 
 static int elementwise_grid(const dmpt_ctx* ctx, long long work_items, int threads) {
@@ -648,6 +697,16 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
     }
     CK(cudaEventRecord(ctx->ev_t[1], st));
 
+    if (ctx->opt.loop_graph && !h_d0_early && ctx->opt.order != 3) {
+        // device-side loop: one graph launch, no flag for the host to look at (order 3 sets the first scale of S3
+        // between layers 1 and 2 and keeps the chunked launches)
+        int rcg = build_loop_graph(ctx);
+        if (rcg) return rcg;
+        CK(cudaGraphLaunch(ctx->loop_exec, st));
+        CK(cudaEventRecord(ctx->ev_t[2], st));
+        ctx->loop_used = true;       // finish() adds layers x passes per layer to the launch count
+        return DMPT_OK;
+    }
     // Layer loop.  Launches are enqueued in chunks, two chunks ahead of the GPU; after each chunk a
     // 4-byte copy of ctl.done lands in pinned memory.  Launches after convergence exit at once.
     const int max_layers = ctx->opt.max_layers;
@@ -706,6 +765,8 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
     const DmptCtl& c = *ctx->h_ctl;
     int status = c.status;
     if (status == 0 && !c.done) status = DMPT_ENOCONV;
+    if (ctx->loop_used) launches += c.layers * passes_per_layer(ctx);      // device-side loop: count from the layers
+    ctx->loop_used = false;
     if (res) {
         res->status = status;
         res->layers = c.layers;

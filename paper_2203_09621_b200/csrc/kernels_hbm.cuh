@@ -460,7 +460,13 @@ __global__ void __launch_bounds__(1024) dmpt_lanczos_small_kernel(const float* _
         __syncthreads();
         return bc;
     };
-    const bool on = i < n;
+    // rows padded to a power of two >= 32; the 1024 threads split every column sum into tpr slices of k
+    int rows = 32;
+    while (rows < n) rows <<= 1;
+    const int tpr = 1024 / rows, row = i & (rows - 1), slice = i / rows;
+    const int k_per = (n + tpr - 1) / tpr, k0 = slice * k_per, k1 = min(n, k0 + k_per);
+    __shared__ double part[1024];
+    const bool on = i < n;                       // thread i also owns element i of the vectors
     double x = on ? lanczos_start(i) : 0.0;
     const double nrm = sqrt(block_sum(x * x));
     double v_cur = x / nrm, v_prev = 0.0, beta_prev = 0.0;
@@ -469,10 +475,16 @@ __global__ void __launch_bounds__(1024) dmpt_lanczos_small_kernel(const float* _
         __syncthreads();
         v[i] = v_cur;
         __syncthreads();
+        double acc = 0.0;
+        if (row < n) {
+#pragma unroll 8
+            for (int k = k0; k < k1; ++k) acc += (double)h0[(size_t)k * ld + row] * v[k];
+        }
+        part[i] = acc;
+        __syncthreads();
         double w = 0.0;
         if (on) {
-#pragma unroll 8
-            for (int k = 0; k < n; ++k) w += (double)h0[(size_t)k * ld + i] * v[k];
+            for (int q = 0; q < tpr; ++q) w += part[q * rows + i];       // fixed order
             w -= beta_prev * v_prev;
         }
         const double alpha = block_sum(on ? v_cur * w : 0.0);

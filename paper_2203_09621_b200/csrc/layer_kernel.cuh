@@ -129,6 +129,10 @@ struct LayerParams {
     // order-parallel pair (DmptProblem::pair_side): per-layer records from the order-0 side; side 1 writes them in
     // its control step, side 2 reads its copies at the start of every launch.  NULL otherwise.
     DmptHandoff* handoff;
+    // device-side loop (dmpt_options::loop_graph): the layer launches are the body of a CUDA-graph WHILE node; the
+    // control step sets its condition (1: another layer, 0: done).  use_cond = 0: launches come from the host in chunks.
+    cudaGraphConditionalHandle cond;
+    int use_cond;
 };
 
 __device__ __forceinline__ uint32_t pack2(__half a, __half b) {
@@ -475,7 +479,11 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     griddep_wait();
     // ---- the decision for this layer, taken by the previous launch (both CTAs of a pair read the same)
     DmptCtl c_in = *p.ctl;
-    if (c_in.done) return;
+    if (c_in.done) {
+        // (a run that was over before its first layer, e.g. degenerate bounds: end the WHILE loop)
+        if (PASS == 0 && p.use_cond && blockIdx.x == 0 && threadIdx.x == 0) cudaGraphSetConditional(p.cond, 0u);
+        return;
+    }
     if (PASS == 0 && p.pb.pair_side == 2) {
         handoff_merge(c_in, p.handoff[c_in.layer]);
         if (c_in.done) {            // the order-0 side stopped with an error: pass it on and stop
@@ -941,6 +949,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             if (p.pb.pair_side == 2) handoff_merge(nc, p.handoff[nc.layer]);      // what this launch ran with
             control_finalize(nc, p.logs, p.pb, red, p.handoff);
             *p.ctl = nc;
+            if (p.use_cond) cudaGraphSetConditional(p.cond, nc.done ? 0u : 1u);
         }
     }
 }

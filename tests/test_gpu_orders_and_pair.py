@@ -463,3 +463,68 @@ def test_bench_side_modes_print_one_json_line(dev):
             assert len(d["fd_sweep"]) == 6 and d["best"]["two_point_over_dmpt"] > 1.0 and d["cpu_baseline"]["kind"] == "oracle"
         else:
             assert d["config"]["bit_identical_to_single_context"] is True and d["value"] > 0
+
+
+# ------------------------------------------------------------------------------------------ device-side layer loop
+@pytest.mark.parametrize("cfg,n,order,nf", [(1, 256, 1, 1), (1, 256, 0, 1), (1, 200, 2, 1), (2, 512, 1, 2), (4, 1284, 1, 1)])
+def test_loop_graph_is_bit_identical_to_chunked_launches(dev, cfg, n, order, nf):
+    """dmpt_options::loop_graph: the layer loop as ONE launch of a CUDA graph whose WHILE node is driven by the control
+    step on the device (no flag for the host).  Same kernels: D0, D1 (D2, every field), layer counts and sigma equal
+    the chunked-launch run bit for bit; the launch count is reported from the layers."""
+    from paper_2203_09621_b200 import Dmpt
+    from workloads import make_config
+
+    wl = make_config(cfg, n=n)
+    h0, h1 = torch.from_numpy(wl.h0).to(dev), torch.from_numpy(wl.h1).to(dev)
+    got = {}
+    for lg in (False, True):
+        s = Dmpt(n, device=dev, order=order, num_fields=nf, loop_graph=lg)
+        if nf > 1:
+            s.set_hamiltonian_fields(h0, [h1, (h1 * 0.5).contiguous()], wl.n_occ)
+            r = s.run_fields()
+            r = s.run_fields()                      # a second run re-uses the instantiated graph
+            mats = [r.d0] + list(r.d1)
+        else:
+            s.set_hamiltonian(h0, h1 if order else None, wl.n_occ)
+            r = s.run_orders()
+            r = s.run_orders()
+            mats = [m for m in (r.d0, r.d1, r.d2) if m is not None]
+        assert r.status == 0
+        got[lg] = (r, [m.clone() for m in mats])
+        s.close()
+    (a, ma), (b, mb) = got[False], got[True]
+    assert (a.layers, a.layers_d0, a.layers_d1, a.layers_d2, a.sigma) == (b.layers, b.layers_d0, b.layers_d1, b.layers_d2, b.sigma)
+    assert all(torch.equal(x, y) for x, y in zip(ma, mb))
+    passes = order if order >= 2 else (2 if nf > 1 else 1)
+    assert b.launches >= b.layers * passes and b.launches <= b.layers * passes + 12
+
+
+def test_loop_graph_ends_on_errors_and_follows_n_occ(dev):
+    """The WHILE loop must also end when the run is over before its first layer (degenerate bounds) and at max_layers;
+    the graph holds a copy of the problem description and is rebuilt when n_occ changes."""
+    from paper_2203_09621_b200 import Dmpt
+    from paper_2203_09621_b200 import binding as B
+    from workloads import make_config
+
+    s = Dmpt(128, device=dev, loop_graph=True)
+    z = torch.zeros((128, 128), device=dev)
+    s.set_hamiltonian(z, z, 64)
+    r = s.run(check=False)
+    assert r.status == B.DMPT_EDEGENERATE and r.layers == 0
+    s.close()
+    wl = make_config(1)
+    h0, h1 = torch.from_numpy(wl.h0).to(dev), torch.from_numpy(wl.h1).to(dev)
+    s = Dmpt(256, device=dev, loop_graph=True, max_layers=5)
+    s.set_hamiltonian(h0, h1, wl.n_occ)
+    r = s.run(check=False)
+    assert r.status == B.DMPT_ENOCONV and r.layers == 5
+    s.close()
+    s = Dmpt(256, device=dev, loop_graph=True)
+    t = Dmpt(256, device=dev)
+    for n_occ in (wl.n_occ, 100, wl.n_occ):
+        s.set_hamiltonian(h0, h1, n_occ)
+        t.set_hamiltonian(h0, h1, n_occ)
+        a, b = s.run(check=False), t.run(check=False)
+        assert a.status == b.status and a.layers == b.layers and torch.equal(a.d0, b.d0) and torch.equal(a.d1, b.d1)
+    s.close()
+    t.close()
