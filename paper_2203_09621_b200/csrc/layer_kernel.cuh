@@ -912,35 +912,46 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         is_last = (prev == gridDim.x - 1);
     }
     __syncthreads();
-    if (is_last && warp == 0) {
+    if (is_last) {
         __threadfence();
-        // fixed-order fp64 reduction: lane l sums slots l, l+32, ...; then a shuffle tree
+        // fixed-order fp64 reduction by the whole CTA: thread t sums slots t, t + 384, ...; a shuffle tree per warp;
+        // the twelve warp sums are added in warp order
+        __shared__ double s_red[kNumThreads / 32][RED_COUNT];
         const int nslots = gridDim.x * kNumEpiWarps;
+        const bool second = p.pb.order >= 2 || p.pb.nfields >= 2;       // slots 2, 3 come from the other passes
+        const bool third = p.pb.order == 3;                             // slot 3 from the order-3 pass
         double red[RED_COUNT];
 #pragma unroll
         for (int k = 0; k < RED_COUNT; ++k) red[k] = 0.0;
-        for (int s = lane; s < nslots; s += 32) {
-            const volatile double* in = p.partials + (size_t)s * RED_COUNT;
-            const volatile double* in2 = p.partials2 + (size_t)s * RED_COUNT;
-            const volatile double* in3 = p.partials3 + (size_t)s * RED_COUNT;
+        for (int s = (int)threadIdx.x; s < nslots; s += kNumThreads) {
+            const double* in = p.partials + (size_t)s * RED_COUNT;          // written by other CTAs: read past L1
+            const double* in2 = p.partials2 + (size_t)s * RED_COUNT;
+            const double* in3 = p.partials3 + (size_t)s * RED_COUNT;
 #pragma unroll
             for (int k = 0; k < RED_COUNT; ++k) {
-                const bool second = p.pb.order >= 2 || p.pb.nfields >= 2;       // slots 2, 3 come from the other passes
-                const bool third = p.pb.order == 3;                             // slot 3 from the order-3 pass
-                if (k == RED_MAX1) red[k] = fmax(red[k], in[k]);
-                else if (k == RED_MAX2) { if (second) red[k] = fmax(red[k], in2[k]); }
-                else if (k == RED_MAX3) { if (second) red[k] = fmax(red[k], third ? in3[k] : in2[k]); }
-                else if (k == RED_FRO2) { if (second) red[k] += in2[k]; }
-                else if (k == RED_FRO3) { if (second) red[k] += third ? in3[k] : in2[k]; }
-                else red[k] += in[k];
+                if (k == RED_MAX1) red[k] = fmax(red[k], __ldcg(in + k));
+                else if (k == RED_MAX2) { if (second) red[k] = fmax(red[k], __ldcg(in2 + k)); }
+                else if (k == RED_MAX3) { if (second) red[k] = fmax(red[k], __ldcg((third ? in3 : in2) + k)); }
+                else if (k == RED_FRO2) { if (second) red[k] += __ldcg(in2 + k); }
+                else if (k == RED_FRO3) { if (second) red[k] += __ldcg((third ? in3 : in2) + k); }
+                else if (k < RED_FRO2) red[k] += __ldcg(in + k);
             }
         }
 #pragma unroll
         for (int k = 0; k < RED_COUNT; ++k) {
             if (k == RED_MAX1 || k == RED_MAX2 || k == RED_MAX3) red[k] = warp_max(red[k]);
             else red[k] = warp_sum(red[k]);
+            if (lane == 0) s_red[warp][k] = red[k];
         }
-        if (lane == 0) {
+        __syncthreads();
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int k = 0; k < RED_COUNT; ++k) {
+                double v = s_red[0][k];
+                for (int w = 1; w < kNumThreads / 32; ++w)
+                    v = (k == RED_MAX1 || k == RED_MAX2 || k == RED_MAX3) ? fmax(v, s_red[w][k]) : v + s_red[w][k];
+                red[k] = v;
+            }
             DmptCtl nc = *p.ctl;
             nc.ticket = 0;
             nc.wave = 0;
