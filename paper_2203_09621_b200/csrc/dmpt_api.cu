@@ -383,6 +383,7 @@ static int create_impl(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_w
         return fail(DMPT_ECUDA);
     }
     if (max_clusters > ctx->num_sms / 2) max_clusters = ctx->num_sms / 2;
+    if (max_clusters > kRedStride / (2 * kNumEpiWarps)) max_clusters = kRedStride / (2 * kNumEpiWarps);   // partials: [component][slot]
     ctx->grid_layer = 2 * (L.num_tiles < max_clusters ? L.num_tiles : max_clusters);
 
     LayerParams& lp = ctx->lp;

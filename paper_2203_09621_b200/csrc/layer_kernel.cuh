@@ -74,6 +74,7 @@ template <> struct PassCfg<4> { static constexpr int kOps = 8, kStages = 2; };
 constexpr int kChunkK = 128;               // promotion interval along K
 constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
+constexpr int kRedStride = 2048;           // per-warp partials are stored [component][slot], slot < gridDim.x * 8 <= 2048
 constexpr int kTmemCols = 512;
 constexpr int kEpiWarp0 = 4;               // warpgroup 0: TMA producer, MMA issuer, two idle warps; warpgroups 1, 2: epilogue
 constexpr int kNumEpiWarps = 8;
@@ -881,17 +882,18 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         const double mx1 = warp_max((double)r_mx1);
         const double mx0 = warp_max((double)r_mx0);
         if (lane == 0) {
+            // component-major: [RED_x][slot], so that the control step reads consecutive doubles
             double* out = (PASS == 0 ? p.partials : (PASS == 4 ? p.partials3 : p.partials2)) +
-                          ((size_t)blockIdx.x * kNumEpiWarps + (warp - kEpiWarp0)) * RED_COUNT;
-            out[RED_TR_S0] = r_tr;
-            out[RED_FRO_S0] = r_fs0;
-            out[RED_FRO0] = PASS == 0 ? r_f0 : 0.0;
-            out[RED_FRO1] = PASS == 0 ? r_f1 : 0.0;
-            out[RED_MAX1] = PASS == 0 ? mx1 : 0.0;
-            out[RED_FRO2] = PASS == 1 ? r_f1 : (PASS == 2 ? r_f0 : 0.0);      // slot 2: S2, or field 2
-            out[RED_MAX2] = PASS == 1 ? mx1 : (PASS == 2 ? mx0 : 0.0);
-            out[RED_FRO3] = (PASS == 2 || PASS == 4) ? r_f1 : 0.0;             // slot 3: field 3, or S3
-            out[RED_MAX3] = (PASS == 2 || PASS == 4) ? mx1 : 0.0;
+                          ((size_t)blockIdx.x * kNumEpiWarps + (warp - kEpiWarp0));
+            out[RED_TR_S0 * kRedStride] = r_tr;
+            out[RED_FRO_S0 * kRedStride] = r_fs0;
+            out[RED_FRO0 * kRedStride] = PASS == 0 ? r_f0 : 0.0;
+            out[RED_FRO1 * kRedStride] = PASS == 0 ? r_f1 : 0.0;
+            out[RED_MAX1 * kRedStride] = PASS == 0 ? mx1 : 0.0;
+            out[RED_FRO2 * kRedStride] = PASS == 1 ? r_f1 : (PASS == 2 ? r_f0 : 0.0);      // slot 2: S2, or field 2
+            out[RED_MAX2 * kRedStride] = PASS == 1 ? mx1 : (PASS == 2 ? mx0 : 0.0);
+            out[RED_FRO3 * kRedStride] = (PASS == 2 || PASS == 4) ? r_f1 : 0.0;             // slot 3: field 3, or S3
+            out[RED_MAX3 * kRedStride] = (PASS == 2 || PASS == 4) ? mx1 : 0.0;
         }
     }
 
@@ -924,17 +926,17 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
 #pragma unroll
         for (int k = 0; k < RED_COUNT; ++k) red[k] = 0.0;
         for (int s = (int)threadIdx.x; s < nslots; s += kNumThreads) {
-            const double* in = p.partials + (size_t)s * RED_COUNT;          // written by other CTAs: read past L1
-            const double* in2 = p.partials2 + (size_t)s * RED_COUNT;
-            const double* in3 = p.partials3 + (size_t)s * RED_COUNT;
+            const double* in = p.partials + s;          // written by other CTAs: read past L1
+            const double* in2 = p.partials2 + s;
+            const double* in3 = p.partials3 + s;
 #pragma unroll
             for (int k = 0; k < RED_COUNT; ++k) {
-                if (k == RED_MAX1) red[k] = fmax(red[k], __ldcg(in + k));
-                else if (k == RED_MAX2) { if (second) red[k] = fmax(red[k], __ldcg(in2 + k)); }
-                else if (k == RED_MAX3) { if (second) red[k] = fmax(red[k], __ldcg((third ? in3 : in2) + k)); }
-                else if (k == RED_FRO2) { if (second) red[k] += __ldcg(in2 + k); }
-                else if (k == RED_FRO3) { if (second) red[k] += __ldcg((third ? in3 : in2) + k); }
-                else if (k < RED_FRO2) red[k] += __ldcg(in + k);
+                if (k == RED_MAX1) red[k] = fmax(red[k], __ldcg(in + k * kRedStride));
+                else if (k == RED_MAX2) { if (second) red[k] = fmax(red[k], __ldcg(in2 + k * kRedStride)); }
+                else if (k == RED_MAX3) { if (second) red[k] = fmax(red[k], __ldcg((third ? in3 : in2) + k * kRedStride)); }
+                else if (k == RED_FRO2) { if (second) red[k] += __ldcg(in2 + k * kRedStride); }
+                else if (k == RED_FRO3) { if (second) red[k] += __ldcg((third ? in3 : in2) + k * kRedStride); }
+                else if (k < RED_FRO2) red[k] += __ldcg(in + k * kRedStride);
             }
         }
 #pragma unroll
@@ -944,14 +946,18 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             if (lane == 0) s_red[warp][k] = red[k];
         }
         __syncthreads();
-        if (threadIdx.x == 0) {
-#pragma unroll
-            for (int k = 0; k < RED_COUNT; ++k) {
-                double v = s_red[0][k];
-                for (int w = 1; w < kNumThreads / 32; ++w)
-                    v = (k == RED_MAX1 || k == RED_MAX2 || k == RED_MAX3) ? fmax(v, s_red[w][k]) : v + s_red[w][k];
-                red[k] = v;
+        // the twelve warp sums of component k are added by lane k (fp64 adds are slow: not one thread for all)
+        if (warp == 0) {
+            double v = 0.0;
+            if (lane < RED_COUNT) {
+                const bool is_max = lane == RED_MAX1 || lane == RED_MAX2 || lane == RED_MAX3;
+                v = s_red[0][lane];
+                for (int w = 1; w < kNumThreads / 32; ++w) v = is_max ? fmax(v, s_red[w][lane]) : v + s_red[w][lane];
             }
+#pragma unroll
+            for (int k = 0; k < RED_COUNT; ++k) red[k] = __shfl_sync(0xffffffffu, v, k);
+        }
+        if (threadIdx.x == 0) {
             DmptCtl nc = *p.ctl;
             nc.ticket = 0;
             nc.wave = 0;
