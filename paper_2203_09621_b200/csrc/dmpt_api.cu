@@ -274,10 +274,29 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
     for (int i = 0; i < 3; ++i)
         for (int t = 0; t < 2; ++t)
             if (encode_epi(&ctx->lp.emap32[i][t], f32[i], false, t == 1)) return DMPT_ECUDA;
+    // (hi, lo) pairs as 3D tensors: dimension 2 = the word (hi: plane 0, lo: plane 1); the two matrices of a pair are
+    // consecutive blocks of the workspace (make_layout), n_pad^2 fp16 apart
     for (int b = 0; b < 2; ++b)
-        for (int m = 0; m < 4; ++m)
-            for (int t = 0; t < 2; ++t)
-                if (encode_epi(&ctx->lp.emap16[b][m][t], ctx->at<void>(L.h[b][m]), true, t == 1)) return DMPT_ECUDA;
+        for (int pr = 0; pr < 2; ++pr)
+            for (int t = 0; t < 2; ++t) {
+                const bool mirrored = t == 1;
+                if (L.h[b][2 * pr + 1] - L.h[b][2 * pr] != (size_t)L.n_pad * L.n_pad * 2) {
+                    snprintf(ctx->err, sizeof ctx->err, "workspace layout: hi and lo of an operand pair are not adjacent");
+                    return DMPT_ECUDA;
+                }
+                const cuuint64_t dims3[3] = {(cuuint64_t)L.n_pad, (cuuint64_t)L.n_pad, 2};
+                const cuuint64_t str3[2] = {(cuuint64_t)L.n_pad * 2, (cuuint64_t)L.n_pad * L.n_pad * 2};
+                const cuuint32_t box3[3] = {(cuuint32_t)(mirrored ? 32 : kSub), (cuuint32_t)(mirrored ? kSub : 32), 2};
+                const cuuint32_t es3[3] = {1, 1, 1};
+                CUresult r = encode(&ctx->lp.emap16[b][pr][t], CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3,
+                                    ctx->at<void>(L.h[b][2 * pr]), dims3, str3, box3, es3, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                    mirrored ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_32B,
+                                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                if (r != CUDA_SUCCESS) {
+                    snprintf(ctx->err, sizeof ctx->err, "cuTensorMapEncodeTiled (operand-pair map) failed with CUresult %d", (int)r);
+                    return DMPT_ECUDA;
+                }
+            }
     return DMPT_OK;
 }
 

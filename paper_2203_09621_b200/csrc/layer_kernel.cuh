@@ -107,7 +107,9 @@ struct LayerParams {
     CUtensorMap maps[2][8];     // [buffer][Mhi, Mlo, S1hi, S1lo, S2hi, S2lo, S3hi, S3lo], box = kBK x kBRows, SWIZZLE_64B
     // epilogue maps: [..][0] direct 16 x 32 box (fp32: SWIZZLE_64B, fp16: SWIZZLE_32B), [..][1] mirrored 32 x 16 box
     CUtensorMap emap32[3][2];   // fp32 iterates S0, S1[0], S1[1]
-    CUtensorMap emap16[2][4][2];  // fp16 operand matrices [buffer][Mhi, Mlo, S1hi, S1lo]
+    CUtensorMap emap16[2][2][2];  // fp16 operand PAIRS [buffer][(Mhi, Mlo), (S1hi, S1lo)]: 3D maps, the hi and the lo matrix
+                                // of a pair lie back to back in the workspace and are the two planes of one tensor, so
+                                // that one TMA store writes a block of both
     float* s0;                  // fp32 S0, updated in place, ld = n_pad
     float* s1[2];               // fp32 S1, ping-pong
     float* s2[2];               // fp32 response slot 2, ping-pong (order 2: S2; multi-field: S1 of field 2)
@@ -148,11 +150,10 @@ struct EpiOut {
     const float* old;      // fp32 matrix holding the previous iterate
     __half* hi;
     __half* lo;
-    // TMA path: maps of the same four matrices (direct box; the mirrored box is the next map)
+    // TMA path: maps of the same matrices (direct box; the mirrored box is the next map); m_hl: the (hi, lo) pair
     const CUtensorMap* m_old;
     const CUtensorMap* m_dst;
-    const CUtensorMap* m_hi;
-    const CUtensorMap* m_lo;
+    const CUtensorMap* m_hl;
 };
 
 struct EpiTma {            // shared-memory addresses of this warp's staging
@@ -252,7 +253,7 @@ __device__ __forceinline__ void final_epilogue(float (&acc)[kHalfCols], const Ep
 // final_epilogue with w = 2, dg = 0 (so delta = -+unscale acc exactly and S <- fmaf(+-unscale, acc, old)), but
 //   * the old iterate comes by TMA into this warp's ring (issued one step ahead),
 //   * the new iterate and its split are written to shared memory in the direct and the transposed layout and
-//     leave by six TMA stores per 32 x 16 block: full lines instead of row-per-thread accesses,
+//     leave by four TMA stores per 32 x 16 block (fp32 and the (hi, lo) pair; direct and mirrored): full lines instead of row-per-thread accesses,
 //   * the split uses the packed conversions (cvt.rn.f16x2.f32).
 // step s (0 .. ns-1) of the tile handles product s / 4 (0: P0, 1: P1; when only one is live it is steps 0-3) and
 // columns (s & 3) * 16 of this thread's 64.
@@ -442,10 +443,8 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
         if (lane == 0) {
             tma_store_2d(o.m_dst, et.ring[slot], gc0, gr0);
             tma_store_2d(o.m_dst + 1, et.t32, gr0, gc0);
-            tma_store_2d(o.m_hi, et.dhi, gc0, gr0);
-            tma_store_2d(o.m_hi + 1, et.thi, gr0, gc0);
-            tma_store_2d(o.m_lo, et.dlo, gc0, gr0);
-            tma_store_2d(o.m_lo + 1, et.tlo, gr0, gc0);
+            tma_store_3d(o.m_hl, et.dhi, gc0, gr0, 0);          // dhi, dlo: the two planes of the direct box
+            tma_store_3d(o.m_hl + 1, et.thi, gr0, gc0, 0);      // thi, tlo: of the mirrored box
             bulk_commit();
         }
     }
@@ -728,9 +727,9 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             o1.dst = p.s1[c.s1_buf ^ 1]; o1.old = p.s1[c.s1_buf];
             o1.hi = p.h[c.s1_buf ^ 1][S1H]; o1.lo = p.h[c.s1_buf ^ 1][S1L];
             o0.m_old = o0.m_dst = &p.emap32[0][0];
-            o0.m_hi = &p.emap16[c.s0_buf ^ 1][MH][0]; o0.m_lo = &p.emap16[c.s0_buf ^ 1][ML][0];
+            o0.m_hl = &p.emap16[c.s0_buf ^ 1][0][0];
             o1.m_old = &p.emap32[1 + c.s1_buf][0]; o1.m_dst = &p.emap32[1 + (c.s1_buf ^ 1)][0];
-            o1.m_hi = &p.emap16[c.s1_buf ^ 1][S1H][0]; o1.m_lo = &p.emap16[c.s1_buf ^ 1][S1L][0];
+            o1.m_hl = &p.emap16[c.s1_buf ^ 1][1][0];
         } else if (PASS == 1) {
             o0.dst = nullptr; o0.old = nullptr; o0.hi = nullptr; o0.lo = nullptr;
             o1.dst = p.s2[c.s2_buf ^ 1]; o1.old = p.s2[c.s2_buf];
