@@ -252,28 +252,20 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
                 return DMPT_ECUDA;
             }
         }
-    // epilogue maps of the layer kernel's TMA path (layer_kernel.cuh, final_epilogue_tma): per matrix a direct
-    // 16 x 32 box (swizzled so that one thread per row reads and writes it without bank conflicts) and a
-    // mirrored 32 x 16 box (written transposed, one row per instruction)
-    auto encode_epi = [&](CUtensorMap* m, void* base, bool fp16, bool mirrored) -> int {
-        const cuuint64_t est1[1] = {(cuuint64_t)L.n_pad * (fp16 ? 2 : 4)};
-        const cuuint32_t ebox[2] = {(cuuint32_t)(mirrored ? 32 : kSub), (cuuint32_t)(mirrored ? kSub : 32)};
-        const CUtensorMapSwizzle sw = mirrored ? CU_TENSOR_MAP_SWIZZLE_NONE
-                                               : (fp16 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_64B);
-        CUresult r = encode(m, fp16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims,
-                            est1, ebox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
-                            fp16 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+    // epilogue maps of the layer kernel's TMA path (layer_kernel.cuh, final_epilogue_tma).  fp32 iterates: a 16 x 32 box,
+    // swizzled so that one thread per row reads and writes it without bank conflicts
+    void* f32[3] = {ctx->at<void>(L.s0), ctx->at<void>(L.s1[0]), ctx->at<void>(L.s1[1])};
+    for (int i = 0; i < 3; ++i) {
+        const cuuint64_t est1[1] = {(cuuint64_t)L.n_pad * 4};
+        const cuuint32_t ebox[2] = {(cuuint32_t)kSub, 32};
+        CUresult r = encode(&ctx->lp.emap32[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, f32[i], dims, est1, ebox, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) {
             snprintf(ctx->err, sizeof ctx->err, "cuTensorMapEncodeTiled (epilogue map) failed with CUresult %d", (int)r);
             return DMPT_ECUDA;
         }
-        return DMPT_OK;
-    };
-    void* f32[3] = {ctx->at<void>(L.s0), ctx->at<void>(L.s1[0]), ctx->at<void>(L.s1[1])};
-    for (int i = 0; i < 3; ++i)
-        for (int t = 0; t < 2; ++t)
-            if (encode_epi(&ctx->lp.emap32[i][t], f32[i], false, t == 1)) return DMPT_ECUDA;
+    }
     // (hi, lo) pairs as 3D tensors: dimension 2 = the word (hi: plane 0, lo: plane 1); the two matrices of a pair are
     // consecutive blocks of the workspace (make_layout), n_pad^2 fp16 apart
     for (int b = 0; b < 2; ++b)
@@ -286,11 +278,12 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
                 }
                 const cuuint64_t dims3[3] = {(cuuint64_t)L.n_pad, (cuuint64_t)L.n_pad, 2};
                 const cuuint64_t str3[2] = {(cuuint64_t)L.n_pad * 2, (cuuint64_t)L.n_pad * L.n_pad * 2};
-                const cuuint32_t box3[3] = {(cuuint32_t)(mirrored ? 32 : kSub), (cuuint32_t)(mirrored ? kSub : 32), 2};
+                // direct: 32 columns (two epilogue steps) x 32 rows, 64-byte rows; mirrored: 32 columns x 16 rows
+                const cuuint32_t box3[3] = {32, (cuuint32_t)(mirrored ? kSub : 32), 2};
                 const cuuint32_t es3[3] = {1, 1, 1};
                 CUresult r = encode(&ctx->lp.emap16[b][pr][t], CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3,
                                     ctx->at<void>(L.h[b][2 * pr]), dims3, str3, box3, es3, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                    mirrored ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_32B,
+                                    mirrored ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_64B,
                                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
                 if (r != CUDA_SUCCESS) {
                     snprintf(ctx->err, sizeof ctx->err, "cuTensorMapEncodeTiled (operand-pair map) failed with CUresult %d", (int)r);
@@ -579,6 +572,16 @@ static int elementwise_grid(const dmpt_ctx* ctx, long long work_items, int threa
     return (int)blocks;
 }
 
+// Lower triangle of an fp32 workspace iterate <- its upper triangle (the layer kernel's TMA epilogue keeps only the
+// blocks on or above the diagonal up to date): before the iterate is copied out or read row by row.
+static int symmetrize(dmpt_ctx* ctx, float* m, cudaStream_t st, int* launches = nullptr) {
+    const long long tiles = (long long)(ctx->L.n_pad / 32) * (ctx->L.n_pad / 32);
+    dmpt_symmetrize_kernel<<<elementwise_grid(ctx, tiles * 256, 256), 256, 0, st>>>(m, ctx->L.n_pad);
+    CK(cudaGetLastError());
+    if (launches) ++*launches;
+    return DMPT_OK;
+}
+
 // a2 + a3 fused (dmpt_transform_split_kernel): S0, S1_f and their first operand splits in one pass over H0, H1_f.
 static int launch_transform_split(dmpt_ctx* ctx, const float* d_h0, const H1Ptrs& h1p, int ld, int nf, int* grid_out) {
     const Layout& L = ctx->L;
@@ -742,6 +745,7 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
                 // max|S3_2| <= 2 max_i ||row_i S1_1|| max_j ||row_j S2_1||; two HBM passes (reading R12 at order 3).
                 unsigned long long* est = ctx->at<unsigned long long>(L.s2_est);
                 const int rg = elementwise_grid(ctx, (long long)np * 32, 256);
+                { int rs = symmetrize(ctx, ctx->lp.s1[1], st, launches); if (rs) return rs; }      // whole rows are read
                 dmpt_rowsq_max_kernel<<<rg, 256, 0, st>>>(ctx->lp.s1[1], np, est + 1);
                 CK(cudaGetLastError());
                 dmpt_rowsq_max_kernel<<<rg, 256, 0, st>>>(ctx->lp.s2[1], np, est + 2);
@@ -765,6 +769,7 @@ static int run_core(dmpt_ctx* ctx, const float* d_h0, const float* d_h1, int ld,
         CK(cudaEventSynchronize(ctx->ev[w % kNumEvents]));
         if (h_d0_early && !*early_issued && ctx->h_flags0[w % kFlagSlots] && !ctx->h_flags[w % kFlagSlots]) {
             // the launch that set conv0 has completed: S0 will not change any more
+            { int rs = symmetrize(ctx, ctx->lp.s0, ctx->side, launches); if (rs) return rs; }
             CK(cudaMemcpy2DAsync(h_d0_early, (size_t)ld_early * 4, ctx->lp.s0, (size_t)np * 4, (size_t)n * 4, n,
                                  cudaMemcpyDeviceToHost, ctx->side));
             CK(cudaEventRecord(ctx->ev_side, ctx->side));
@@ -874,6 +879,8 @@ static int run_orders_impl(dmpt_ctx* ctx, float* d_d0, float* d_d1, float* d_d2,
     if (rc) return rc;
     if ((rc = fetch_ctl(ctx))) return rc;
     if ((rc = unscale_outputs(ctx, &launches))) return rc;
+    if ((rc = symmetrize(ctx, ctx->lp.s0, ctx->stream, &launches))) return rc;
+    if (order >= 1 && (rc = symmetrize(ctx, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], ctx->stream, &launches))) return rc;
     CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
     if (order >= 1)
         CK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
@@ -917,6 +924,8 @@ extern "C" int dmpt_run_fields(dmpt_ctx* ctx, float* d_d0, float* const* d_d1, i
     const DmptCtl& c = *ctx->h_ctl;
     const float* src[3] = {ctx->lp.s1[c.s1_buf & 1], nf > 1 ? ctx->lp.s2[c.s2_buf & 1] : nullptr,
                            nf > 2 ? ctx->lp.s3[c.s3_buf & 1] : nullptr};
+    if ((rc = symmetrize(ctx, ctx->lp.s0, ctx->stream, &launches))) return rc;
+    if ((rc = symmetrize(ctx, ctx->lp.s1[c.s1_buf & 1], ctx->stream, &launches))) return rc;
     CK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
     for (int f = 0; f < nf; ++f)
         CK(cudaMemcpy2DAsync(d_d1[f], (size_t)ld * 4, src[f], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -957,10 +966,13 @@ extern "C" int dmpt_run_fields_host(dmpt_ctx* ctx, const float* h_h0, const floa
     const DmptCtl& c = *ctx->h_ctl;
     const float* src[3] = {ctx->lp.s1[c.s1_buf & 1], nf > 1 ? ctx->lp.s2[c.s2_buf & 1] : nullptr,
                            nf > 2 ? ctx->lp.s3[c.s3_buf & 1] : nullptr};
-    if (early)
+    if ((rc = symmetrize(ctx, ctx->lp.s1[c.s1_buf & 1], st, &launches))) return rc;
+    if (early) {
         CK(cudaStreamWaitEvent(st, ctx->ev_side, 0));
-    else
+    } else {
+        if ((rc = symmetrize(ctx, ctx->lp.s0, st, &launches))) return rc;
         CK(cudaMemcpy2DAsync(h_d0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToHost, st));
+    }
     for (int f = 0; f < nf; ++f)
         CK(cudaMemcpy2DAsync(h_d1[f], (size_t)ld_out * 4, src[f], np * 4, n * 4, n, cudaMemcpyDeviceToHost, st));
     return finish(ctx, res, launches);
@@ -988,10 +1000,13 @@ extern "C" int dmpt_run_host(dmpt_ctx* ctx, const float* h_h0, const float* h_h1
     if (rc) return rc;
     if ((rc = fetch_ctl(ctx))) return rc;
     if ((rc = unscale_outputs(ctx, &launches))) return rc;
-    if (early)
+    if (ctx->opt.order >= 1 && (rc = symmetrize(ctx, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], ctx->stream, &launches))) return rc;
+    if (early) {
         CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_side, 0));       // D0 went out while the last layers ran
-    else
+    } else {
+        if ((rc = symmetrize(ctx, ctx->lp.s0, ctx->stream, &launches))) return rc;
         CK(cudaMemcpy2DAsync(h_d0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToHost, ctx->stream));
+    }
     if (ctx->opt.order >= 1)
         CK(cudaMemcpy2DAsync(h_d1, (size_t)ld_out * 4, ctx->lp.s1[ctx->h_ctl->s1_buf & 1], np * 4, n * 4, n,
                              cudaMemcpyDeviceToHost, ctx->stream));
@@ -1055,6 +1070,8 @@ extern "C" int dmpt_layer_products(dmpt_ctx* ctx, const float* d_s0, const float
     CK(cudaGetLastError());
     int rc = launch_pass<0>(ctx);
     if (rc) return rc;
+    if ((rc = symmetrize(ctx, ctx->lp.s0, st))) return rc;
+    if ((rc = symmetrize(ctx, ctx->lp.s1[1], st))) return rc;
     CK(cudaMemcpy2DAsync(d_x0, (size_t)ld_out * 4, ctx->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaMemcpy2DAsync(d_x1, (size_t)ld_out * 4, ctx->lp.s1[1], np * 4, n * 4, n, cudaMemcpyDeviceToDevice, st));
     CK(cudaStreamSynchronize(st));
@@ -1225,6 +1242,7 @@ extern "C" int dmpt_fd_response(dmpt_ctx* ctx, const float* d_h0, const float* d
         int rc = run_core(ctx, hp, nullptr, n, &launches);
         if (rc) return rc;
         if ((rc = fetch_ctl(ctx))) return rc;
+        if ((rc = symmetrize(ctx, ctx->lp.s0, st))) return rc;
         dmpt_fd_accum_kernel<<<egrid, 256, 0, st>>>(ctx->lp.s0, n, np, ws[k] / h, k == 0, d_d1, ld_out);
         CK(cudaGetLastError());
         CK(cudaEventRecord(ctx->ev_t[3], st));
@@ -1687,12 +1705,14 @@ extern "C" int dmpt_pair_run(dmpt_pair* pr, float* d_d0, float* d_d1, int ld, dm
     PK(cudaEventRecord(c1->ev_t[2], pr->st[1]));
     if (fetch_ctl(c1)) { snprintf(pr->err, sizeof pr->err, "%s", c1->err); return DMPT_ECUDA; }
     if (unscale_outputs(c1, &launches)) { snprintf(pr->err, sizeof pr->err, "%s", c1->err); return DMPT_ECUDA; }
+    if (symmetrize(c1, c1->lp.s1[c1->h_ctl->s1_buf & 1], pr->st[1], &launches)) { snprintf(pr->err, sizeof pr->err, "%s", c1->err); return DMPT_ECUDA; }
     PK(cudaMemcpy2DAsync(d_d1, (size_t)ld * 4, c1->lp.s1[c1->h_ctl->s1_buf & 1], np * 4, n * 4, n,
                          cudaMemcpyDeviceToDevice, pr->st[1]));
     PK(cudaEventRecord(c1->ev_t[3], pr->st[1]));
     PK(cudaSetDevice(pr->dev[0]));
     PK(cudaStreamSynchronize(pr->copy));
     if (fetch_ctl(c0)) { snprintf(pr->err, sizeof pr->err, "%s", c0->err); return DMPT_ECUDA; }
+    if (symmetrize(c0, c0->lp.s0, pr->st[0], &launches)) { snprintf(pr->err, sizeof pr->err, "%s", c0->err); return DMPT_ECUDA; }
     PK(cudaMemcpy2DAsync(d_d0, (size_t)ld * 4, c0->lp.s0, np * 4, n * 4, n, cudaMemcpyDeviceToDevice, pr->st[0]));
     PK(cudaStreamSynchronize(pr->st[0]));
     PK(cudaSetDevice(pr->dev[1]));

@@ -594,6 +594,33 @@ __global__ void __launch_bounds__(256) dmpt_pad_copy_t_kernel(const float* __res
 }
 
 // ---------------------------------------------------------------------------------------------
+// Lower triangle <- transpose of the upper triangle, in place, on an n_pad x n_pad workspace matrix.  The layer
+// kernel's TMA epilogue keeps only the blocks on or above the diagonal of the fp32 iterates up to date (nothing reads
+// the others during a run: every product works on tiles i <= j); this pass restores the full symmetric matrix before
+// an iterate leaves the workspace.  32 x 32 tiles through shared memory: full lines in, full lines out.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dmpt_symmetrize_kernel(float* __restrict__ a, int n_pad) {
+    __shared__ float tile[32][33];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int T = n_pad >> 5;
+    const long long num = (long long)T * T;
+    for (long long t = blockIdx.x; t < num; t += gridDim.x) {
+        const int bi = (int)(t / T), bj = (int)(t - (long long)bi * T);      // destination tile (bi, bj), bi >= bj
+        if (bi < bj) continue;
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 4; ++k)                                           // source tile (bj, bi), above the diagonal
+            tile[ty + 8 * k][tx] = a[(size_t)(bj * 32 + ty + 8 * k) * n_pad + bi * 32 + tx];
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int r = bi * 32 + ty + 8 * k, c = bj * 32 + tx;
+            if (r > c) a[(size_t)r * n_pad + c] = tile[tx][ty + 8 * k];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Finite-difference response from ground-state runs (Eqs. 83-84): the two elementwise steps.
 //   dmpt_axpy_kernel:     out = H0 + t H1, formed in fp64 and rounded once (n x n, dense, leading dimension n)
 //   dmpt_fd_accum_kernel: acc = (first ? 0 : acc) + w D, w = stencil weight / (denominator h), fp64 per element

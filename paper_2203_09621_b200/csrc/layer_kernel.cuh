@@ -84,12 +84,14 @@ constexpr int kNumThreads = 32 * (kEpiWarp0 + kNumEpiWarps);   // 384
 constexpr int kRegsLight = 152, kRegsEpi = 176;
 constexpr int kHalfCols = kTile / 2;       // accumulator columns per epilogue thread and product
 constexpr int kSub = 16;                   // columns per step of the final epilogue
-// Final epilogue through shared memory and TMA (PASS 0, off-diagonal tiles).  Each epilogue warp owns 10 KiB:
+// Final epilogue through shared memory and TMA (PASS 0).  Each epilogue warp owns 10 KiB:
 //   ring[2]  32 x 16 fp32 (SWIZZLE_64B): the old iterate arrives here by TMA, the new one is written in place
-//   t32      16 x 32 fp32: the same block transposed (mirrored copy)
-//   dhi, dlo 32 x 16 fp16 (SWIZZLE_32B);  thi, tlo 16 x 32 fp16: the operand split, direct and mirrored
+//   dhi, dlo 32 x 32 fp16 (SWIZZLE_64B): the operand split of TWO consecutive steps, stored as one box of 64-byte rows
+//   thi, tlo 16 x 32 fp16: the split of one step, transposed (mirrored copy)
+// The fp32 iterates are only kept up to date on and above the diagonal (no product reads the rest); the lower triangle
+// is restored when an iterate leaves the workspace (dmpt_symmetrize_kernel).
 constexpr int kEpiWarpBytes = 10240;
-constexpr int kEpiRing = 2048, kEpiT32 = 4096, kEpiDhi = 6144, kEpiDlo = 7168, kEpiThi = 8192, kEpiTlo = 9216;
+constexpr int kEpiRing = 2048, kEpiDhi = 4096, kEpiDlo = 6144, kEpiThi = 8192, kEpiTlo = 9216;
 template <int PASS> struct TmaEpilogue { static constexpr bool value = PASS == 0; };
 template <int PASS>
 constexpr int smem_bytes() {
@@ -105,8 +107,8 @@ enum Pos : int { PM_H = 0, PM_L = 1, PY_H = 2, PY_L = 3, PZ_H = 4, PZ_L = 5 };
 
 struct LayerParams {
     CUtensorMap maps[2][8];     // [buffer][Mhi, Mlo, S1hi, S1lo, S2hi, S2lo, S3hi, S3lo], box = kBK x kBRows, SWIZZLE_64B
-    // epilogue maps: [..][0] direct 16 x 32 box (fp32: SWIZZLE_64B, fp16: SWIZZLE_32B), [..][1] mirrored 32 x 16 box
-    CUtensorMap emap32[3][2];   // fp32 iterates S0, S1[0], S1[1]
+    // epilogue maps of the fp16 pairs: [..][0] direct 32 x 32 box (SWIZZLE_64B), [..][1] mirrored 32 x 16 box
+    CUtensorMap emap32[3];      // fp32 iterates S0, S1[0], S1[1]: 16 x 32 box, SWIZZLE_64B
     CUtensorMap emap16[2][2][2];  // fp16 operand PAIRS [buffer][(Mhi, Mlo), (S1hi, S1lo)]: 3D maps, the hi and the lo matrix
                                 // of a pair lie back to back in the workspace and are the two planes of one tensor, so
                                 // that one TMA store writes a block of both
@@ -157,7 +159,7 @@ struct EpiOut {
 };
 
 struct EpiTma {            // shared-memory addresses of this warp's staging
-    uint32_t ring[2], t32, dhi, dlo, thi, tlo, bar[2];
+    uint32_t ring[2], dhi, dlo, thi, tlo, bar[2];
 };
 
 template <int ORDER>
@@ -252,8 +254,10 @@ __device__ __forceinline__ void final_epilogue(float (&acc)[kHalfCols], const Ep
 // Final epilogue of one product on an OFF-DIAGONAL tile, through shared memory and TMA: the same arithmetic as
 // final_epilogue with w = 2, dg = 0 (so delta = -+unscale acc exactly and S <- fmaf(+-unscale, acc, old)), but
 //   * the old iterate comes by TMA into this warp's ring (issued one step ahead),
-//   * the new iterate and its split are written to shared memory in the direct and the transposed layout and
-//     leave by four TMA stores per 32 x 16 block (fp32 and the (hi, lo) pair; direct and mirrored): full lines instead of row-per-thread accesses,
+//   * the new iterate and its split are written to shared memory (the split also transposed) and leave by TMA stores:
+//     per 32 x 16 block the fp32 values and the mirrored (hi, lo) pair, per two blocks the direct (hi, lo) pair as
+//     one box of 64-byte rows - full lines instead of row-per-thread accesses, and as few, as wide TMA requests as
+//     the staging allows (the stores are bound by the TMA unit's request rate),
 //   * the split uses the packed conversions (cvt.rn.f16x2.f32).
 // step s (0 .. ns-1) of the tile handles product s / 4 (0: P0, 1: P1; when only one is live it is steps 0-3) and
 // columns (s & 3) * 16 of this thread's 64.
@@ -344,8 +348,6 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
                         const uint32_t lw = *reinterpret_cast<const uint32_t*>(&l2);
                         ph[(j >> 1) & 3] = hw;
                         pl[(j >> 1) & 3] = lw;
-                        sts32(et.t32 + (uint32_t)j * 128u + (uint32_t)lane * 4u, __float_as_uint(nn[0]));
-                        sts32(et.t32 + (uint32_t)(j + 1) * 128u + (uint32_t)lane * 4u, __float_as_uint(nn[1]));
                         sts16(et.thi + (uint32_t)j * 64u + (uint32_t)lane * 2u, (uint16_t)(hw & 0xFFFF));
                         sts16(et.thi + (uint32_t)(j + 1) * 64u + (uint32_t)lane * 2u, (uint16_t)(hw >> 16));
                         sts16(et.tlo + (uint32_t)j * 64u + (uint32_t)lane * 2u, (uint16_t)(lw & 0xFFFF));
@@ -375,12 +377,12 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
                         o.lo[g] = __ushort_as_half(lds16(et.dlo + b));
                     }
                 }
-                // mirrored copy, one row of 32 columns per instruction, where row < column of the original
+                // mirrored copy of the split (the fp32 iterate is kept on and above the diagonal only), one row of 32
+                // columns per instruction, where row < column of the original
 #pragma unroll 4
                 for (uint32_t j = 0; j < 16; ++j) {
                     if (gr < gc0 + (int)j) {
                         const size_t g = (size_t)(gc0 + (int)j) * ld + gr;
-                        o.dst[g] = lds32f(et.t32 + j * 128u + (uint32_t)lane * 4u);
                         o.hi[g] = __ushort_as_half(lds16(et.thi + j * 64u + (uint32_t)lane * 2u));
                         o.lo[g] = __ushort_as_half(lds16(et.tlo + j * 64u + (uint32_t)lane * 2u));
                     }
@@ -424,8 +426,6 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
                     ph[(j >> 1) & 3] = hw;
                     pl[(j >> 1) & 3] = lw;
                     // transposed: for a fixed column the 32 lanes write one row of the mirrored block
-                    sts32(et.t32 + (uint32_t)j * 128u + (uint32_t)lane * 4u, __float_as_uint(n0));
-                    sts32(et.t32 + (uint32_t)(j + 1) * 128u + (uint32_t)lane * 4u, __float_as_uint(n1));
                     sts16(et.thi + (uint32_t)j * 64u + (uint32_t)lane * 2u, (uint16_t)(hw & 0xFFFF));
                     sts16(et.thi + (uint32_t)(j + 1) * 64u + (uint32_t)lane * 2u, (uint16_t)(hw >> 16));
                     sts16(et.tlo + (uint32_t)j * 64u + (uint32_t)lane * 2u, (uint16_t)(lw & 0xFFFF));
@@ -433,8 +433,10 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
                 }
                 sts128(a32, __float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3]));   // in place
             }
-            sts128(et.dhi + row32 + (((uint32_t)q2 ^ sw32) << 4), ph[0], ph[1], ph[2], ph[3]);
-            sts128(et.dlo + row32 + (((uint32_t)q2 ^ sw32) << 4), pl[0], pl[1], pl[2], pl[3]);
+            // chunk (2 (sc & 1) + q2) of this thread's 64-byte row of the two-step direct box
+            const uint32_t ch = (((uint32_t)(2 * (sc & 1) + q2)) ^ sw64) << 4;
+            sts128(et.dhi + row64 + ch, ph[0], ph[1], ph[2], ph[3]);
+            sts128(et.dlo + row64 + ch, pl[0], pl[1], pl[2], pl[3]);
         }
         r_fs += (double)(2.f * f_fs);           // off-diagonal elements count twice
         r_fro += (double)(2.f * f_fro);
@@ -442,9 +444,8 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
         __syncwarp();
         if (lane == 0) {
             tma_store_2d(o.m_dst, et.ring[slot], gc0, gr0);
-            tma_store_2d(o.m_dst + 1, et.t32, gr0, gc0);
-            tma_store_3d(o.m_hl, et.dhi, gc0, gr0, 0);          // dhi, dlo: the two planes of the direct box
-            tma_store_3d(o.m_hl + 1, et.thi, gr0, gc0, 0);      // thi, tlo: of the mirrored box
+            tma_store_3d(o.m_hl + 1, et.thi, gr0, gc0, 0);      // thi, tlo: the two planes of the mirrored box
+            if (sc & 1) tma_store_3d(o.m_hl, et.dhi, gc0 - kSub, gr0, 0);      // dhi, dlo: 32 columns of two steps
             bulk_commit();
         }
     }
@@ -726,9 +727,9 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
             o0.hi = p.h[c.s0_buf ^ 1][MH]; o0.lo = p.h[c.s0_buf ^ 1][ML];
             o1.dst = p.s1[c.s1_buf ^ 1]; o1.old = p.s1[c.s1_buf];
             o1.hi = p.h[c.s1_buf ^ 1][S1H]; o1.lo = p.h[c.s1_buf ^ 1][S1L];
-            o0.m_old = o0.m_dst = &p.emap32[0][0];
+            o0.m_old = o0.m_dst = &p.emap32[0];
             o0.m_hl = &p.emap16[c.s0_buf ^ 1][0][0];
-            o1.m_old = &p.emap32[1 + c.s1_buf][0]; o1.m_dst = &p.emap32[1 + (c.s1_buf ^ 1)][0];
+            o1.m_old = &p.emap32[1 + c.s1_buf]; o1.m_dst = &p.emap32[1 + (c.s1_buf ^ 1)];
             o1.m_hl = &p.emap16[c.s1_buf ^ 1][1][0];
         } else if (PASS == 1) {
             o0.dst = nullptr; o0.old = nullptr; o0.hi = nullptr; o0.lo = nullptr;
@@ -754,7 +755,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         uint32_t ring_phase = 0;
         {
             const uint32_t eb = epi_base + (uint32_t)(warp - kEpiWarp0) * kEpiWarpBytes;
-            et.ring[0] = eb; et.ring[1] = eb + kEpiRing; et.t32 = eb + kEpiT32;
+            et.ring[0] = eb; et.ring[1] = eb + kEpiRing;
             et.dhi = eb + kEpiDhi; et.dlo = eb + kEpiDlo; et.thi = eb + kEpiThi; et.tlo = eb + kEpiTlo;
             et.bar[0] = ring_bar(warp - kEpiWarp0, 0); et.bar[1] = ring_bar(warp - kEpiWarp0, 1);
         }
