@@ -72,7 +72,8 @@ typedef struct dmpt_options {
                        /* D1_a for each in one run - S0^2 once per layer, S0.S1_a per field (the x, y, z       */
                        /* fields of the polarizability, Eq. 79).  Use the *_fields entry points.  */
     int epilogue_direct; /* 0 (default): the layer kernel's final epilogue goes through shared memory and TMA (old      */
-                       /* iterate in, new iterate and its split out, direct and mirrored, as full lines); 1: every  */
+                       /* iterate in, new iterate and its split out as full lines; the lower triangle of the fp32   */
+                       /* iterates is restored when they leave the workspace); 1: every                             */
                        /* thread reads and writes its own row of the tile directly (round 1's path, kept for A/B     */
                        /* measurements; same arithmetic, bit-identical results)                                      */
     int lanczos_steps; /* bounds == 2: number of Lanczos steps, 1..64; 0 = default (20)                          */
