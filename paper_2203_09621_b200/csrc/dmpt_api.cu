@@ -386,7 +386,7 @@ static int create_impl(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_w
     {
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(ctx->num_sms & ~1);
-        cfg.blockDim = dim3(kNumThreads);
+        cfg.blockDim = dim3(Warps<1>::kThreads);
         cfg.dynamicSmemBytes = smem_bytes<1>();
         CKC(cudaOccupancyMaxActiveClusters(&max_clusters, dmpt_layer_kernel<1>, &cfg));
     }
@@ -477,7 +477,7 @@ static int launch_pass(dmpt_ctx* ctx, cudaStream_t capture = nullptr) {
     // a cooperative launch guarantees it or fails
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(ctx->grid_layer);
-    cfg.blockDim = dim3(kNumThreads);
+    cfg.blockDim = dim3(Warps<PASS>::kThreads);
     cfg.dynamicSmemBytes = smem_bytes<PASS>();
     cfg.stream = capture ? capture : ctx->stream;
     cudaLaunchAttribute attr[2];

@@ -33,9 +33,11 @@
 // CTA pairs: a cluster of two CTAs (one TPC) shares a 256 x 128 pair tile through
 // tcgen05.mma.cta_group::2 (see the comment on the kernel).
 //
-// Warp roles (per CTA, three warpgroups): warp 0 TMA producer, warp 1 MMA issuer (leader CTA, one elected lane) and
-// TMEM owner, warps 2-3 idle (they only hand their registers over), warps 4-11 epilogue: warp w owns TMEM lane
-// quadrant w % 4 and column half (w - 4) / 4 of both accumulators (64 + 64 fp32 registers per thread).  TMEM holds two accumulator stages
+// Warp roles (per CTA): warp 0 TMA producer, warp 1 MMA issuer (leader CTA, one elected lane) and TMEM owner, then the
+// eight epilogue warps: epilogue warp e owns TMEM lane quadrant (its warp index) % 4 and column half e / 4 of both
+// accumulators (64 + 64 fp32 registers per thread).  The order-2, order-3 and A.B^T passes have two more warps between
+// them that only hand their registers over (setmaxnreg, three warpgroups); PASS 0 and PASS 2 measured faster without
+// (Warps<PASS>).  TMEM holds two accumulator stages
 // (2 x [P0 | P1] x 128 columns): the drain of chunk c overlaps the MMAs of chunk c + 1.
 //
 // Orders: PASS 0 of the kernel does orders 0 and 1 (order 0 alone when the context was created
@@ -76,14 +78,18 @@ constexpr int kKbPerChunk = kChunkK / kBK;
 constexpr int kAccStages = 2;
 constexpr int kRedStride = 2048;           // per-warp partials are stored [component][slot], slot < gridDim.x * 8 <= 2048
 constexpr int kTmemCols = 512;
-constexpr int kEpiWarp0 = 4;               // warpgroup 0: TMA producer, MMA issuer, two idle warps; warpgroups 1, 2: epilogue
 constexpr int kNumEpiWarps = 8;
-constexpr int kNumThreads = 32 * (kEpiWarp0 + kNumEpiWarps);   // 384
 // Registers: 384 threads x 168 at launch.  Where kSetMaxNReg says so, warpgroup 0 then gives registers back
 // (setmaxnreg.dec) and the two epilogue warpgroups, which hold 2 x 64 fp32 accumulators per thread, grow to 176
 // (152 + 2 x 176 = 504 <= 512 registers per lane of a scheduler)
 constexpr int kRegsLight = 152, kRegsEpi = 176;
 template <int PASS> struct kSetMaxNReg { static constexpr bool value = PASS == 1 || PASS == 3 || PASS == 4; };
+// Warps of a CTA: TMA producer, MMA issuer, [two idle warps that only exist to hand their registers over: with setmaxnreg
+// a warpgroup of four], then the eight epilogue warps.  PASS 0 and PASS 2: 10 warps (320 threads); the others: 12 (384).
+template <int PASS> struct Warps {
+    static constexpr int kEpi0 = kSetMaxNReg<PASS>::value ? 4 : 2;         // first epilogue warp
+    static constexpr int kThreads = 32 * (kEpi0 + kNumEpiWarps);
+};
 constexpr int kHalfCols = kTile / 2;       // accumulator columns per epilogue thread and product
 constexpr int kSub = 16;                   // columns per step of the final epilogue
 // Final epilogue through shared memory and TMA (PASS 0).  Each epilogue warp owns 10 KiB:
@@ -469,10 +475,12 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
 //         reads the operands of S0_{n-1}, S1_{n-1}, S2_{n-1} and the decision pass 0 of layer n-1 left in
 //         DmptCtl, writes S2_n into the other buffer and leaves ||V2||_F^2, max|S2_n| in partials2.
 template <int PASS>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kNumThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Warps<PASS>::kThreads, 1)
 dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     constexpr int kOps = PassCfg<PASS>::kOps;
     constexpr int kStages = PassCfg<PASS>::kStages;
+    constexpr int kEpiWarp0 = Warps<PASS>::kEpi0;
+    constexpr int kNumThreads = Warps<PASS>::kThreads;
     constexpr int kStageBytes = kOps * (kABytes + kBBytes);
     constexpr int kBOff = kOps * kABytes;          // B tiles follow the A tiles inside a stage
     // Layer launches that do not need the wave barrier are chained by programmatic dependent launch: the next launch
