@@ -246,7 +246,8 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
             CUresult r = encode(&ctx->lp.maps[b][m], CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
                                 ctx->at<void>(L.h[b][m]), dims, strides, box, estr,
                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
-                                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                // 256-byte promotion: measured 30.73 -> 30.58 ms per layer at N = 16384 against 128 B
+                                CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) {
                 snprintf(ctx->err, sizeof ctx->err, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
                 return DMPT_ECUDA;
