@@ -44,6 +44,7 @@ extern "C" {
 #define DMPT_ENOCONV      -5   /* max_layers reached; outputs hold the last iterate                   */
 #define DMPT_ENUMERIC     -6   /* NaN/Inf in the scalar state, or fp16 overflow of a scaled iterate   */
 #define DMPT_EWORKSPACE   -7   /* workspace too small or misaligned                                   */
+#define DMPT_ELIMIT       -8   /* size beyond a compiled-in limit (DMPT_NOALLOC_MAX_N)                */
 
 typedef struct dmpt_ctx dmpt_ctx;
 
@@ -273,6 +274,22 @@ int dmpt_pair_set_hamiltonian(dmpt_pair *pair, const float *d_h0, const float *d
 int dmpt_pair_run(dmpt_pair *pair, float *d_d0, float *d_d1, int ld, dmpt_result *res);
 int dmpt_pair_destroy(dmpt_pair *pair);
 const char *dmpt_pair_last_cuda_error(const dmpt_pair *pair);
+
+/* Step a1 for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc).  The Gershgorin discs of d_h0 (device, n x n, row-major, leading dimension ld >= n)
+ * -> d_eps[0] = eps_min, d_eps[1] = eps_max (DEVICE, two doubles, caller-owned), in the arithmetic of
+ * dmpt_spectral_bounds.  No context is needed; the call allocates nothing on the device or the host (no cudaMalloc,
+ * cudaFree, cudaHostAlloc, no allocating library routine): its scratch - the disc ends of every row and one counter
+ * - is a static device array of 256 + 16 DMPT_NOALLOC_MAX_N bytes (1 MiB) inside the library, held by every GPU
+ * that loads libdmpt.so until the process exits.  The call enqueues one memset and one kernel on `cuda_stream`
+ * (a cudaStream_t of the CURRENT device, which must also hold d_h0 and d_eps; NULL = the default stream) and returns
+ * without waiting: d_eps is valid once the stream has reached that point.
+ *   n > DMPT_NOALLOC_MAX_N -> DMPT_ELIMIT ("size beyond a compiled-in limit"), nothing enqueued; null pointers,
+ *   n <= 0, ld < n -> DMPT_EINVAL; a failed launch -> DMPT_ECUDA.
+ * All calls on one device share the scratch, which keeps the last call's contents: calls ordered on one stream (or
+ * by events) are safe, calls that overlap on the GPU race on it and their results are undefined. */
+#define DMPT_NOALLOC_MAX_N 65536
+int dmpt_spectral_bounds_noalloc(const float *d_h0, int n, int ld, double *d_eps, void *cuda_stream);
 
 const char *dmpt_strerror(int code);
 /* Text of the last CUDA error seen by this context (empty string if none). */

@@ -21,6 +21,8 @@ from .binding import (  # noqa: F401
     dmpt_run_host,
     dmpt_set_hamiltonian,
     dmpt_spectral_bounds,
+    dmpt_spectral_bounds_noalloc,
+    spectral_bounds_noalloc,
     dmpt_initial_transform,
     dmpt_split,
     dmpt_strerror,

@@ -21,10 +21,13 @@ EXPORTED_SYMBOLS = (
     "dmpt_run_fields_host",
     "dmpt_pair_workspace_bytes", "dmpt_pair_create", "dmpt_pair_set_hamiltonian", "dmpt_pair_run", "dmpt_pair_destroy",
     "dmpt_pair_last_cuda_error",
+    "dmpt_spectral_bounds_noalloc",
 )
 
 DMPT_OK, DMPT_EINVAL, DMPT_ESTATE, DMPT_ECUDA = 0, -1, -2, -3
 DMPT_EDEGENERATE, DMPT_ENOCONV, DMPT_ENUMERIC, DMPT_EWORKSPACE = -4, -5, -6, -7
+DMPT_ELIMIT = -8
+DMPT_NOALLOC_MAX_N = 65536
 
 
 class DmptOptions(C.Structure):
@@ -92,6 +95,8 @@ def lib():
         L.dmpt_run_fields_host.restype = C.c_int
         L.dmpt_congruence.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
         L.dmpt_congruence.restype = C.c_int
+        L.dmpt_spectral_bounds_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.dmpt_spectral_bounds_noalloc.restype = C.c_int
         L.dmpt_fd_response.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_int,
                                        C.c_void_p, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.dmpt_fd_response.restype = C.c_int
@@ -295,6 +300,31 @@ def dmpt_spectral_bounds(ctx, h0_ptr, ld):
     lo, hi = C.c_double(), C.c_double()
     rc = int(lib().dmpt_spectral_bounds(ctx, C.c_void_p(h0_ptr), int(ld), C.byref(lo), C.byref(hi)))
     return rc, lo.value, hi.value
+
+
+def dmpt_spectral_bounds_noalloc(h0_ptr, n, ld, eps_ptr, stream=0) -> int:
+    """Context-free a1 with static scratch (include/dmpt.h): device pointers in, two device doubles out, stream-ordered."""
+    return int(lib().dmpt_spectral_bounds_noalloc(C.c_void_p(h0_ptr), int(n), int(ld), C.c_void_p(eps_ptr),
+                                                  C.c_void_p(stream)))
+
+
+def spectral_bounds_noalloc(h0, out, stream=None):
+    """Gershgorin bounds of the CUDA fp32 matrix `h0` into `out` (CUDA float64, two elements: eps_min, eps_max), enqueued
+    on `stream` (torch stream; default: the current one) with no allocation on either side.  `out` is returned; it is
+    valid once the stream has reached this point.  n > DMPT_NOALLOC_MAX_N raises DmptError(DMPT_ELIMIT)."""
+    import torch
+
+    if h0.dim() != 2 or h0.shape[0] != h0.shape[1] or h0.dtype != torch.float32 or h0.stride(1) != 1 or not h0.is_cuda:
+        raise ValueError("h0: a square CUDA fp32 matrix with unit column stride is required")
+    if out.dtype != torch.float64 or out.numel() < 2 or not out.is_contiguous() or out.device != h0.device:
+        raise ValueError("out: two contiguous float64 elements on h0's device are required")
+    with torch.cuda.device(h0.device):
+        st = stream if stream is not None else torch.cuda.current_stream()
+        rc = dmpt_spectral_bounds_noalloc(h0.data_ptr(), h0.shape[0], h0.stride(0) if h0.shape[0] > 1 else 1,
+                                          out.data_ptr(), st.cuda_stream)
+    if rc != DMPT_OK:
+        raise DmptError(rc, "dmpt_spectral_bounds_noalloc")
+    return out
 
 
 def dmpt_initial_transform(ctx, h0_ptr, h1_ptr, ld, eps_min, eps_max, s0_ptr, s1_ptr, ld_out):

@@ -1,4 +1,4 @@
-"""Build step: compile csrc/dmpt_api.cu into libdmpt.so (in-tree) with nvcc for sm_100a.
+"""Build step: compile csrc/dmpt_api.cu and csrc/noalloc.cu into libdmpt.so (in-tree) with nvcc for sm_100a.
 
 nvcc cross-compiles without a GPU.  Usage: `python -m paper_2203_09621_b200.build [--force]`.
 """
@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdmpt.so")
-SOURCES = ["dmpt_api.cu"]
+SOURCES = ["dmpt_api.cu", "noalloc.cu"]
 HEADERS = ["ptx.cuh", "control.cuh", "kernels_hbm.cuh", "layer_kernel.cuh",
            os.path.join("..", "..", "include", "dmpt.h")]
 NVCC_FLAGS = [

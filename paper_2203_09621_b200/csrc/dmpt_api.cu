@@ -219,6 +219,7 @@ extern "C" const char* dmpt_strerror(int code) {
         case DMPT_ENOCONV: return "max_layers reached before the stopping tests fired";
         case DMPT_ENUMERIC: return "NaN/Inf in the scalar state";
         case DMPT_EWORKSPACE: return "workspace too small or not 256-byte aligned";
+        case DMPT_ELIMIT: return "size beyond a compiled-in limit (n > DMPT_NOALLOC_MAX_N of the no-allocation entry point)";
         default: return "unknown error code";
     }
 }
