@@ -310,11 +310,13 @@ def run_ours(args):
     ev0.record()
     flops = fma = ms_loop = 0.0
     launches = layers_total = 0
+    dev_mhz = []
     for _ in range(args.steps):
         res, fl, fx = one_run()
         flops += fl
         fma += fx
         ms_loop += res.ms_loop
+        dev_mhz.append(getattr(res, "sm_clock_mhz", 0.0))
         launches += res.launches
         layers_total += res.layers
     ev1.record()
@@ -366,6 +368,16 @@ def run_ours(args):
         peak_tf = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
         layer_ms = ms_loop / max(1, layers_total)
         achieved_tf = 2.0 * fma / (ms_loop * 1e-3) / 1e12
+        # the SM clock of the layer loop from the device's own counters (dmpt_result.sm_clock_mhz): under the power cap
+        # it lies below what nvidia-smi samples show; the tensor peak AT that clock is what the kernel can be held to
+        dev_mhz = [m for m in dev_mhz if m > 0.0]
+        sm_mhz_device = sum(dev_mhz) / len(dev_mhz) if dev_mhz else None
+        if clocks is not None:
+            clocks["sm_mhz_device"] = sm_mhz_device
+            clocks["sm_mhz_device_note"] = ("SM cycle counters over the device nanosecond timer across the layer loop, "
+                                            "all SMs (dmpt_result.sm_clock_mhz); sm_mhz is nvidia-smi's sample")
+        n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_at_clock = n_sm * 4096 * sm_mhz_device * 1e6 / 1e12 if sm_mhz_device else None      # T-FMA/s, fp16 dense
         # the oracle as it stands on THIS workload: 3 layers at the bench N when that is about
         # 1-3 min of host time, the whole run when it is shorter; per-layer seconds and the time-to-D1 extrapolated
         # with O3's layer count.  A second, smaller sample (n = 4096 generator, 20 layers) keeps round 1's key.
@@ -404,7 +416,11 @@ def run_ours(args):
                          "traffic_source": traffic_src,
                          "peak_kind": f"bf16_tflops_sustained, {peaks_kind} (fp16 = bf16 rate), 2 flops per FMA",
                          "avg_launch_ms": layer_ms, "executed_tfma_per_s": achieved_tf / 2.0,
-                         "frac_nominal_1125_tfma": achieved_tf / 2.0 / NOMINAL_FP16_TFMA},
+                         "frac_nominal_1125_tfma": achieved_tf / 2.0 / NOMINAL_FP16_TFMA,
+                         "tfma_peak_at_device_clock": peak_at_clock,
+                         "frac_of_peak_at_device_clock": (achieved_tf / 2.0 / peak_at_clock) if peak_at_clock else None,
+                         "device_clock_note": "4096 dense fp16 FMA per SM and clock x SMs x clocks.sm_mhz_device: "
+                                              "what is left of the nominal peak at the clock the 1 kW cap allows"},
             "cpu_baseline": dict({"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": cpu_dt,
                                   "sample": f"oracle.dnn_sp2_pt (fp64) on the bench workload itself (config {args.config}, "
                                             f"n={ref_n}), first {cpu_layers} layers incl. bounds and transform",

@@ -107,7 +107,9 @@ typedef struct dmpt_result {
     double ms_bounds;          /* a1: Gershgorin kernel, which also takes max|H1| (+ scalar set-up)      */
     double ms_transform;       /* a2 + a3 fused: S0, S1 and their first operand split (+ first decision) */
     double ms_split;           /* what follows it before the loop (order 2: S2_0 = 0 and its first scale) */
-    double reserved_d[1];
+    double sm_clock_mhz;       /* SM clock of the layer loop, MHz: SM cycle counters over the device's nanosecond */
+                               /* timer between the first and the last layer launch, all SMs; 0 if fewer than two  */
+                               /* layers ran.  Under a power cap it lies below what nvidia-smi samples report.      */
     /* Per-layer records, entry n-1 for layer n.  Caller-allocated HOST arrays of max_layers
      * entries each, or NULL to skip.  Entries the run did not reach are left untouched. */
     int8_t *sigma;             /* sigma_n                                         */

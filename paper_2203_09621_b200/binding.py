@@ -47,7 +47,7 @@ class _CResult(C.Structure):
         ("launches", C.c_int), ("layers_d2", C.c_int), ("layers_d3", C.c_int), ("reserved_i", C.c_int * 1),
         ("eps_min", C.c_double), ("eps_max", C.c_double), ("fro_err0", C.c_double),
         ("ms_total", C.c_double), ("ms_loop", C.c_double), ("ms_bounds", C.c_double),
-        ("ms_transform", C.c_double), ("ms_split", C.c_double), ("reserved_d", C.c_double * 1),
+        ("ms_transform", C.c_double), ("ms_split", C.c_double), ("sm_clock_mhz", C.c_double),
         ("sigma", C.POINTER(C.c_int8)), ("tr_s", C.POINTER(C.c_double)), ("tr_x", C.POINTER(C.c_double)),
         ("id_err", C.POINTER(C.c_double)), ("fro_err1", C.POINTER(C.c_double)),
         ("fro_err2", C.POINTER(C.c_double)), ("fro_err3", C.POINTER(C.c_double)),
@@ -360,6 +360,7 @@ class DmptResult:
     ms_bounds: float = 0.0
     ms_transform: float = 0.0
     ms_split: float = 0.0
+    sm_clock_mhz: float = 0.0     # SM clock of the layer loop from the device's own counters (include/dmpt.h)
     layers_d2: int = 0
     sigma: list = field(default_factory=list)
     tr_s: list = field(default_factory=list)
@@ -453,7 +454,7 @@ class Dmpt:
         return DmptResult(status=rc, layers=r.layers, layers_d0=r.layers_d0, layers_d1=r.layers_d1,
                           launches=r.launches, eps_min=r.eps_min, eps_max=r.eps_max, fro_err0=r.fro_err0,
                           ms_total=r.ms_total, ms_loop=r.ms_loop, ms_bounds=r.ms_bounds,
-                          ms_transform=r.ms_transform, ms_split=r.ms_split,
+                          ms_transform=r.ms_transform, ms_split=r.ms_split, sm_clock_mhz=r.sm_clock_mhz,
                           sigma=list(bufs["sigma"][:nl]), tr_s=list(bufs["tr_s"][:nl]),
                           tr_x=list(bufs["tr_x"][:nl]), id_err=list(bufs["id_err"][:nl]),
                           fro_err1=list(bufs["fro_err1"][:nl]),

@@ -78,6 +78,16 @@ struct DmptLogs {   // device arrays, max_layers entries, entry n-1 for layer n
     double* fro1;
     double* fro2;
     double* fro3;
+    struct DmptClockStamps* clk;     // SM clock stamps of the layer launches (may be null)
+};
+
+// (clock64, globaltimer) of every SM at the start of the first and of the latest order-0 launch of a run: their
+// difference is the SM clock the layer loop really ran at (dmpt_result.sm_clock_mhz).  Under the power cap it is
+// well below what nvidia-smi samples show.
+constexpr int kMaxSmStamps = 256;
+struct DmptClockStamps {
+    long long first[kMaxSmStamps][2];
+    long long last[kMaxSmStamps][2];
 };
 
 struct DmptProblem {

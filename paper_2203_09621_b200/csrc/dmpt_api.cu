@@ -41,7 +41,7 @@ struct Layout {
         tiles, tiles_full;
     size_t s0, s1[2], s2[2], s3[2];
     size_t h[2][8];          // [buffer][S0hi, S0lo, S1hi, S1lo, slot-2 hi, lo, slot-3 hi, lo]
-    size_t stage_h0, stage_h1, stage_hx[2], lanczos;
+    size_t stage_h0, stage_h1, stage_hx[2], lanczos, clk;
     size_t total;
 };
 
@@ -81,6 +81,7 @@ Layout make_layout(int n, int order, int nfields) {
     L.partials3 = c.take(kPartialDoubles * sizeof(double));
     L.handoff = c.take((kMaxLayersCap + 2) * sizeof(DmptHandoff));
     L.lanczos = c.take(sizeof(LanczosState) + 3 * (size_t)L.n_pad * sizeof(double));
+    L.clk = c.take(sizeof(DmptClockStamps));
     L.tiles = c.take((size_t)L.num_tiles * sizeof(uint32_t));
     L.tiles_full = c.take((size_t)(nb / 2) * nb * sizeof(uint32_t));
     L.s0 = c.take(np2 * 4);
@@ -426,6 +427,7 @@ static int create_impl(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_w
     lp.logs.fro1 = ctx->at<double>(L.fro1);
     lp.logs.fro2 = ctx->at<double>(L.fro2);
     lp.logs.fro3 = ctx->at<double>(L.fro3);
+    lp.logs.clk = ctx->at<DmptClockStamps>(L.clk);
     lp.partials = ctx->at<double>(L.partials);
     lp.partials2 = ctx->at<double>(L.partials2);
     lp.partials3 = ctx->at<double>(L.partials3);
@@ -816,7 +818,19 @@ static int finish(dmpt_ctx* ctx, dmpt_result* res, int launches) {
         res->ms_transform = ms;
         CK(cudaEventElapsedTime(&ms, ctx->ev_t[5], ctx->ev_t[1]));
         res->ms_split = ms;
+        res->sm_clock_mhz = 0.0;
         const int nl = c.layers;
+        if (nl > 1) {       // SM cycles over device nanoseconds between the first and the last layer launch, all SMs
+            std::vector<DmptClockStamps> cs(1);
+            CK(cudaMemcpy(cs.data(), ctx->at<DmptClockStamps>(L.clk), sizeof(DmptClockStamps), cudaMemcpyDeviceToHost));
+            double cyc = 0.0, ns = 0.0;
+            for (int i = 0; i < kMaxSmStamps; ++i)
+                if (cs[0].first[i][1] > 0 && cs[0].last[i][1] > cs[0].first[i][1]) {
+                    cyc += (double)(cs[0].last[i][0] - cs[0].first[i][0]);
+                    ns += (double)(cs[0].last[i][1] - cs[0].first[i][1]);
+                }
+            if (ns > 0.0) res->sm_clock_mhz = 1e3 * cyc / ns;
+        }
         if (nl > 0) {
             std::vector<int> sg(nl);
             if (res->sigma) {
@@ -1744,6 +1758,7 @@ extern "C" int dmpt_pair_run(dmpt_pair* pr, float* d_d0, float* d_d1, int ld, dm
         PK(cudaEventElapsedTime(&ms, c1->ev_t[4], c1->ev_t[5]));
         res->ms_transform = ms;
         res->ms_split = 0.0;
+        res->sm_clock_mhz = 0.0;      // two devices, two clocks: not reported for the pair
         const int nl = k1.layers, nl0 = k0.layers < nl ? k0.layers : nl;
         if (nl > 0) {
             std::vector<int> sg(nl);

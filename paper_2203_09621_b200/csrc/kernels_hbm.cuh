@@ -713,6 +713,9 @@ __global__ void dmpt_bounds_to_ctl_kernel(const long long* __restrict__ bounds, 
 __global__ void dmpt_control_init_kernel(DmptCtl* ctl, DmptLogs logs, DmptProblem pb,
                                          const double* __restrict__ partials, int nblocks, DmptHandoff* handoff) {
     if (blockIdx.x || threadIdx.x >= 32) return;
+    if (logs.clk)
+        for (int i = threadIdx.x; i < kMaxSmStamps; i += 32)
+            logs.clk->first[i][0] = logs.clk->first[i][1] = logs.clk->last[i][0] = logs.clk->last[i][1] = 0;
     double t = 0.0, f = 0.0;
     for (int b = threadIdx.x; b < nblocks; b += 32) {
         t += partials[b * 3 + 0];

@@ -446,6 +446,10 @@ def test_runs_are_deterministic_and_wave_sync_does_not_change_results(dev):
     a = _run(wl, dev, wave_sync=True)
     b = _run(wl, dev, wave_sync=False)
     assert a[0].layers == b[0].layers and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    # the SM clock the layer loop ran at, from the device's own counters (dmpt_result.sm_clock_mhz): a plausible clock,
+    # on every run (the stamps are cleared at the start of each)
+    for r in (a[0], b[0]):
+        assert 300.0 < r.sm_clock_mhz < 2600.0, r.sm_clock_mhz
 
 
 def test_run_host_equals_run(dev, config1):
@@ -905,6 +909,7 @@ def test_bench_line_has_the_contract_keys(dev):
     assert d["gpu_launches"] > 0 and d["data"] == "synthetic" and "workload" in d["config"]
     rf = d["roofline"]
     assert rf["bound"] == "tensor" and rf["unit"] == "TFLOP/s" and abs(rf["frac"] - rf["achieved"] / rf["peak"]) < 1e-9
+    assert 300.0 < d["clocks"]["sm_mhz_device"] < 2600.0 and 0.0 < rf["frac_of_peak_at_device_clock"] < 1.0
     e = d["e2e"]
     assert e["value"] > 0 and e["h2d_bytes_per_step"] == 2 * 256 * 256 * 4 and e["d2h_bytes_per_step"] == 2 * 256 * 256 * 4
     cb = d["cpu_baseline"]
