@@ -47,6 +47,32 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback"
 
 
+def library_gemm_sustained(dev, dtype, seconds=3.0, m=8192):
+    """Context for the roofline line, not its denominator: the library GEMM (torch.matmul = cuBLAS) of the layer
+    kernel's OPERAND dtype, m^3, back to back for `seconds` under the same power cap, TFLOP/s at 2 flops per FMA.
+    MEASURED_PEAKS.json holds the bf16 figure; fp16 operands cost more energy per product than bf16's."""
+    import torch
+
+    a = torch.randn((m, m), device=dev, dtype=torch.float32).to(dtype)
+    b = torch.randn((m, m), device=dev, dtype=torch.float32).to(dtype)
+    c = torch.empty((m, m), device=dev, dtype=dtype)
+    for _ in range(20):
+        torch.matmul(a, b, out=c)
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps, batch = 0, 50
+    t0 = time.perf_counter()
+    e0.record()
+    while time.perf_counter() - t0 < seconds:
+        for _ in range(batch):
+            torch.matmul(a, b, out=c)
+        torch.cuda.synchronize(dev)
+        reps += batch
+    e1.record()
+    torch.cuda.synchronize(dev)
+    return 2.0 * m ** 3 * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12
+
+
 class ClockSampler:
     """nvidia-smi clocks/throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -376,6 +402,9 @@ def run_ours(args):
             clocks["sm_mhz_device"] = sm_mhz_device
             clocks["sm_mhz_device_note"] = ("SM cycle counters over the device nanosecond timer across the layer loop, "
                                             "all SMs (dmpt_result.sm_clock_mhz); sm_mhz is nvidia-smi's sample")
+        lib_tf = None
+        if n >= 8192 and nf == 1 and order == 1:            # the sizes the power cap governs
+            lib_tf = library_gemm_sustained(dev, torch.float16)
         n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
         peak_at_clock = n_sm * 4096 * sm_mhz_device * 1e6 / 1e12 if sm_mhz_device else None      # T-FMA/s, fp16 dense
         # the oracle as it stands on THIS workload: 3 layers at the bench N when that is about
@@ -417,6 +446,12 @@ def run_ours(args):
                          "peak_kind": f"bf16_tflops_sustained, {peaks_kind} (fp16 = bf16 rate), 2 flops per FMA",
                          "avg_launch_ms": layer_ms, "executed_tfma_per_s": achieved_tf / 2.0,
                          "frac_nominal_1125_tfma": achieved_tf / 2.0 / NOMINAL_FP16_TFMA,
+                         "library_fp16_gemm_sustained": ({"tflops": lib_tf, "frac": achieved_tf / lib_tf,
+                                                          "what": "torch.matmul fp16 8192^3 (cuBLAS) back to back for "
+                                                                  "3 s on this GPU, after the timed region: the "
+                                                                  "library GEMM of the kernel's operand dtype under "
+                                                                  "the same cap; context, not the denominator"}
+                                                         if lib_tf else None),
                          "tfma_peak_at_device_clock": peak_at_clock,
                          "frac_of_peak_at_device_clock": (achieved_tf / 2.0 / peak_at_clock) if peak_at_clock else None,
                          "device_clock_note": "4096 dense fp16 FMA per SM and clock x SMs x clocks.sm_mhz_device: "
