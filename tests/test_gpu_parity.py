@@ -314,6 +314,25 @@ def test_reduced_configs_match_oracle(dev, cfg, n):
     _check_scalars(res, ref, (d0, d1))
 
 
+@pytest.mark.parametrize("cfg,n,seed", [(1, 384, 11), (2, 640, 12), (3, 768, 13), (4, 896, 14), (4, 1280, 15), (2, 1028, 16)])
+def test_other_seeds_of_the_generators_match_oracle(dev, cfg, n, seed):
+    """The tolerances are not tuned to one draw: other seeds of every generator (another H0, another H1, the same
+    construction), sizes between the ones above, against O2 with the same checks."""
+    from oracle.dnn_sp2_pt import dnn_sp2_pt
+    from workloads import make_config
+
+    wl = make_config(cfg, n=n, seed=seed)
+    ref = dnn_sp2_pt(wl.h0, wl.h1, wl.n_occ)
+    assert ref.status == "ok"
+    res, d0, d1 = _run(wl, dev)
+    assert res.status == 0
+    _check_against(ref.d0, ref.d1, wl.n_occ, d0, d1)
+    ref_dh = _o2dh(wl)
+    _check_layer_count(res, ref_dh, ref)
+    _check_layer_count(res, ref_dh, ref, "layers_d0")
+    _check_scalars(res, ref, (d0, d1))
+
+
 @pytest.mark.parametrize("n,order", [(2, 1), (3, 1), (5, 2), (17, 1), (17, 2), (255, 1), (257, 2)])
 def test_smallest_and_off_by_one_sizes(dev, n, order):
     """Degenerate sizes: a 2 x 2 problem (one occupied level), sizes far below one tile, and one row either
