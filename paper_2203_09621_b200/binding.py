@@ -37,7 +37,7 @@ class DmptOptions(C.Structure):
         ("eps_min", C.c_double), ("eps_max", C.c_double),
         ("wave_sync", C.c_int), ("num_fields", C.c_int), ("epilogue_direct", C.c_int), ("lanczos_steps", C.c_int),
         ("no_pdl", C.c_int), ("loop_graph", C.c_int),
-        ("reserved", C.c_int * 2),
+        ("order0_narrow", C.c_int), ("reserved", C.c_int * 1),
     ]
 
 
@@ -381,7 +381,7 @@ class Dmpt:
 
     def __init__(self, n, order=1, max_layers=200, s0_shift=-1, s1_autoscale=True, bounds=None,
                  device="cuda:0", stream=None, wave_sync=True, num_fields=1, epilogue_direct=False, lanczos_steps=0,
-                 pdl=True, loop_graph=False):
+                 pdl=True, loop_graph=False, order0_narrow=False):
         import torch
 
         self.torch = torch
@@ -400,6 +400,7 @@ class Dmpt:
         opt.epilogue_direct = 1 if epilogue_direct else 0
         opt.no_pdl = 0 if pdl else 1
         opt.loop_graph = 1 if loop_graph else 0
+        opt.order0_narrow = 1 if order0_narrow else 0
         self.num_fields = int(num_fields)
         if isinstance(bounds, str):
             if bounds != "lanczos":

@@ -255,6 +255,21 @@ static int build_tensor_maps(dmpt_ctx* ctx) {
                 return DMPT_ECUDA;
             }
         }
+    // order-0 contexts: the same two operand matrices again as 128-byte rows (64 columns, SWIZZLE_128B) in the unused
+    // slots S3H, S3L, for the ground-state instantiation of pass 0 (dmpt_layer_kernel<0, true>)
+    if (L.order == 0)
+        for (int b = 0; b < 2; ++b)
+            for (int m = 0; m < 2; ++m) {
+                const cuuint32_t wbox[2] = {(cuuint32_t)(2 * kBK), (cuuint32_t)kBRows};
+                CUresult r = encode(&ctx->lp.maps[b][S3H + m], CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
+                                    ctx->at<void>(L.h[b][m]), dims, strides, wbox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                if (r != CUDA_SUCCESS) {
+                    snprintf(ctx->err, sizeof ctx->err, "cuTensorMapEncodeTiled (wide map) failed with CUresult %d", (int)r);
+                    return DMPT_ECUDA;
+                }
+            }
     // epilogue maps of the layer kernel's TMA path (layer_kernel.cuh, final_epilogue_tma).  fp32 iterates: a 16 x 32 box,
     // swizzled so that one thread per row reads and writes it without bank conflicts
     void* f32[3] = {ctx->at<void>(L.s0), ctx->at<void>(L.s1[0]), ctx->at<void>(L.s1[1])};
@@ -367,6 +382,7 @@ static int create_impl(dmpt_ctx** out, int n, const dmpt_options* opt, void* d_w
     CKC(cudaEventCreateWithFlags(&ctx->ev_side, cudaEventDisableTiming));
     CKC(cudaHostAlloc(&ctx->h_ctl, sizeof(DmptCtl), cudaHostAllocDefault));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<0>()));
+    CKC(cudaFuncSetAttribute(dmpt_layer_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<0>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<1>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<2>()));
     CKC(cudaFuncSetAttribute(dmpt_layer_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes<3>()));
@@ -492,7 +508,10 @@ static int launch_pass(dmpt_ctx* ctx, cudaStream_t capture = nullptr) {
     attr[1].val.programmaticStreamSerializationAllowed = (ctx->lp.wave_sync || ctx->opt.no_pdl || capture) ? 0 : 1;
     cfg.attrs = attr;
     cfg.numAttrs = 2;
-    CK(cudaLaunchKernelEx(&cfg, dmpt_layer_kernel<PASS>, ctx->lp));
+    if (PASS == 0 && ctx->opt.order == 0 && ctx->lp.pb.pair_side == 0 && !ctx->opt.order0_narrow)
+        CK(cudaLaunchKernelEx(&cfg, dmpt_layer_kernel<0, true>, ctx->lp));      // ground state: 128-byte operand rows
+    else
+        CK(cudaLaunchKernelEx(&cfg, dmpt_layer_kernel<PASS>, ctx->lp));
     return DMPT_OK;
 }
 

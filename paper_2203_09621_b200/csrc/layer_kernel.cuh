@@ -474,10 +474,21 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
 //         scale 2^(a + e2)), combined in fp32 in the epilogue.  Launched BEFORE pass 0 of the same layer: it
 //         reads the operands of S0_{n-1}, S1_{n-1}, S2_{n-1} and the decision pass 0 of layer n-1 left in
 //         DmptCtl, writes S2_n into the other buffer and leaves ||V2||_F^2, max|S2_n| in partials2.
-template <int PASS>
+// WIDE (PASS 0 at order 0 only): the ground-state instantiation.  It stages the two operands of M.M only, in k-blocks
+// of 64 columns - 128-byte operand rows, SWIZZLE_128B, through the tensor maps in slots S3H, S3L - in the same 48 KiB
+// per stage: half the TMA requests per byte.  With 64-byte rows order 0 asks the request path (one request per
+// operand row) for 1.5 x what first order does per MMA and the MMAs wait for it (item 6).  Same k16
+// steps in the same order: bit-identical results.
+template <int PASS, bool WIDE = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Warps<PASS>::kThreads, 1)
 dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
-    constexpr int kOps = PassCfg<PASS>::kOps;
+    static_assert(!WIDE || PASS == 0, "the wide k-block is the order-0 instantiation of pass 0");
+    constexpr int kOps = WIDE ? 2 : PassCfg<PASS>::kOps;
+    constexpr int kBK = WIDE ? 2 * dmpt::kBK : dmpt::kBK;          // these four shadow the namespace's
+    constexpr int kRowBytes = kBK * 2;
+    constexpr int kABytes = kTile * kRowBytes;
+    constexpr int kBBytes = kBRows * kRowBytes;
+    constexpr int kKbPerChunk = kChunkK / kBK;
     constexpr int kStages = PassCfg<PASS>::kStages;
     constexpr int kEpiWarp0 = Warps<PASS>::kEpi0;
     constexpr int kNumThreads = Warps<PASS>::kThreads;
@@ -550,7 +561,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
     const bool with_p0 = (PASS == 3 || PASS == 4) ? true : (PASS == 0 ? c.mode0 != MODE_FROZEN : (PASS == 1 || c.conv2 == 0));
     const bool with_p1 = (PASS == 3 || PASS == 4) ? true
                                    : (PASS == 0 ? p.pb.order >= 1 : (PASS == 1 || (p.pb.nfields >= 3 && c.conv3 == 0)));
-    const int nops = (with_p1 || PASS == 3) ? kOps : kOps - 2;    // the last operand pair only feeds accumulator 1
+    const int nops = WIDE ? 2 : ((with_p1 || PASS == 3) ? kOps : kOps - 2);    // the last operand pair only feeds accumulator 1
     unsigned int* wave_ctr = PASS == 0 ? &p.ctl->wave : (PASS == 4 ? &p.ctl->wave3 : &p.ctl->wave2);
 
     if (warp == 0 && lane == 0) {
@@ -594,7 +605,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
         {
             // staged operand pairs: PASS 0: M, S1;  PASS 1: M, S1, S2;  PASS 2: M, slot 2, slot 3;  PASS 4: M, S1, S2, S3
             const CUtensorMap* maps[8] = {
-                &p.maps[c.s0_buf][MH], &p.maps[c.s0_buf][ML],
+                &p.maps[c.s0_buf][WIDE ? S3H : MH], &p.maps[c.s0_buf][WIDE ? S3L : ML],
                 PASS == 2 ? &p.maps[c.s2_buf][S2H] : &p.maps[c.s1_buf][S1H],
                 PASS == 2 ? &p.maps[c.s2_buf][S2L] : &p.maps[c.s1_buf][S1L],
                 PASS == 2 ? &p.maps[c.s3_buf][S3H] : &p.maps[c.s2_buf][S2H],
@@ -669,7 +680,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                         tc_fence_after();
                         const uint32_t base = smem_base + stage * kStageBytes;
                         if (elect_one()) {
-                            uint64_t a[kOps], b[kOps];
+                            uint64_t a[kOps < 6 ? 6 : kOps], b[kOps < 6 ? 6 : kOps];
 #pragma unroll
                             for (int o = 0; o < kOps; ++o) {
                                 a[o] = make_smem_desc<kRowBytes>(base + o * kABytes);
@@ -697,7 +708,7 @@ dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
                                 auto cross = [&](uint32_t d, int yh, int yl) { cross2(d, PM_H, PM_L, yh, yl); };
                                 if (PASS == 0) {            // P0 = M.M, P1 = M.S1 + S1.M
                                     if (with_p0) square(d0, PM_H, PM_L);
-                                    if (with_p1) cross(d1, PY_H, PY_L);
+                                    if (!WIDE && with_p1) cross(d1, PY_H, PY_L);
                                 } else if (PASS == 3) {     // C = A.B^T: Ahi.Bhi + Ahi.Blo + Alo.Bhi, two column blocks
                                     umma_f16<2>(d0, a[PM_H] + adv, b[PY_H] + adv, idesc, accum);
                                     umma_f16<2>(d0, a[PM_H] + adv, b[PY_L] + adv, idesc, 1);

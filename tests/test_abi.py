@@ -70,7 +70,7 @@ def test_host_only_entry_points():
     o = p.dmpt_default_options()
     assert (o.max_layers, o.order, o.s0_shift, o.s1_autoscale, o.bounds, o.wave_sync, o.num_fields) == \
         (200, 1, -1, 1, 0, 1, 1)
-    assert list(o.reserved) == [0] * 2 and o.loop_graph == 0 and o.epilogue_direct == 0 and o.lanczos_steps == 0 and o.no_pdl == 0
+    assert list(o.reserved) == [0] * 1 and o.order0_narrow == 0 and o.loop_graph == 0 and o.epilogue_direct == 0 and o.lanczos_steps == 0 and o.no_pdl == 0
     assert p.dmpt_strerror(0) == "ok"
     for code in range(-7, 0):
         assert p.dmpt_strerror(code) not in ("ok", "unknown error code")

@@ -825,6 +825,21 @@ def test_ground_state_mode_matches_oracle(dev, cfg, n):
     assert r1.layers_d0 == res.layers and np.array_equal(e0, d0)
 
 
+@pytest.mark.parametrize("cfg,n", [(1, 200), (2, 1284), (4, 2304)])
+def test_ground_state_wide_k_blocks_are_bit_identical(dev, cfg, n):
+    """Order 0 runs the layer kernel's ground-state instantiation (64-column k-blocks, 128-byte operand rows, two staged
+    operands); `order0_narrow` keeps the general one.  Same k-steps in the same order: D0, the stop layer and every
+    per-layer record are equal bit for bit (n = 2304: 171 pair tiles, two waves)."""
+    from workloads import make_config
+
+    wl = make_config(cfg, n=n)
+    a, a0 = _run0(wl.h0, wl.n_occ, dev)
+    b, b0 = _run0(wl.h0, wl.n_occ, dev, order0_narrow=True)
+    assert a.status == 0 and b.status == 0 and a.layers == b.layers
+    assert np.array_equal(a0, b0)
+    assert a.sigma == b.sigma and a.tr_s == b.tr_s and a.tr_x == b.tr_x and a.id_err == b.id_err
+
+
 def test_finite_difference_of_ground_state_runs_gives_the_response(dev, config1):
     """PAPER.md:562-566 (Eq. 83): D1 ~ [D0(H0 + h H1) - D0(H0 - h H1)] / 2h.  Two order-0 runs against the
     order-1 run of the same library - the paper's own validation of the perturbation recursion (Fig. 5)."""
