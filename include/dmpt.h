@@ -87,7 +87,8 @@ typedef struct dmpt_options {
                        /* order 3).  0 (default): launches enqueued in chunks of 2-8 layers, two chunks ahead,      */
                        /* one pinned flag per chunk.  Same kernels, bit-identical results                           */
     int order0_narrow; /* order 0 only.  0 (default): the ground-state instantiation of the layer kernel, which stages  */
-                       /* its two operands in k-blocks of 64 columns (128-byte rows: half the TMA requests per byte);  */
+                       /* its two operands in k-blocks of 64 columns (128-byte rows: full stages, twice the bytes in   */
+                       /* flight);                                                                                     */
                        /* 1: the general instantiation with 32-column k-blocks (A/B measurements; same k-steps in the  */
                        /* same order, bit-identical results)                                                           */
     int reserved[1];   /* must be 0                                                                   */

@@ -475,10 +475,11 @@ __device__ __forceinline__ void final_epilogue_tma(const float (&acc)[kHalfCols]
 //         reads the operands of S0_{n-1}, S1_{n-1}, S2_{n-1} and the decision pass 0 of layer n-1 left in
 //         DmptCtl, writes S2_n into the other buffer and leaves ||V2||_F^2, max|S2_n| in partials2.
 // WIDE (PASS 0 at order 0 only): the ground-state instantiation.  It stages the two operands of M.M only, in k-blocks
-// of 64 columns - 128-byte operand rows, SWIZZLE_128B, through the tensor maps in slots S3H, S3L - in the same 48 KiB
-// per stage: half the TMA requests per byte.  With 64-byte rows order 0 asks the request path (one request per
-// operand row) for 1.5 x what first order does per MMA and the MMAs wait for it (item 6).  Same k16
-// steps in the same order: bit-identical results.
+// of 64 columns - 128-byte operand rows, SWIZZLE_128B, through the tensor maps in slots S3H, S3L - so that its 48 KiB
+// stages are full: twice the operand bytes in flight per CTA (3 x 40 KiB, as first order has) with half the TMA
+// instructions.  The general instantiation at order 0 fills half of every stage (60 KiB in flight) while asking for
+// 1.5 x first order's bytes per MMA, and the MMAs wait for the loads: tensor pipe 55 % against 89 % (DESIGN.md 12,
+// item 6).  Same k16 steps in the same order: bit-identical results.
 template <int PASS, bool WIDE = false>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(Warps<PASS>::kThreads, 1)
 dmpt_layer_kernel(const __grid_constant__ LayerParams p) {
